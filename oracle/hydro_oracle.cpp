@@ -1,0 +1,626 @@
+// hydro_oracle.cpp -- CPU ORACLE.  TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// A plain, slow, single-threaded restatement of the hot path of arxiv 1604.03360
+// ("Relativistic hydrodynamics on graphics processing units"): the spatial operator L(u) of
+// PAPER.md:17-20 Eq. (2), evaluated three times per third-order Runge-Kutta step
+// on a Cartesian grid of five conserved fields E, Mx, My, Mz, R with p = e/3.
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+// load this library.  It shares no source, header, table or helper with the CUDA path under
+// paper_1604_03360_b200/csrc/ and neither includes the other.
+//
+// The paper gives Eqs. (1)-(2) and names the schemes; every formula it does not print is taken
+// from SURVEY.md section 8(c) (items O1..O9, readings Q1..Q18, restated in DESIGN.md section 3).
+// Each function cites the item it follows.  No blocking, fusion or reordering: loops follow the
+// definitions so that they can be checked against SURVEY/DESIGN by eye.
+//
+// Parity pins (tests/test_oracle_*.py, all `-m "not gpu"`): con2prim round trip; wave speeds vs
+// numerical eigenvalues of dF/dU; WENO5/7 coefficients re-derived with exact rationals, linear
+// limit, orders 5/7; LLF and MUSTA consistency and scalar closed forms; SSP-RK3 stability
+// polynomial; uniform state, conservation, symmetry; exact Sod Riemann solution; d-dimensional
+// Hubble closed forms.  No function here is "parity unpinned".
+//
+// Build: g++ -O2 -std=c++17 -shared -fPIC -ffp-contract=off hydro_oracle.cpp -o liboracle_hydro.so
+// (-ffp-contract=off: no FMA contraction, the arithmetic is exactly what is written).
+
+#include <cmath>
+#include <cstddef>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+namespace {
+
+enum { WENO5 = 0, WENO7 = 1, MUSTA_FORCE = 2 };
+enum { BC_OUTFLOW = 0, BC_PERIODIC = 1, BC_HUBBLE = 2 };
+enum { OK = 0, EINVAL_ = -1, ENOMEM_ = -2, EUNPHYSICAL = -4 };
+enum { NF = 5 };  // E, Mx, My, Mz, R
+
+// ------------------------------------------------------------------------------------------
+// O1. conserved -> primitive, closed form for p = e/3 (reading Q16).
+//   s = sqrt(4E^2 - 3M^2); v_i = 3 M_i/(2E + s); e = 3(E-|M|)(E+|M|)/(s+E); p = e/3;
+//   n = R sqrt(1 - v^2).  Q16: clamp E >= 1e-300 and |M| <= (1-1e-12)E, raising a flag.
+template <class T>
+struct Prim {
+    T e, p, n, v[3];
+};
+
+template <class T>
+Prim<T> con2prim(const T u[NF], int* flag) {
+    T E = u[0], M[3] = {u[1], u[2], u[3]}, R = u[4];
+    if (!(E >= (T)1e-300)) {
+        E = (T)1e-300;
+        if (flag) *flag = 1;
+    }
+    T Mabs = std::sqrt(M[0] * M[0] + M[1] * M[1] + M[2] * M[2]);
+    const T lim = ((T)1 - (T)1e-12) * E;
+    if (Mabs > lim) {
+        const T sc = lim / Mabs;
+        for (int i = 0; i < 3; ++i) M[i] *= sc;
+        Mabs = lim;
+        if (flag) *flag = 1;
+    }
+    const T s = std::sqrt((T)4 * E * E - (T)3 * Mabs * Mabs);
+    Prim<T> w;
+    T v2 = 0;
+    for (int i = 0; i < 3; ++i) {
+        w.v[i] = (T)3 * M[i] / ((T)2 * E + s);
+        v2 += w.v[i] * w.v[i];
+    }
+    w.e = (T)3 * (E - Mabs) * (E + Mabs) / (s + E);
+    w.p = w.e / (T)3;
+    w.n = R * std::sqrt((T)1 - v2);
+    return w;
+}
+
+// ------------------------------------------------------------------------------------------
+// O2. directional characteristic speed, c_s^2 = 1/3:
+//   a_d = ( |v_d|(1-cs2) + cs sqrt((1-v^2)(1 - v_d^2 - (v^2 - v_d^2) cs2)) ) / (1 - v^2 cs2)
+template <class T>
+T signal_speed(const T v[3], int d) {
+    const T cs2 = (T)1 / (T)3;
+    const T cs = std::sqrt(cs2);
+    const T v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+    const T vd = v[d];
+    const T disc = ((T)1 - v2) * ((T)1 - vd * vd - (v2 - vd * vd) * cs2);
+    return (std::fabs(vd) * ((T)1 - cs2) + cs * std::sqrt(disc)) / ((T)1 - v2 * cs2);
+}
+
+// ------------------------------------------------------------------------------------------
+// a5. physical flux in direction d (SURVEY section 8 notation; PAPER.md:13 f_i(u)):
+//   F_E = M_d, F_{M_j} = M_j v_d + p delta_{jd}, F_R = R v_d.
+template <class T>
+void phys_flux(const T u[NF], const Prim<T>& w, int d, T F[NF]) {
+    F[0] = u[1 + d];
+    for (int j = 0; j < 3; ++j) F[1 + j] = u[1 + j] * w.v[d] + (j == d ? w.p : (T)0);
+    F[4] = u[4] * w.v[d];
+}
+
+// ------------------------------------------------------------------------------------------
+// O3. WENO5 (Jiang-Shu), value at i+1/2 from f_{i-2..i+2} = (a,b,c,d,e).
+template <class T>
+T weno5(const T f[5], T eps) {
+    const T a = f[0], b = f[1], c = f[2], d = f[3], e = f[4];
+    const T q0 = ((T)2 * a - (T)7 * b + (T)11 * c) / (T)6;
+    const T q1 = (-b + (T)5 * c + (T)2 * d) / (T)6;
+    const T q2 = ((T)2 * c + (T)5 * d - e) / (T)6;
+    const T t13 = (T)13 / (T)12, quarter = (T)1 / (T)4;
+    const T b0 = t13 * (a - 2 * b + c) * (a - 2 * b + c) + quarter * (a - 4 * b + 3 * c) * (a - 4 * b + 3 * c);
+    const T b1 = t13 * (b - 2 * c + d) * (b - 2 * c + d) + quarter * (b - d) * (b - d);
+    const T b2 = t13 * (c - 2 * d + e) * (c - 2 * d + e) + quarter * (3 * c - 4 * d + e) * (3 * c - 4 * d + e);
+    const T a0 = ((T)1 / (T)10) / ((eps + b0) * (eps + b0));
+    const T a1 = ((T)6 / (T)10) / ((eps + b1) * (eps + b1));
+    const T a2 = ((T)3 / (T)10) / ((eps + b2) * (eps + b2));
+    const T sum = a0 + a1 + a2;
+    return (a0 / sum) * q0 + (a1 / sum) * q1 + (a2 / sum) * q2;
+}
+
+// O4. WENO7 (Balsara-Shu), value at i+1/2 from f_{i-3..i+3} = (a..g).
+// The integer-coefficient forms are 240x the smoothness indicators.
+template <class T>
+T weno7(const T f[7], T eps) {
+    const T a = f[0], b = f[1], c = f[2], d = f[3], e = f[4], ff = f[5], g = f[6];
+    const T q0 = (-(T)3 * a + (T)13 * b - (T)23 * c + (T)25 * d) / (T)12;
+    const T q1 = (b - (T)5 * c + (T)13 * d + (T)3 * e) / (T)12;
+    const T q2 = (-c + (T)7 * d + (T)7 * e - ff) / (T)12;
+    const T q3 = ((T)3 * d + (T)13 * e - (T)5 * ff + g) / (T)12;
+    const T B0 = a * (547 * a - 3882 * b + 4642 * c - 1854 * d) + b * (7043 * b - 17246 * c + 7042 * d) +
+                 c * (11003 * c - 9402 * d) + 2107 * d * d;
+    const T B1 = b * (267 * b - 1642 * c + 1602 * d - 494 * e) + c * (2843 * c - 5966 * d + 1922 * e) +
+                 d * (3443 * d - 2522 * e) + 547 * e * e;
+    const T B2 = c * (547 * c - 2522 * d + 1922 * e - 494 * ff) + d * (3443 * d - 5966 * e + 1602 * ff) +
+                 e * (2843 * e - 1642 * ff) + 267 * ff * ff;
+    const T B3 = d * (2107 * d - 9402 * e + 7042 * ff - 1854 * g) + e * (11003 * e - 17246 * ff + 4642 * g) +
+                 ff * (7043 * ff - 3882 * g) + 547 * g * g;
+    const T be[4] = {B0 / (T)240, B1 / (T)240, B2 / (T)240, B3 / (T)240};
+    const T dl[4] = {(T)1 / (T)35, (T)12 / (T)35, (T)18 / (T)35, (T)4 / (T)35};
+    const T q[4] = {q0, q1, q2, q3};
+    T al[4], sum = 0;
+    for (int k = 0; k < 4; ++k) {
+        al[k] = dl[k] / ((eps + be[k]) * (eps + be[k]));
+        sum += al[k];
+    }
+    T r = 0;
+    for (int k = 0; k < 4; ++k) r += (al[k] / sum) * q[k];
+    return r;
+}
+
+// ------------------------------------------------------------------------------------------
+// O5. component-wise local Lax-Friedrichs WENO flux at i+1/2, direction d.
+//   cells[k], k = 0..2r-1, are u_{i-r+1} .. u_{i+r}.
+//   alpha = max_k a_d(cells[k]);  f+-_k = (F_d(u_k) +- alpha u_k)/2;
+//   fhat = WENO(f+ on i-r+1..i+r-1) + WENO(f- on the mirrored stencil i+r..i-r+2).
+template <class T>
+void llf_weno_split(int r, const T cells[][NF], const T F[][NF], const T a[], T eps, T fhat[NF]) {
+    const int m = 2 * r;
+    T alpha = a[0];
+    for (int k = 1; k < m; ++k) alpha = std::fmax(alpha, a[k]);
+    for (int c = 0; c < NF; ++c) {
+        T fp[7], fm[7];
+        for (int k = 0; k < 2 * r - 1; ++k) {
+            fp[k] = (F[k][c] + alpha * cells[k][c]) / (T)2;                   // i-r+1 .. i+r-1
+            fm[k] = (F[m - 1 - k][c] - alpha * cells[m - 1 - k][c]) / (T)2;   // i+r .. i-r+2
+        }
+        fhat[c] = (r == 3) ? weno5(fp, eps) + weno5(fm, eps) : weno7(fp, eps) + weno7(fm, eps);
+    }
+}
+
+// the same, starting from the conserved cells only (a2, a3, a5 done per cell first)
+template <class T>
+void llf_weno_flux(int r, const T cells[][NF], int d, T eps, T fhat[NF], int* flag) {
+    T F[8][NF], a[8];
+    for (int k = 0; k < 2 * r; ++k) {
+        const Prim<T> w = con2prim(cells[k], flag);
+        phys_flux(cells[k], w, d, F[k]);
+        a[k] = signal_speed(w.v, d);
+    }
+    llf_weno_split(r, cells, F, a, eps, fhat);
+}
+
+// ------------------------------------------------------------------------------------------
+// O6. MUSCL with minmod on the conserved variables.
+template <class T>
+T minmod(T a, T b) {
+    if (a * b <= (T)0) return (T)0;
+    return (a > 0 ? (T)1 : (T)-1) * std::fmin(std::fabs(a), std::fabs(b));
+}
+
+// O7. MUSTA-FORCE flux, K stages.
+//   cells[0..3] = u_{i-1}, u_i, u_{i+1}, u_{i+2}.  tau = C/S, S = max(a_d(Q_L), a_d(Q_R)) per stage.
+template <class T>
+void musta_force_flux(const T cells[4][NF], int d, int K, T C, T fstar[NF], int* flag) {
+    T QL[NF], QR[NF];
+    for (int c = 0; c < NF; ++c) {
+        const T di = minmod(cells[1][c] - cells[0][c], cells[2][c] - cells[1][c]);
+        const T dip = minmod(cells[2][c] - cells[1][c], cells[3][c] - cells[2][c]);
+        QL[c] = cells[1][c] + di / (T)2;
+        QR[c] = cells[2][c] - dip / (T)2;
+    }
+    for (int stage = 1;; ++stage) {
+        const Prim<T> wl = con2prim(QL, flag), wr = con2prim(QR, flag);
+        T FL[NF], FR[NF], QM[NF], FM[NF];
+        phys_flux(QL, wl, d, FL);
+        phys_flux(QR, wr, d, FR);
+        const T S = std::fmax(signal_speed(wl.v, d), signal_speed(wr.v, d));
+        const T tau = C / S;
+        for (int c = 0; c < NF; ++c) QM[c] = (QL[c] + QR[c]) / (T)2 - tau * (FR[c] - FL[c]) / (T)2;
+        const Prim<T> wm = con2prim(QM, flag);
+        phys_flux(QM, wm, d, FM);
+        for (int c = 0; c < NF; ++c)
+            fstar[c] = (FL[c] + (T)2 * FM[c] + FR[c] - (QR[c] - QL[c]) / tau) / (T)4;
+        if (stage == K) return;
+        for (int c = 0; c < NF; ++c) {
+            QL[c] = QL[c] - tau * (fstar[c] - FL[c]);
+            QR[c] = QR[c] - tau * (FR[c] - fstar[c]);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Grid solver: ghost fill (a1), L(u) (a2..a8), SSP-RK3 (a9), max signal speed (a4).
+template <class T>
+struct Solver {
+    int n[3];      // nx, ny, nz
+    int g[3];      // ghost width per axis (0 on an inactive axis, n == 1)
+    int np[3];     // padded extents
+    int scheme, r; // r = stencil half-width = ghost width on active axes (3 / 4 / 2)
+    double dx;
+    int bc[3] = {BC_OUTFLOW, BC_OUTFLOW, BC_OUTFLOW};
+    double eps = 1e-6, musta_cfl = 0.9, t = 0.0;
+    int musta_stages = 2;
+    double origin[3] = {0, 0, 0};
+    double hub_t0 = 1, hub_e0 = 1, hub_n0 = 1, hub_b[3] = {0, 0, 0};
+    int flag = 0;
+    std::vector<T> u;  // padded state, [5][npz][npy][npx]
+
+    Solver(int nx, int ny, int nz, double dx_, int scheme_) : scheme(scheme_), dx(dx_) {
+        n[0] = nx; n[1] = ny; n[2] = nz;
+        r = scheme == WENO5 ? 3 : scheme == WENO7 ? 4 : 2;
+        for (int a = 0; a < 3; ++a) {
+            g[a] = n[a] > 1 ? r : 0;
+            np[a] = n[a] + 2 * g[a];
+        }
+        u.assign((size_t)NF * np[0] * np[1] * np[2], (T)0);
+    }
+    size_t ncell_pad() const { return (size_t)np[0] * np[1] * np[2]; }
+    size_t ncell() const { return (size_t)n[0] * n[1] * n[2]; }
+    // index of padded cell (i,j,k), each in [-g, n+g)
+    size_t pidx(int i, int j, int k) const {
+        return ((size_t)(k + g[2]) * np[1] + (size_t)(j + g[1])) * np[0] + (size_t)(i + g[0]);
+    }
+    void load(const std::vector<T>& pad, int i, int j, int k, T out[NF]) const {
+        const size_t s = ncell_pad(), p = pidx(i, j, k);
+        for (int c = 0; c < NF; ++c) out[c] = pad[c * s + p];
+    }
+
+    // exact d-dimensional Hubble state at a cell centre and time tt:
+    // Hubble axes = axes whose BC is BC_HUBBLE; d = their number;
+    // v_i = x_i/t, tau^2 = t^2 - sum x_i^2, e = e0 (t0/tau)^(4d/3), n = n0 (t0/tau)^d exp(-s/2),
+    // s = sum (x_i/t)^2 / b_i^2 over Hubble axes with b_i > 0.  Returned as conserved variables.
+    void hubble_cons(int i, int j, int k, double tt, T out[NF]) const {
+        const int ix[3] = {i, j, k};
+        double r2 = 0, s = 0, v[3] = {0, 0, 0};
+        int d = 0;
+        for (int a = 0; a < 3; ++a) {
+            if (bc[a] != BC_HUBBLE) continue;
+            const double x = origin[a] + (ix[a] + 0.5) * dx;
+            ++d;
+            r2 += x * x;
+            v[a] = x / tt;
+            if (hub_b[a] > 0) s += (x / tt) * (x / tt) / (hub_b[a] * hub_b[a]);
+        }
+        const double tau = std::sqrt(tt * tt - r2);
+        const double e = hub_e0 * std::pow(hub_t0 / tau, 4.0 * d / 3.0);
+        const double nn = hub_n0 * std::pow(hub_t0 / tau, (double)d) * std::exp(-0.5 * s);
+        const double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+        const double g2 = 1.0 / (1.0 - v2), p = e / 3.0, w = (e + p) * g2;
+        out[0] = (T)(w - p);
+        for (int a = 0; a < 3; ++a) out[1 + a] = (T)(w * v[a]);
+        out[4] = (T)(nn * std::sqrt(g2));
+    }
+
+    // a1. ghost fill of a padded array at time tt: face ghosts only, axis by axis.
+    // outflow: copy the nearest interior cell into every ghost layer; periodic: wrap;
+    // Hubble: closed form at the ghost cell centre.
+    void fill_ghosts(std::vector<T>& pad, double tt) const {
+        const size_t s = ncell_pad();
+        for (int a = 0; a < 3; ++a) {
+            if (g[a] == 0) continue;
+            const int a1 = (a + 1) % 3, a2 = (a + 2) % 3;
+            for (int q2 = 0; q2 < n[a2]; ++q2)
+                for (int q1 = 0; q1 < n[a1]; ++q1)
+                    for (int l = 1; l <= g[a]; ++l)
+                        for (int side = 0; side < 2; ++side) {
+                            int ix[3], src[3];
+                            ix[a1] = src[a1] = q1;
+                            ix[a2] = src[a2] = q2;
+                            ix[a] = side == 0 ? -l : n[a] - 1 + l;
+                            T val[NF];
+                            if (bc[a] == BC_HUBBLE) {
+                                hubble_cons(ix[0], ix[1], ix[2], tt, val);
+                            } else {
+                                if (bc[a] == BC_PERIODIC)
+                                    src[a] = side == 0 ? n[a] - l : l - 1;
+                                else
+                                    src[a] = side == 0 ? 0 : n[a] - 1;
+                                load(pad, src[0], src[1], src[2], val);
+                            }
+                            const size_t p = pidx(ix[0], ix[1], ix[2]);
+                            for (int c = 0; c < NF; ++c) pad[c * s + p] = val[c];
+                        }
+        }
+    }
+
+    // interface flux at the upper face of cell (i,j,k) along axis a; the index along a may be -1.
+    // prim/spd hold the per-cell results of a2/a3 for the whole padded array (WENO path only).
+    void iface_flux(const std::vector<T>& pad, const std::vector<Prim<T>>& prim, int i, int j, int k,
+                    int a, T fh[NF]) {
+        const int ix[3] = {i, j, k};
+        if (scheme == MUSTA_FORCE) {
+            T cells[4][NF];
+            for (int m = 0; m < 4; ++m) {
+                int jx[3] = {ix[0], ix[1], ix[2]};
+                jx[a] += m - 1;
+                load(pad, jx[0], jx[1], jx[2], cells[m]);
+            }
+            musta_force_flux<T>(cells, a, musta_stages, (T)musta_cfl, fh, &flag);
+        } else {
+            T cells[8][NF], F[8][NF], sp[8];
+            for (int m = 0; m < 2 * r; ++m) {
+                int jx[3] = {ix[0], ix[1], ix[2]};
+                jx[a] += m - r + 1;
+                load(pad, jx[0], jx[1], jx[2], cells[m]);
+                const Prim<T>& w = prim[pidx(jx[0], jx[1], jx[2])];
+                phys_flux(cells[m], w, a, F[m]);
+                sp[m] = signal_speed(w.v, a);
+            }
+            llf_weno_split<T>(r, cells, F, sp, (T)eps, fh);
+        }
+    }
+
+    // a2..a8. L(u) of Eq. (2): L = sum_d (fhat_{i-1/2,d} - fhat_{i+1/2,d})/dx over
+    // the active axes, in the order x, y, z.  `pad` must have its ghosts filled.  Lout is interior.
+    // Step 1: con2prim of every padded cell that a sweep can touch (face ghosts; the unused edge and
+    // corner ghosts hold zeros and are skipped).  Step 2: per axis, every interface flux once.
+    // Step 3: the difference of the two faces of each cell.
+    void eval_L(const std::vector<T>& pad, std::vector<T>& Lout) {
+        const size_t N = ncell();
+        Lout.assign(NF * N, (T)0);
+        std::vector<Prim<T>> prim;
+        if (scheme != MUSTA_FORCE) {
+            prim.resize(ncell_pad());
+            for (int k = -g[2]; k < n[2] + g[2]; ++k)
+                for (int j = -g[1]; j < n[1] + g[1]; ++j)
+                    for (int i = -g[0]; i < n[0] + g[0]; ++i) {
+                        const int out = (i < 0 || i >= n[0]) + (j < 0 || j >= n[1]) + (k < 0 || k >= n[2]);
+                        if (out > 1) continue;
+                        T c[NF];
+                        load(pad, i, j, k, c);
+                        prim[pidx(i, j, k)] = con2prim(c, &flag);
+                    }
+        }
+        for (int a = 0; a < 3; ++a) {
+            if (g[a] == 0) continue;
+            // fh[q] = flux at the upper face along a of the cell whose a-index is shifted by -1:
+            // faces are indexed -1 .. n[a]-1 along a, interior along the other axes.
+            int m[3] = {n[0], n[1], n[2]};
+            m[a] += 1;
+            std::vector<T> fh((size_t)NF * m[0] * m[1] * m[2]);
+            for (int k = 0; k < m[2]; ++k)
+                for (int j = 0; j < m[1]; ++j)
+                    for (int i = 0; i < m[0]; ++i) {
+                        int ix[3] = {i, j, k};
+                        ix[a] -= 1;
+                        T f[NF];
+                        iface_flux(pad, prim, ix[0], ix[1], ix[2], a, f);
+                        for (int c = 0; c < NF; ++c) fh[(((size_t)k * m[1] + j) * m[0] + i) * NF + c] = f[c];
+                    }
+            for (int k = 0; k < n[2]; ++k)
+                for (int j = 0; j < n[1]; ++j)
+                    for (int i = 0; i < n[0]; ++i) {
+                        const size_t q = ((size_t)k * n[1] + j) * n[0] + i;
+                        int up[3] = {i, j, k};
+                        up[a] += 1;
+                        const T* fm = &fh[(((size_t)k * m[1] + j) * m[0] + i) * NF];
+                        const T* fp = &fh[(((size_t)up[2] * m[1] + up[1]) * m[0] + up[0]) * NF];
+                        for (int c = 0; c < NF; ++c) Lout[c * N + q] += (fm[c] - fp[c]) / (T)dx;
+                    }
+        }
+    }
+
+    void set_interior(std::vector<T>& pad, const T* in) const {
+        const size_t N = ncell(), s = ncell_pad();
+        for (int c = 0; c < NF; ++c)
+            for (int k = 0; k < n[2]; ++k)
+                for (int j = 0; j < n[1]; ++j)
+                    for (int i = 0; i < n[0]; ++i)
+                        pad[c * s + pidx(i, j, k)] = in[c * N + ((size_t)k * n[1] + j) * n[0] + i];
+    }
+    void get_interior(const std::vector<T>& pad, T* out) const {
+        const size_t N = ncell(), s = ncell_pad();
+        for (int c = 0; c < NF; ++c)
+            for (int k = 0; k < n[2]; ++k)
+                for (int j = 0; j < n[1]; ++j)
+                    for (int i = 0; i < n[0]; ++i)
+                        out[c * N + ((size_t)k * n[1] + j) * n[0] + i] = pad[c * s + pidx(i, j, k)];
+    }
+
+    // L of an interior state given by the caller, ghosts filled at time tt.
+    void eval_L_interior(const T* in, double tt, T* Lout_) {
+        std::vector<T> pad(u.size(), (T)0), L;
+        set_interior(pad, in);
+        fill_ghosts(pad, tt);
+        eval_L(pad, L);
+        std::memcpy(Lout_, L.data(), L.size() * sizeof(T));
+    }
+
+    // a9 / O8. Shu-Osher SSP-RK3 (Q1), stage times t, t+dt, t+dt/2:
+    //   u1 = u + dt L(u);  u2 = 3/4 u + 1/4 (u1 + dt L(u1));  u_new = 1/3 u + 2/3 (u2 + dt L(u2)).
+    void step(double dt) {
+        const size_t s = ncell_pad(), N = ncell();
+        std::vector<T> L, u1(u.size(), (T)0), u2(u.size(), (T)0);
+        const T h = (T)dt;
+        fill_ghosts(u, t);
+        eval_L(u, L);
+        for (int c = 0; c < NF; ++c) for (int k = 0; k < n[2]; ++k) for (int j = 0; j < n[1]; ++j) for (int i = 0; i < n[0]; ++i) {
+            const size_t p = c * s + pidx(i, j, k), q = c * N + ((size_t)k * n[1] + j) * n[0] + i;
+            u1[p] = u[p] + h * L[q];
+        }
+        fill_ghosts(u1, t + dt);
+        eval_L(u1, L);
+        for (int c = 0; c < NF; ++c) for (int k = 0; k < n[2]; ++k) for (int j = 0; j < n[1]; ++j) for (int i = 0; i < n[0]; ++i) {
+            const size_t p = c * s + pidx(i, j, k), q = c * N + ((size_t)k * n[1] + j) * n[0] + i;
+            u2[p] = (T)3 / (T)4 * u[p] + (T)1 / (T)4 * (u1[p] + h * L[q]);
+        }
+        fill_ghosts(u2, t + 0.5 * dt);
+        eval_L(u2, L);
+        for (int c = 0; c < NF; ++c) for (int k = 0; k < n[2]; ++k) for (int j = 0; j < n[1]; ++j) for (int i = 0; i < n[0]; ++i) {
+            const size_t p = c * s + pidx(i, j, k), q = c * N + ((size_t)k * n[1] + j) * n[0] + i;
+            u[p] = (T)1 / (T)3 * u[p] + (T)2 / (T)3 * (u2[p] + h * L[q]);
+        }
+        t += dt;
+    }
+
+    // a4. max over interior cells and active axes of a_d.
+    double max_signal_speed() {
+        double m = 0;
+        for (int k = 0; k < n[2]; ++k)
+            for (int j = 0; j < n[1]; ++j)
+                for (int i = 0; i < n[0]; ++i) {
+                    T c[NF];
+                    load(u, i, j, k, c);
+                    const Prim<T> w = con2prim(c, &flag);
+                    for (int a = 0; a < 3; ++a)
+                        if (g[a] > 0) m = std::fmax(m, (double)signal_speed(w.v, a));
+                }
+        return m;
+    }
+};
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// C ABI (host pointers everywhere).  Mirrors include/hydro.h with the prefix oracle_.
+struct oracle_ctx {
+    int precision = 0;  // 0 = f64, 1 = f32 (Q17 diagnostic)
+    int nx, ny, nz, scheme;
+    double dx;
+    Solver<double>* d = nullptr;
+    Solver<float>* f = nullptr;
+};
+
+#define BOTH(ctx, stmt)                                   \
+    do {                                                  \
+        if ((ctx)->d) { auto* S = (ctx)->d; stmt; }       \
+        if ((ctx)->f) { auto* S = (ctx)->f; stmt; }       \
+    } while (0)
+
+extern "C" {
+
+int oracle_create(oracle_ctx** out, int nx, int ny, int nz, double dx, int scheme) {
+    if (!out || nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || scheme < 0 || scheme > 2) return EINVAL_;
+    oracle_ctx* c = new oracle_ctx;
+    c->nx = nx; c->ny = ny; c->nz = nz; c->dx = dx; c->scheme = scheme;
+    c->d = new Solver<double>(nx, ny, nz, dx, scheme);
+    *out = c;
+    return OK;
+}
+
+void oracle_destroy(oracle_ctx* c) {
+    if (!c) return;
+    delete c->d;
+    delete c->f;
+    delete c;
+}
+
+int oracle_set_option(oracle_ctx* c, const char* key, double v) {
+    if (!c || !key) return EINVAL_;
+    const std::string k(key);
+    if (k == "precision") {
+        const int p = (int)v;
+        if (p != 0 && p != 1) return EINVAL_;
+        if (p == c->precision) return OK;
+        // switching precision re-creates the solver; options set earlier are carried over
+        if (p == 1) {
+            auto* S = new Solver<float>(c->nx, c->ny, c->nz, c->dx, c->scheme);
+            auto* D = c->d;
+            for (int a = 0; a < 3; ++a) { S->bc[a] = D->bc[a]; S->origin[a] = D->origin[a]; S->hub_b[a] = D->hub_b[a]; }
+            S->eps = D->eps; S->musta_cfl = D->musta_cfl; S->musta_stages = D->musta_stages; S->t = D->t;
+            S->hub_t0 = D->hub_t0; S->hub_e0 = D->hub_e0; S->hub_n0 = D->hub_n0;
+            delete c->d; c->d = nullptr; c->f = S;
+        } else {
+            auto* S = new Solver<double>(c->nx, c->ny, c->nz, c->dx, c->scheme);
+            auto* D = c->f;
+            for (int a = 0; a < 3; ++a) { S->bc[a] = D->bc[a]; S->origin[a] = D->origin[a]; S->hub_b[a] = D->hub_b[a]; }
+            S->eps = D->eps; S->musta_cfl = D->musta_cfl; S->musta_stages = D->musta_stages; S->t = D->t;
+            S->hub_t0 = D->hub_t0; S->hub_e0 = D->hub_e0; S->hub_n0 = D->hub_n0;
+            delete c->f; c->f = nullptr; c->d = S;
+        }
+        c->precision = p;
+        return OK;
+    }
+    int rc = OK;
+    BOTH(c, {
+        if (k == "bc_x" || k == "bc_y" || k == "bc_z") {
+            const int b = (int)v;
+            if (b < 0 || b > 2) rc = EINVAL_; else S->bc[k[3] - 'x'] = b;
+        } else if (k == "musta_stages") { if (v < 1) rc = EINVAL_; else S->musta_stages = (int)v; }
+        else if (k == "musta_cfl") { if (!(v > 0)) rc = EINVAL_; else S->musta_cfl = v; }
+        else if (k == "weno_eps") { if (!(v > 0)) rc = EINVAL_; else S->eps = v; }
+        else if (k == "t") S->t = v;
+        else if (k == "x0") S->origin[0] = v;
+        else if (k == "y0") S->origin[1] = v;
+        else if (k == "z0") S->origin[2] = v;
+        else if (k == "hubble_t0") S->hub_t0 = v;
+        else if (k == "hubble_e0") S->hub_e0 = v;
+        else if (k == "hubble_n0") S->hub_n0 = v;
+        else if (k == "hubble_bx") S->hub_b[0] = v;
+        else if (k == "hubble_by") S->hub_b[1] = v;
+        else if (k == "hubble_bz") S->hub_b[2] = v;
+        else rc = EINVAL_;
+    });
+    return rc;
+}
+
+int oracle_set_state(oracle_ctx* c, const void* cons) {
+    if (!c || !cons) return EINVAL_;
+    if (c->d) c->d->set_interior(c->d->u, (const double*)cons);
+    if (c->f) c->f->set_interior(c->f->u, (const float*)cons);
+    BOTH(c, S->flag = 0);
+    return OK;
+}
+
+int oracle_get_state(oracle_ctx* c, void* out) {
+    if (!c || !out) return EINVAL_;
+    if (c->d) c->d->get_interior(c->d->u, (double*)out);
+    if (c->f) c->f->get_interior(c->f->u, (float*)out);
+    return OK;
+}
+
+int oracle_step(oracle_ctx* c, double dt, int nsteps) {
+    if (!c || nsteps < 0 || !(dt > 0)) return EINVAL_;
+    int flag = 0;
+    for (int s = 0; s < nsteps; ++s) BOTH(c, S->step(dt));
+    BOTH(c, flag |= S->flag);
+    return flag ? EUNPHYSICAL : OK;
+}
+
+int oracle_max_signal_speed(oracle_ctx* c, double* out) {
+    if (!c || !out) return EINVAL_;
+    BOTH(c, *out = S->max_signal_speed());
+    return OK;
+}
+
+int oracle_get_time(oracle_ctx* c, double* out) {
+    if (!c || !out) return EINVAL_;
+    BOTH(c, *out = S->t);
+    return OK;
+}
+
+// L(u) of a caller-supplied interior state with ghosts filled at time t_stage (one RK stage's
+// spatial operator; used for the per-stage parity bound of BASELINE.json north_star).
+int oracle_eval_L(oracle_ctx* c, const void* cons, double t_stage, void* L_out) {
+    if (!c || !cons || !L_out) return EINVAL_;
+    if (c->d) c->d->eval_L_interior((const double*)cons, t_stage, (double*)L_out);
+    if (c->f) c->f->eval_L_interior((const float*)cons, t_stage, (float*)L_out);
+    return OK;
+}
+
+// ---- pointwise pieces exported for the pins (fp64) -------------------------------------------
+// prim_out = e, p, n, vx, vy, vz.  Returns 1 if the Q16 clamp fired.
+int oracle_con2prim(const double u[5], double prim_out[6]) {
+    int flag = 0;
+    const Prim<double> w = con2prim<double>(u, &flag);
+    prim_out[0] = w.e; prim_out[1] = w.p; prim_out[2] = w.n;
+    prim_out[3] = w.v[0]; prim_out[4] = w.v[1]; prim_out[5] = w.v[2];
+    return flag;
+}
+double oracle_signal_speed(const double v[3], int d) { return signal_speed<double>(v, d); }
+void oracle_phys_flux(const double u[5], int d, double F[5]) {
+    int flag = 0;
+    const Prim<double> w = con2prim<double>(u, &flag);
+    phys_flux<double>(u, w, d, F);
+}
+double oracle_weno5(const double f[5], double eps) { return weno5<double>(f, eps); }
+double oracle_weno7(const double f[7], double eps) { return weno7<double>(f, eps); }
+double oracle_minmod(double a, double b) { return minmod<double>(a, b); }
+// cells: [2r][5] row-major, u_{i-r+1}..u_{i+r}; r = 3 (WENO5) or 4 (WENO7)
+int oracle_llf_weno_flux(int r, const double* cells, int d, double eps, double fhat[5]) {
+    if (r != 3 && r != 4) return EINVAL_;
+    double cc[8][NF];
+    std::memcpy(cc, cells, sizeof(double) * 2 * r * NF);
+    int flag = 0;
+    llf_weno_flux<double>(r, cc, d, eps, fhat, &flag);
+    return flag;
+}
+// cells: [4][5] row-major, u_{i-1}..u_{i+2}
+int oracle_musta_force_flux(const double* cells, int d, int K, double C, double fstar[5]) {
+    double cc[4][NF];
+    std::memcpy(cc, cells, sizeof(cc));
+    int flag = 0;
+    musta_force_flux<double>(cc, d, K, C, fstar, &flag);
+    return flag;
+}
+
+}  // extern "C"
