@@ -1,0 +1,140 @@
+/* hydro.h -- C ABI of libhydro_b200: the data-parallel hot path of arxiv 1604.03360
+ * ("Relativistic hydrodynamics on graphics processing units") on NVIDIA B200 (sm_100a).
+ *
+ * What the library computes (citations are PAPER.md lines, i.e. the paper's text):
+ *   - the conservative system of Eq. (1), for five fields E, M_x, M_y, M_z, R
+ *     (energy, momenta, conserved charge) with the equation of state p = e/3;
+ *   - the method-of-lines operator L(u) of Eq. (2): for every cell the sum over the
+ *     active axes of (f(x - e_i/2) - f(x + e_i/2)) / |e_i| with interface fluxes from
+ *       WENO5 / WENO7 finite-difference reconstruction (section 1.2) on local
+ *       Lax-Friedrichs split fluxes, or
+ *       MUSTA-FORCE with MUSCL/minmod (section 1.1);
+ *   - the "standard, third order Runge-Kutta" of PAPER.md:20 (Shu-Osher SSP-RK3): three L(u) per step.
+ * Everything the paper does not print (EOS, splitting, wave speeds, epsilon, ghost rules) follows the
+ * readings Q1..Q18 listed in DESIGN.md section 3.
+ *
+ * Conventions
+ *   - Every function returns a status (HYDRO_OK = 0 or a negative HYDRO_E*); nothing throws or aborts.
+ *     hydro_last_error() gives a text for the last failure on that context.
+ *   - "device pointer" = CUDA device memory owned by the caller (e.g. torch.empty(..., device="cuda")
+ *     .data_ptr()); "host pointer" = ordinary host memory owned by the caller.  The library never frees
+ *     or keeps a caller buffer beyond the call, except the workspace bound with hydro_bind_workspace,
+ *     which must stay alive until hydro_destroy or the next bind.
+ *   - State layout at the boundary: interior cells only, [5][nz][ny][nx], x fastest, field order
+ *     E, M_x, M_y, M_z, R; element type double (HYDRO_F64) or float (HYDRO_F32) per "precision".
+ *     Ghost cells are internal to the library.
+ *   - An axis with n = 1 is inactive: no sweep, no ghosts, not part of the max signal speed.  This is
+ *     how the 1+1D shock tube runs as 400 x 1 x 1.
+ *   - All work is enqueued on the stream set with hydro_set_stream (default: the legacy default
+ *     stream).  Calls that return data to the host synchronise that stream; the others are
+ *     asynchronous.  One context per stream; a context is not thread-safe.
+ *   - There is no CPU fallback anywhere: without a CUDA device every compute call fails with
+ *     HYDRO_ECUDA.
+ */
+#ifndef HYDRO_B200_H
+#define HYDRO_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hydro_ctx hydro_ctx; /* opaque, owned by the library */
+
+enum { HYDRO_WENO5 = 0, HYDRO_WENO7 = 1, HYDRO_MUSTA_FORCE = 2 };          /* scheme            */
+enum { HYDRO_BC_OUTFLOW = 0, HYDRO_BC_PERIODIC = 1, HYDRO_BC_HUBBLE = 2 }; /* per axis          */
+enum { HYDRO_F64 = 0, HYDRO_F32 = 1 };                                     /* "precision"       */
+enum { HYDRO_KERNEL_AUTO = 0, HYDRO_KERNEL_GENERIC = 1, HYDRO_KERNEL_FUSED = 2 }; /* "kernel"   */
+enum {
+    HYDRO_OK = 0,
+    HYDRO_EINVAL = -1,      /* bad argument, unknown option, call out of order                   */
+    HYDRO_ENOMEM = -2,      /* workspace missing or too small                                    */
+    HYDRO_ECUDA = -3,       /* a CUDA runtime call or kernel launch failed (text in last_error)  */
+    HYDRO_EUNPHYSICAL = -4  /* con2prim had to clamp a cell (E < 1e-300 or |M| > (1-1e-12) E)    */
+};
+
+/* Create a context for an nx x ny x nz grid of spacing dx (same on all axes, the |e_i| of Eq. (2),
+ * PAPER.md:17-20) and one of the three schemes.  Allocates no device memory.  Ghost width on active
+ * axes: 3 (WENO5), 4 (WENO7), 2 (MUSTA-FORCE).  EINVAL for n < 1, dx <= 0, unknown scheme, or an
+ * active axis shorter than the ghost width. */
+int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme);
+
+/* Set an option.  Must precede hydro_bind_workspace for "precision" (it changes the workspace size).
+ *   "precision"     HYDRO_F64 (default) | HYDRO_F32: arithmetic and storage type of the whole path
+ *   "bc_x|bc_y|bc_z" boundary rule per axis (default outflow = copy the nearest interior cell)
+ *   "weno_eps"      epsilon of the WENO weights (default 1e-6, reading Q5)
+ *   "musta_stages"  K of MUSTA-FORCE (default 2, reading Q8);  "musta_cfl" its local Courant number
+ *                   (default 0.9, reading Q7)
+ *   "t"             current time (used by the analytic Hubble ghost fill)
+ *   "x0|y0|z0"      coordinate of the low face of the domain on each axis
+ *   "hubble_t0|hubble_e0|hubble_n0|hubble_bx|hubble_by|hubble_bz"  parameters of the closed-form
+ *                   Hubble flow used by HYDRO_BC_HUBBLE (readings Q13, Q14)
+ *   "kernel"        HYDRO_KERNEL_AUTO (default: fused stage kernel where the grid allows, else the
+ *                   generic one) | HYDRO_KERNEL_GENERIC | HYDRO_KERNEL_FUSED (EINVAL at step time if
+ *                   the grid does not allow it)
+ * EINVAL for an unknown key or a value out of range. */
+int hydro_set_option(hydro_ctx *ctx, const char *key, double value);
+
+/* cuda_stream: a cudaStream_t passed as void* (torch.cuda.current_stream().cuda_stream); NULL = the
+ * legacy default stream. */
+int hydro_set_stream(hydro_ctx *ctx, void *cuda_stream);
+
+/* Bytes of device memory the context needs for its padded state copies (three: u^n and two RK stage
+ * buffers), the per-cell primitive arrays and a small control block. */
+size_t hydro_workspace_bytes(const hydro_ctx *ctx);
+
+/* Hand the context its device memory (256-byte aligned, at least hydro_workspace_bytes()).  The caller
+ * keeps ownership.  ENOMEM if too small, EINVAL if misaligned.  Zero-fills it on the stream. */
+int hydro_bind_workspace(hydro_ctx *ctx, void *device_ptr, size_t bytes);
+
+/* Copy the interior conserved state in from / out to a DEVICE pointer ([5][nz][ny][nx], element type
+ * per "precision").  Asynchronous on the stream.  set_state also clears the unphysical flag. */
+int hydro_set_state(hydro_ctx *ctx, const void *cons_device);
+int hydro_get_state(hydro_ctx *ctx, void *cons_device_out);
+
+/* The same through HOST pointers: the library stages through the first RK buffer with
+ * cudaMemcpyAsync and synchronises the stream before returning.  These are the end-to-end entry points
+ * (bench.py "e2e"). */
+int hydro_set_state_host(hydro_ctx *ctx, const void *cons_host);
+int hydro_get_state_host(hydro_ctx *ctx, void *cons_host_out);
+
+/* Advance nsteps SSP-RK3 steps of fixed size dt (per stage: ghost fill, con2prim +
+ * signal speeds, L(u) of Eq. (2) fused with the Runge-Kutta combination).  Asynchronous. */
+int hydro_step(hydro_ctx *ctx, double dt, int nsteps);
+
+/* The same with dt = cfl * dx / (max signal speed of the state at the start of each step), the
+ * maximum taken on the device by the stage-1 con2prim kernel: no host synchronisation (reading Q10).
+ * Asynchronous. */
+int hydro_step_cfl(hydro_ctx *ctx, double cfl, int nsteps);
+
+/* max over interior cells and active axes of the characteristic speed a_d (a3-a4).
+ * Writes one double to a HOST pointer; synchronises the stream. */
+int hydro_max_signal_speed(hydro_ctx *ctx, double *out_host);
+
+/* L(u) of Eq. (2) for a caller-supplied interior state (DEVICE pointers, same layout as the state)
+ * with ghosts filled at time t_stage: one Runge-Kutta stage's spatial operator, for per-stage parity.
+ * Uses the RK stage buffers as scratch; the context's own state u^n is left untouched. */
+int hydro_eval_L(hydro_ctx *ctx, const void *cons_device, double t_stage, void *L_device_out);
+
+/* Current time (host pointer) and sticky status: HYDRO_OK or HYDRO_EUNPHYSICAL.  Both synchronise. */
+int hydro_get_time(hydro_ctx *ctx, double *t_host);
+int hydro_status(hydro_ctx *ctx);
+
+/* Number of kernels the context has launched since creation (bench.py "gpu_launches"). */
+long long hydro_launch_count(const hydro_ctx *ctx);
+
+/* Text of the last error on this context ("" if none).  Valid until the next call on the context. */
+const char *hydro_last_error(const hydro_ctx *ctx);
+
+void hydro_destroy(hydro_ctx *ctx);
+
+/* Machine probe, independent of any context: run a register-resident chain of fused multiply-adds on
+ * every SM for about `millis` milliseconds and write the sustained rate in TFLOP/s (2 flops per FMA) to
+ * a HOST pointer.  precision = HYDRO_F64 or HYDRO_F32.  Used for the "alu" roofline denominator. */
+int hydro_probe_fma_peak(int precision, int millis, void *cuda_stream, double *tflops_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HYDRO_B200_H */

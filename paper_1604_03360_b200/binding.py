@@ -1,0 +1,202 @@
+"""Thin ctypes binding of libhydro_b200.so (include/hydro.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels.  PyTorch is used for device memory
+(the workspace and the state tensors) and for the stream handle.  Importing this module loads the
+shared library and fails loudly if it has not been built; there is no CPU fallback.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+WENO5, WENO7, MUSTA_FORCE = 0, 1, 2
+BC_OUTFLOW, BC_PERIODIC, BC_HUBBLE = 0, 1, 2
+F64, F32 = 0, 1
+KERNEL_AUTO, KERNEL_GENERIC, KERNEL_FUSED = 0, 1, 2
+OK, EINVAL, ENOMEM, ECUDA, EUNPHYSICAL = 0, -1, -2, -3, -4
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhydro_b200.so")
+
+SYMBOLS = [
+    "hydro_create", "hydro_set_option", "hydro_set_stream", "hydro_workspace_bytes", "hydro_bind_workspace",
+    "hydro_set_state", "hydro_get_state", "hydro_set_state_host", "hydro_get_state_host", "hydro_step",
+    "hydro_step_cfl", "hydro_max_signal_speed", "hydro_eval_L", "hydro_get_time", "hydro_status",
+    "hydro_launch_count", "hydro_last_error", "hydro_destroy", "hydro_probe_fma_peak",
+]
+
+
+class HydroError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("hydro error %d: %s" % (code, msg))
+        self.code = code
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libhydro_b200.so is not built (run `python -m paper_1604_03360_b200.build`); "
+                          "the hot path has no CPU fallback")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, dbl, i32, sz = ctypes.c_void_p, ctypes.c_double, ctypes.c_int, ctypes.c_size_t
+    pd = ctypes.POINTER(ctypes.c_double)
+    L.hydro_create.argtypes = [ctypes.POINTER(vp), i32, i32, i32, dbl, i32]
+    L.hydro_set_option.argtypes = [vp, ctypes.c_char_p, dbl]
+    L.hydro_set_stream.argtypes = [vp, vp]
+    L.hydro_workspace_bytes.argtypes = [vp]
+    L.hydro_workspace_bytes.restype = sz
+    L.hydro_bind_workspace.argtypes = [vp, vp, sz]
+    L.hydro_set_state.argtypes = [vp, vp]
+    L.hydro_get_state.argtypes = [vp, vp]
+    L.hydro_set_state_host.argtypes = [vp, vp]
+    L.hydro_get_state_host.argtypes = [vp, vp]
+    L.hydro_step.argtypes = [vp, dbl, i32]
+    L.hydro_step_cfl.argtypes = [vp, dbl, i32]
+    L.hydro_max_signal_speed.argtypes = [vp, pd]
+    L.hydro_eval_L.argtypes = [vp, vp, dbl, vp]
+    L.hydro_get_time.argtypes = [vp, pd]
+    L.hydro_status.argtypes = [vp]
+    L.hydro_launch_count.argtypes = [vp]
+    L.hydro_launch_count.restype = ctypes.c_longlong
+    L.hydro_last_error.argtypes = [vp]
+    L.hydro_last_error.restype = ctypes.c_char_p
+    L.hydro_destroy.argtypes = [vp]
+    L.hydro_destroy.restype = None
+    L.hydro_probe_fma_peak.argtypes = [i32, i32, vp, pd]
+    return L
+
+
+lib = _load()
+
+
+def probe_fma_peak(precision=F64, millis=200):
+    """Sustained FMA rate in TFLOP/s (hydro_probe_fma_peak)."""
+    out = ctypes.c_double()
+    rc = lib.hydro_probe_fma_peak(precision, millis, torch.cuda.current_stream().cuda_stream, ctypes.byref(out))
+    if rc != OK:
+        raise HydroError(rc, "hydro_probe_fma_peak")
+    return out.value
+
+
+class Hydro:
+    """hydro_create ... hydro_destroy with the same names; tensors in, tensors out."""
+
+    def __init__(self, nx, ny, nz, dx, scheme, precision=F64, device="cuda", **options):
+        self._h = ctypes.c_void_p()
+        rc = lib.hydro_create(ctypes.byref(self._h), nx, ny, nz, float(dx), scheme)
+        if rc != OK:
+            raise HydroError(rc, "hydro_create(%d,%d,%d,%g,%d)" % (nx, ny, nz, dx, scheme))
+        self.shape = (5, nz, ny, nx)
+        self.device = torch.device(device)
+        self.dtype = torch.float32 if precision == F32 else torch.float64
+        self._ws = None
+        if precision != F64:
+            self.set_option("precision", precision)
+        for k, v in options.items():
+            self.set_option(k, v)
+
+    def _check(self, rc):
+        if rc != OK:
+            raise HydroError(rc, lib.hydro_last_error(self._h).decode())
+
+    def set_option(self, key, value):
+        self._check(lib.hydro_set_option(self._h, key.encode(), float(value)))
+
+    def workspace_bytes(self):
+        return lib.hydro_workspace_bytes(self._h)
+
+    def bind(self):
+        """Allocate the workspace with torch and hand it to the library; use torch's current stream."""
+        nbytes = self.workspace_bytes()
+        self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self._ws.data_ptr() + 255) // 256 * 256
+        self._check(lib.hydro_set_stream(self._h, torch.cuda.current_stream(self.device).cuda_stream))
+        self._check(lib.hydro_bind_workspace(self._h, ptr, nbytes))
+        return self
+
+    def set_stream(self, stream):
+        self._check(lib.hydro_set_stream(self._h, stream.cuda_stream))
+
+    def _dev(self, t):
+        assert t.is_cuda and t.is_contiguous() and t.dtype == self.dtype and tuple(t.shape) == self.shape, \
+            (t.device, t.dtype, tuple(t.shape), self.shape)
+        return t.data_ptr()
+
+    def _host(self, t):
+        assert (not t.is_cuda) and t.is_contiguous() and t.dtype == self.dtype and tuple(t.shape) == self.shape
+        return t.data_ptr()
+
+    def set_state(self, cons):
+        self._check(lib.hydro_set_state(self._h, self._dev(cons)))
+
+    def get_state(self, out=None):
+        if out is None:
+            out = torch.empty(self.shape, dtype=self.dtype, device=self.device)
+        self._check(lib.hydro_get_state(self._h, self._dev(out)))
+        return out
+
+    def set_state_host(self, cons_host):
+        self._check(lib.hydro_set_state_host(self._h, self._host(cons_host)))
+
+    def get_state_host(self, out_host):
+        self._check(lib.hydro_get_state_host(self._h, self._host(out_host)))
+        return out_host
+
+    def step(self, dt, nsteps=1):
+        self._check(lib.hydro_step(self._h, float(dt), int(nsteps)))
+
+    def step_cfl(self, cfl, nsteps=1):
+        self._check(lib.hydro_step_cfl(self._h, float(cfl), int(nsteps)))
+
+    def max_signal_speed(self):
+        v = ctypes.c_double()
+        self._check(lib.hydro_max_signal_speed(self._h, ctypes.byref(v)))
+        return v.value
+
+    def eval_L(self, cons, t_stage=0.0, out=None):
+        if out is None:
+            out = torch.empty(self.shape, dtype=self.dtype, device=self.device)
+        self._check(lib.hydro_eval_L(self._h, self._dev(cons), float(t_stage), self._dev(out)))
+        return out
+
+    @property
+    def time(self):
+        v = ctypes.c_double()
+        self._check(lib.hydro_get_time(self._h, ctypes.byref(v)))
+        return v.value
+
+    def status(self):
+        return lib.hydro_status(self._h)
+
+    @property
+    def launch_count(self):
+        return lib.hydro_launch_count(self._h)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib.hydro_destroy(self._h)
+            self._h = ctypes.c_void_p()
+        self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def from_workload(w, precision=F64, kernel=KERNEL_AUTO, device="cuda"):
+    """Context configured for a workloads.Workload, state uploaded (host numpy -> device)."""
+    h = Hydro(w.n[0], w.n[1], w.n[2], w.dx, w.scheme, precision=precision, device=device)
+    for ax, b in zip("xyz", w.bc):
+        h.set_option("bc_" + ax, b)
+    for ax, x0 in zip("xyz", w.origin):
+        h.set_option(ax + "0", x0)
+    h.set_option("t", w.t0)
+    h.set_option("kernel", kernel)
+    for k, v in w.options.items():
+        h.set_option(k, v)
+    h.bind()
+    h.set_state(torch.from_numpy(w.cons).to(device=device, dtype=h.dtype).contiguous())
+    return h

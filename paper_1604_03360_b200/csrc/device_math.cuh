@@ -1,0 +1,176 @@
+// device_math.cuh -- per-cell and per-interface arithmetic of the hot path (sm_100a).
+//
+// Everything here is the CUDA side's own restatement of DESIGN.md section 2 (steps a2..a7'); it shares
+// no source with oracle/.  The formulas are algebraically those of the paper's schemes (WENO5/7 on
+// LLF-split fluxes; MUSTA-FORCE with MUSCL/minmod) but arranged for the
+// fp64 pipe: undivided differences, fused multiply-adds, cross-multiplied nonlinear weights and one
+// reciprocal per pair of reconstructions.  The rearrangements change rounding only.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+#define HD __host__ __device__ __forceinline__
+
+namespace hydro {
+
+enum { NF = 5 };                       // E, Mx, My, Mz, R
+enum { W_INV = 0, W_P = 1, W_AX = 2 }; // primitive arrays: 1/(E+p) scaled (see con2prim), p, a_x, a_y, a_z
+enum { NW = 5 };
+
+template <class T> HD T tfma(T a, T b, T c);
+template <> HD double tfma<double>(double a, double b, double c) { return fma(a, b, c); }
+template <> HD float tfma<float>(float a, float b, float c) { return fmaf(a, b, c); }
+template <class T> HD T tsqrt(T x);
+template <> HD double tsqrt<double>(double x) { return sqrt(x); }
+template <> HD float tsqrt<float>(float x) { return sqrtf(x); }
+template <class T> HD T tabs(T x) { return x < (T)0 ? -x : x; }
+template <class T> HD T tmax(T a, T b);
+template <> HD double tmax<double>(double a, double b) { return fmax(a, b); }
+template <> HD float tmax<float>(float a, float b) { return fmaxf(a, b); }
+template <class T> HD T tmin(T a, T b);
+template <> HD double tmin<double>(double a, double b) { return fmin(a, b); }
+template <> HD float tmin<float>(float a, float b) { return fminf(a, b); }
+
+// Reciprocal of a positive, finite, normal number.  fp64: MUFU.RCP64H seed (about 2^-23) plus two
+// Newton steps = 4 DFMA, error about 1 ulp, no special-case path.  fp32: the hardware reciprocal.
+HD double fast_rcp(double x) {
+#ifdef __CUDA_ARCH__
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    return y;
+#else
+    return 1.0 / x;
+#endif
+}
+HD float fast_rcp(float x) {
+#ifdef __CUDA_ARCH__
+    return __frcp_rn(x);
+#else
+    return 1.0f / x;
+#endif
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2. conserved -> primitive, closed form for p = e/3 (a2; reading Q16).
+//   s = sqrt(4E^2 - 3M^2);  v_i = 3 M_i/(2E + s);  e = 3(E^2 - M^2)/(s + E);  p = e/3.
+// Returns winv = 3/(2E+s) (so that v_i = M_i * winv) and p.  The clamp E >= 1e-300,
+// |M| <= (1-1e-12) E raises flag; the caller's E and M are left alone (the physical flux keeps using
+// them), the rescaling of M goes into winv.
+template <class T>
+HD void con2prim(T E, T M0, T M1, T M2, T& winv, T& p, T& v2, int& flag) {
+    if (!(E >= (T)1e-300)) {
+        E = (T)1e-300;
+        flag = 1;
+    }
+    T m2 = tfma(M0, M0, tfma(M1, M1, M2 * M2));
+    const T lim = ((T)1 - (T)1e-12) * E;
+    T sc = (T)1;
+    if (m2 > lim * lim) {
+        const T mabs = tsqrt(m2);
+        if (mabs > lim) {
+            sc = lim / mabs;
+            m2 = lim * lim;
+            flag = 1;
+        }
+    }
+    const T s = tsqrt(tfma((T)4 * E, E, (T)-3 * m2));
+    const T w = (T)3 / ((T)2 * E + s);
+    p = tfma(E, E, -m2) / (s + E);
+    v2 = m2 * w * w;
+    winv = w * sc;
+}
+
+// a3. directional characteristic speeds, c_s^2 = 1/3 (a3):
+//   a_d = ( |v_d| (1-cs2) + cs sqrt((1-v^2)(1 - v_d^2 - (v^2 - v_d^2) cs2)) ) / (1 - v^2 cs2)
+template <class T>
+HD T signal_speed(T vd, T v2, T inv_den) {
+    const T cs2 = (T)(1.0 / 3.0);
+    const T cs = (T)0.57735026918962576451;
+    const T vd2 = vd * vd;
+    const T disc = ((T)1 - v2) * ((T)1 - vd2 - (v2 - vd2) * cs2);
+    return (tabs(vd) * ((T)1 - cs2) + cs * tsqrt(disc)) * inv_den;
+}
+template <class T>
+HD T speed_inv_den(T v2) { return (T)1 / ((T)1 - v2 * (T)(1.0 / 3.0)); }
+
+// ------------------------------------------------------------------------------------------------
+// a7. WENO reconstructions in numerator/denominator form.
+// For stencil values f_0..f_{2r-2} (upwind-ordered) the reconstructed value at the interface is
+//   f_c + N / D,   f_c = the centre value f_{r-1},
+// with N = sum_k d_k P_k (q_k - f_c) and D = sum_k d_k P_k, P_k = prod_{j != k} (eps' + beta'_j)^2:
+// the classic weights alpha_k = d_k/(eps+beta_k)^2 multiplied through by prod_j (eps+beta_j)^2
+// (DESIGN.md section 6).  beta' and eps' carry a common scale factor, which cancels in N/D.
+
+// WENO5 (Jiang-Shu, O3).  Here beta' = 4 beta and eps4 = 4 eps.
+template <class T>
+HD void weno5_nd(T a, T b, T c, T d, T e, T eps4, T& N, T& D) {
+    const T D1 = b - a, D2 = c - b, D3 = d - c, D4 = e - d;
+    const T t0 = D2 - D1, t1 = D3 - D2, t2 = D4 - D3;      // second differences
+    const T u0 = tfma((T)3, D2, -D1);                      // a - 4b + 3c
+    const T u1 = D2 + D3;                                  // d - b
+    const T u2 = tfma((T)-3, D3, D4);                      // 3c - 4d + e, sign irrelevant (squared)
+    const T k = (T)(13.0 / 3.0);
+    const T B0 = tfma(k * t0, t0, tfma(u0, u0, eps4));
+    const T B1 = tfma(k * t1, t1, tfma(u1, u1, eps4));
+    const T B2 = tfma(k * t2, t2, tfma(u2, u2, eps4));
+    const T s0 = B0 * B0, s1 = B1 * B1, s2 = B2 * B2;
+    const T P0 = s1 * s2, P1 = s0 * s2, P2 = s0 * s1;
+    // 10 d_k = (1, 6, 3);  q_k - c = (5 D2 - 2 D1)/6, (D2 + 2 D3)/6, (4 D3 - D4)/6
+    const T g0 = tfma((T)(5.0 / 6.0), D2, (T)(-1.0 / 3.0) * D1);
+    const T g1 = tfma((T)2, D3, D2);                       // times 6 d1/(6) = 1
+    const T g2 = tfma((T)2, D3, (T)-0.5 * D4);             // (4 D3 - D4)/6 * 3
+    N = tfma(P0, g0, tfma(P1, g1, P2 * g2));
+    D = tfma((T)6, P1, tfma((T)3, P2, P0));
+}
+
+// WENO7 (Balsara-Shu, O4).  For the cubic through four cell averages written as
+// c0 + c1 x + c2 x^2 + c3 x^3 about the centre of cell i (dx = 1) the smoothness indicator is
+//   beta = (c1 + c3/4)^2 + (13/3) c2^2 + (781/20) c3^2
+// (the integrals of the squared first, second and third derivatives over the cell, summed); in terms
+// of undivided differences c3 = D3/6, c2 = (second difference at i)/2 and c1 follows from matching
+// the averages.  This equals the integer-coefficient quadratic forms of O4 divided by 240.
+template <class T>
+HD void weno7_nd(T a, T b, T c, T d, T e, T f, T g, T eps, T& N, T& D) {
+    // first differences around the centre cell d
+    const T E1 = b - a, E2 = c - b, E3 = d - c, E4 = e - d, E5 = f - e, E6 = g - f;
+    const T S1 = E2 - E1, S2 = E3 - E2, S3 = E4 - E3, S4 = E5 - E4, S5 = E6 - E5;  // second
+    const T T1 = S2 - S1, T2 = S3 - S2, T3 = S4 - S3, T4 = S5 - S4;                // third
+    // Stencil k holds cells (k..k+3) of (a..g); the centre cell d sits at position 3-k inside it.
+    // Solving "cell averages of the cubic = stencil values" for the coefficients about cell d gives
+    // (checked with exact rationals against the 240-beta forms of O4, and q_k against O4's q_k):
+    //   k=0: c3 = T1/6, c2 = (S2 + T1)/2, c1 + c3/4 = E3 + S2/2 + T1/3
+    //   k=1: c3 = T2/6, c2 = S3/2,        c1 + c3/4 = (E3 + E4)/2 - T2/6
+    //   k=2: c3 = T3/6, c2 = S3/2,        c1 + c3/4 = (E3 + E4)/2 - T3/6
+    //   k=3: c3 = T4/6, c2 = (S4 - T4)/2, c1 + c3/4 = E4 - S4/2 + T4/3
+    const T k13 = (T)(13.0 / 3.0), k781 = (T)(781.0 / 20.0);
+    const T sixth = (T)(1.0 / 6.0);
+    const T c3_0 = T1 * sixth, c2_0 = (T)0.5 * (S2 + T1), m_0 = E3 + tfma((T)0.5, S2, (T)(1.0 / 3.0) * T1);
+    const T c3_1 = T2 * sixth, c2_1 = (T)0.5 * S3, m_1 = tfma((T)(-1.0 / 6.0), T2, (T)0.5 * (E3 + E4));
+    const T c3_2 = T3 * sixth, c2_2 = (T)0.5 * S3, m_2 = tfma((T)(-1.0 / 6.0), T3, (T)0.5 * (E3 + E4));
+    const T c3_3 = T4 * sixth, c2_3 = (T)0.5 * (S4 - T4), m_3 = E4 + tfma((T)-0.5, S4, (T)(1.0 / 3.0) * T4);
+    const T B0 = tfma(m_0, m_0, tfma(k13 * c2_0, c2_0, tfma(k781 * c3_0, c3_0, eps)));
+    const T B1 = tfma(m_1, m_1, tfma(k13 * c2_1, c2_1, tfma(k781 * c3_1, c3_1, eps)));
+    const T B2 = tfma(m_2, m_2, tfma(k13 * c2_2, c2_2, tfma(k781 * c3_2, c3_2, eps)));
+    const T B3 = tfma(m_3, m_3, tfma(k13 * c2_3, c2_3, tfma(k781 * c3_3, c3_3, eps)));
+    const T s0 = B0 * B0, s1 = B1 * B1, s2 = B2 * B2, s3 = B3 * B3;
+    const T s01 = s0 * s1, s23 = s2 * s3;
+    const T P0 = s1 * s23, P1 = s0 * s23, P2 = s01 * s3, P3 = s01 * s2;
+    // q_k - d (centre value) from the candidate polynomials of O4:
+    //   q0 - d = (-3a + 13b - 23c + 13d)/12 = (13 E3 - 10 E2 + 3 E1)/12
+    //   q1 - d = (b - 5c + d + 3e)/12       = (3 E4 + 4 E3 - E2)/12
+    //   q2 - d = (-c - 5d + 7e - f)/12      = (-E5 + 6 E4 + E3)/12
+    //   q3 - d = (-9d + 13e - 5f + g)/12    = (E6 - 4 E5 + 9 E4)/12
+    // 35 d_k = (1, 12, 18, 4)
+    const T g0 = tfma((T)(13.0 / 12.0), E3, tfma((T)(-10.0 / 12.0), E2, (T)(3.0 / 12.0) * E1));
+    const T g1 = tfma((T)3, E4, tfma((T)4, E3, -E2));                        // x 12/12
+    const T g2 = tfma((T)9, E4, tfma((T)1.5, E3, (T)-1.5 * E5));             // x 18/12
+    const T g3 = tfma((T)3, E4, tfma((T)(-4.0 / 3.0), E5, (T)(1.0 / 3.0) * E6)); // x 4/12
+    N = tfma(P0, g0, tfma(P1, g1, tfma(P2, g2, P3 * g3)));
+    D = tfma((T)12, P1, tfma((T)18, P2, tfma((T)4, P3, P0)));
+}
+
+}  // namespace hydro

@@ -1,0 +1,466 @@
+// hydro.cu -- C ABI of libhydro_b200 (include/hydro.h): context, options, workspace carving and the
+// launch sequence of one SSP-RK3 step:
+//   per stage:  halo fill (a1) -> con2prim + speeds [+ max] (a2-a4) -> stage kernel (a5-a9)
+// No CPU arithmetic of the method happens here: the host only orders kernels on the caller's stream.
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+
+#include "../../include/hydro.h"
+#include "grid.cuh"
+#include "kernel_fused.cuh"
+#include "kernel_generic.cuh"
+#include "kernels_aux.cuh"
+
+using namespace hydro;
+
+struct hydro_ctx {
+    int n[3];
+    double dx;
+    int scheme, r;
+    int precision = HYDRO_F64;
+    int kernel = HYDRO_KERNEL_AUTO;
+    int bc[3] = {HYDRO_BC_OUTFLOW, HYDRO_BC_OUTFLOW, HYDRO_BC_OUTFLOW};
+    double eps = 1e-6, musta_cfl = 0.9;
+    int musta_stages = 2;
+    double t_host = 0.0;  // value to push into the control block at bind / set_option("t")
+    HubbleParams H;
+    cudaStream_t stream = nullptr;
+    Geom G;
+    // workspace
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    Ctl* ctl = nullptr;
+    char* U[3] = {nullptr, nullptr, nullptr};  // u^n and two stage buffers (padded, 5 fields each)
+    char* W = nullptr;                          // primitives (padded, 5 arrays)
+    FusedPlan fused;                            // tensor maps etc. for the fused kernel
+    bool fused_ready = false;
+    long long launches = 0;
+    std::string err;
+};
+
+namespace {
+
+int fail(hydro_ctx* c, int code, const char* fmt, ...) {
+    if (c) {
+        char buf[512];
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(buf, sizeof buf, fmt, ap);
+        va_end(ap);
+        c->err = buf;
+    }
+    return code;
+}
+
+size_t esize(const hydro_ctx* c) { return c->precision == HYDRO_F32 ? 4 : 8; }
+
+void make_geom(hydro_ctx* c) {
+    Geom& G = c->G;
+    for (int a = 0; a < 3; ++a) {
+        G.n[a] = c->n[a];
+        G.g[a] = c->n[a] > 1 ? c->r : 0;
+        G.np[a] = G.n[a] + 2 * G.g[a];
+    }
+    const long long q = 16 / (long long)esize(c);  // elements per 16 bytes
+    G.sx = (G.np[0] + q - 1) / q * q;
+    G.sxy = G.sx * G.np[1];
+    const long long vol = G.sxy * G.np[2];
+    const long long q256 = 256 / (long long)esize(c);
+    G.fs = (vol + q256 - 1) / q256 * q256;
+}
+
+size_t state_bytes(const hydro_ctx* c) { return (size_t)NF * (size_t)c->G.fs * esize(c); }
+
+#define CUDA_OK(c, call)                                                                      \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess) return fail(c, HYDRO_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+#define LAUNCHED(c, what)                                                                     \
+    do {                                                                                      \
+        ++(c)->launches;                                                                      \
+        cudaError_t e_ = cudaGetLastError();                                                  \
+        if (e_ != cudaSuccess) return fail(c, HYDRO_ECUDA, "launch %s: %s", what, cudaGetErrorString(e_)); \
+    } while (0)
+
+dim3 blk2d(int bx, int by) { return dim3(bx, by, 1); }
+dim3 grd(int nx, int ny, int nz, dim3 b) { return dim3((nx + b.x - 1) / b.x, (ny + b.y - 1) / b.y, nz); }
+
+__global__ void set_ctl_kernel(Ctl* ctl, double t, int reset_flag) {
+    ctl->t = t;
+    if (reset_flag) {
+        ctl->flag = 0;
+        ctl->maxspeed_bits = 0ull;
+        ctl->dt = 0.0;
+    }
+}
+
+int need_ws(hydro_ctx* c) {
+    if (!c) return HYDRO_EINVAL;
+    if (!c->ws) return fail(c, HYDRO_ENOMEM, "no workspace bound (hydro_bind_workspace)");
+    return HYDRO_OK;
+}
+
+template <class T>
+int do_halo(hydro_ctx* c, T* pad, double tfrac, bool use_abs, double t_abs) {
+    HaloArgs A;
+    long long total = 0;
+    for (int a = 0; a < 3; ++a) {
+        A.bc[a] = c->bc[a];
+        const int a1 = a == 0 ? 1 : 0, a2 = a == 2 ? 1 : 2;
+        A.count[a] = c->G.g[a] ? 2LL * c->G.g[a] * c->G.n[a1] * c->G.n[a2] : 0;
+        total += A.count[a];
+    }
+    A.H = c->H;
+    A.H.dx = c->dx;
+    if (total == 0) return HYDRO_OK;
+    const int tb = 256;
+    halo_fill_kernel<T><<<(unsigned)((total + tb - 1) / tb), tb, 0, c->stream>>>(c->G, A, c->ctl, tfrac, t_abs,
+                                                                                   use_abs ? 1 : 0, pad);
+    LAUNCHED(c, "halo_fill_kernel");
+    return HYDRO_OK;
+}
+
+template <class T>
+int do_prim(hydro_ctx* c, const T* pad, int do_max) {
+    const dim3 b = blk2d(64, 4);
+    prim_kernel<T><<<grd(c->G.np[0], c->G.np[1], c->G.np[2], b), b, 0, c->stream>>>(c->G, pad, (T*)c->W, c->ctl,
+                                                                                      do_max);
+    LAUNCHED(c, "prim_kernel");
+    return HYDRO_OK;
+}
+
+template <class T>
+int do_max_speed(hydro_ctx* c, const T* pad) {
+    const dim3 b = blk2d(64, 4);
+    max_speed_kernel<T><<<grd(c->G.n[0], c->G.n[1], c->G.n[2], b), b, 0, c->stream>>>(c->G, pad, c->ctl);
+    LAUNCHED(c, "max_speed_kernel");
+    return HYDRO_OK;
+}
+
+StageArgs stage_args(const hydro_ctx* c, double ca, double cb, int mode) {
+    StageArgs A;
+    A.ca = ca;
+    A.cb = cb;
+    A.mode = mode;
+    A.inv_dx = 1.0 / c->dx;
+    A.eps = c->eps;
+    A.musta_K = c->musta_stages;
+    A.musta_C = c->musta_cfl;
+    return A;
+}
+
+bool want_fused(const hydro_ctx* c) {
+    if (c->kernel == HYDRO_KERNEL_GENERIC) return false;
+    return fused_supported(c->G, c->scheme, c->precision);
+}
+
+template <class T>
+int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double cb, int mode) {
+    const StageArgs A = stage_args(c, ca, cb, mode);
+    if (want_fused(c)) {
+        if (!c->fused_ready) return fail(c, HYDRO_ECUDA, "fused plan not built: %s", c->fused.err);
+        const int rc = launch_fused<T>(c->fused, c->G, c->scheme, A, Us, (const T*)c->W, Un, Uout, c->ctl, c->stream);
+        if (rc != 0) return fail(c, HYDRO_ECUDA, "fused launch: %s", c->fused.err);
+        ++c->launches;
+        return HYDRO_OK;
+    }
+    if (c->kernel == HYDRO_KERNEL_FUSED)
+        return fail(c, HYDRO_EINVAL, "kernel=fused requested but the grid/scheme does not allow it");
+    const dim3 b = blk2d(32, 4);
+    const dim3 g = grd(c->G.n[0], c->G.n[1], c->G.n[2], b);
+    const T* W = (const T*)c->W;
+    switch (c->scheme) {
+        case HYDRO_WENO5: stage_generic_kernel<T, 0><<<g, b, 0, c->stream>>>(c->G, A, Us, W, Un, Uout, c->ctl); break;
+        case HYDRO_WENO7: stage_generic_kernel<T, 1><<<g, b, 0, c->stream>>>(c->G, A, Us, W, Un, Uout, c->ctl); break;
+        default: stage_generic_kernel<T, 2><<<g, b, 0, c->stream>>>(c->G, A, Us, W, Un, Uout, c->ctl); break;
+    }
+    LAUNCHED(c, "stage_generic_kernel");
+    return HYDRO_OK;
+}
+
+// One SSP-RK3 step (a9, O8):  u1 = u + dt L(u);  u2 = 3/4 u + 1/4 (u1 + dt L(u1));
+// u' = 1/3 u + 2/3 (u2 + dt L(u2)), ghosts at t, t+dt, t+dt/2.  dt_fixed > 0, or CFL mode.
+template <class T>
+int do_step(hydro_ctx* c, double dt_fixed, double cfl) {
+    T* U0 = (T*)c->U[0];
+    T* U1 = (T*)c->U[1];
+    T* U2 = (T*)c->U[2];
+    const bool weno = c->scheme != HYDRO_MUSTA_FORCE;
+    const bool cflmode = !(dt_fixed > 0.0);
+    int rc;
+    // stage 1
+    if ((rc = do_halo<T>(c, U0, 0.0, false, 0.0))) return rc;
+    if (weno) {
+        if ((rc = do_prim<T>(c, U0, cflmode ? 1 : 0))) return rc;
+    } else if (cflmode) {
+        if ((rc = do_max_speed<T>(c, U0))) return rc;
+    }
+    begin_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl, dt_fixed, cfl, c->dx);
+    LAUNCHED(c, "begin_step_kernel");
+    if ((rc = do_stage<T>(c, U0, U0, U1, 0.0, 1.0, 0))) return rc;
+    // stage 2
+    if ((rc = do_halo<T>(c, U1, 1.0, false, 0.0))) return rc;
+    if (weno && (rc = do_prim<T>(c, U1, 0))) return rc;
+    if ((rc = do_stage<T>(c, U1, U0, U2, 0.75, 0.25, 0))) return rc;
+    // stage 3 (writes u^n in place: each cell reads only its own u^n)
+    if ((rc = do_halo<T>(c, U2, 0.5, false, 0.0))) return rc;
+    if (weno && (rc = do_prim<T>(c, U2, 0))) return rc;
+    if ((rc = do_stage<T>(c, U2, U0, U0, 1.0 / 3.0, 2.0 / 3.0, 0))) return rc;
+    end_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
+    LAUNCHED(c, "end_step_kernel");
+    return HYDRO_OK;
+}
+
+template <class T>
+int eval_L_impl(hydro_ctx* c, const void* cons, double t_stage, void* L_out) {
+    T* U1 = (T*)c->U[1];
+    T* U2 = (T*)c->U[2];
+    const dim3 b = blk2d(64, 4);
+    const dim3 g = grd(c->G.n[0], c->G.n[1], c->G.n[2], b);
+    int rc;
+    pack_kernel<T><<<g, b, 0, c->stream>>>(c->G, (const T*)cons, U1);
+    LAUNCHED(c, "pack_kernel");
+    if ((rc = do_halo<T>(c, U1, 0.0, true, t_stage))) return rc;
+    if (c->scheme != HYDRO_MUSTA_FORCE && (rc = do_prim<T>(c, U1, 0))) return rc;
+    if ((rc = do_stage<T>(c, U1, U1, U2, 0.0, 1.0, 1))) return rc;
+    unpack_kernel<T><<<g, b, 0, c->stream>>>(c->G, U2, (T*)L_out);
+    LAUNCHED(c, "unpack_kernel");
+    return HYDRO_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+extern "C" {
+
+int hydro_create(hydro_ctx** out, int nx, int ny, int nz, double dx, int scheme) {
+    if (!out || nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || scheme < 0 || scheme > 2) return HYDRO_EINVAL;
+    hydro_ctx* c = new (std::nothrow) hydro_ctx;
+    if (!c) return HYDRO_ENOMEM;
+    c->n[0] = nx; c->n[1] = ny; c->n[2] = nz;
+    c->dx = dx;
+    c->scheme = scheme;
+    c->r = scheme == HYDRO_WENO5 ? 3 : scheme == HYDRO_WENO7 ? 4 : 2;
+    for (int a = 0; a < 3; ++a)
+        if (c->n[a] > 1 && c->n[a] < c->r) { delete c; return HYDRO_EINVAL; }
+    memset(&c->H, 0, sizeof c->H);
+    c->H.t0 = c->H.e0 = c->H.n0 = 1.0;
+    make_geom(c);
+    *out = c;
+    return HYDRO_OK;
+}
+
+void hydro_destroy(hydro_ctx* c) { delete c; }
+
+const char* hydro_last_error(const hydro_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+long long hydro_launch_count(const hydro_ctx* c) { return c ? c->launches : 0; }
+
+int hydro_set_stream(hydro_ctx* c, void* s) {
+    if (!c) return HYDRO_EINVAL;
+    c->stream = (cudaStream_t)s;
+    return HYDRO_OK;
+}
+
+int hydro_set_option(hydro_ctx* c, const char* key, double v) {
+    if (!c || !key) return HYDRO_EINVAL;
+    const std::string k(key);
+    if (k == "precision") {
+        const int p = (int)v;
+        if (p != HYDRO_F64 && p != HYDRO_F32) return fail(c, HYDRO_EINVAL, "precision must be 0 or 1");
+        if (c->ws && p != c->precision) return fail(c, HYDRO_EINVAL, "precision must be set before the workspace is bound");
+        c->precision = p;
+        make_geom(c);
+    } else if (k == "kernel") {
+        const int p = (int)v;
+        if (p < 0 || p > 2) return fail(c, HYDRO_EINVAL, "kernel must be 0, 1 or 2");
+        c->kernel = p;
+    } else if (k == "bc_x" || k == "bc_y" || k == "bc_z") {
+        const int b = (int)v;
+        if (b < 0 || b > 2) return fail(c, HYDRO_EINVAL, "unknown boundary rule %d", b);
+        c->bc[k[3] - 'x'] = b;
+    } else if (k == "musta_stages") {
+        if (v < 1) return fail(c, HYDRO_EINVAL, "musta_stages < 1");
+        c->musta_stages = (int)v;
+    } else if (k == "musta_cfl") {
+        if (!(v > 0)) return fail(c, HYDRO_EINVAL, "musta_cfl <= 0");
+        c->musta_cfl = v;
+    } else if (k == "weno_eps") {
+        if (!(v > 0)) return fail(c, HYDRO_EINVAL, "weno_eps <= 0");
+        c->eps = v;
+    } else if (k == "t") {
+        c->t_host = v;
+        if (c->ws) {
+            set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, v, 0);
+            LAUNCHED(c, "set_ctl_kernel");
+        }
+    } else if (k == "x0") c->H.origin[0] = v;
+    else if (k == "y0") c->H.origin[1] = v;
+    else if (k == "z0") c->H.origin[2] = v;
+    else if (k == "hubble_t0") c->H.t0 = v;
+    else if (k == "hubble_e0") c->H.e0 = v;
+    else if (k == "hubble_n0") c->H.n0 = v;
+    else if (k == "hubble_bx") c->H.b[0] = v;
+    else if (k == "hubble_by") c->H.b[1] = v;
+    else if (k == "hubble_bz") c->H.b[2] = v;
+    else return fail(c, HYDRO_EINVAL, "unknown option '%s'", key);
+    return HYDRO_OK;
+}
+
+size_t hydro_workspace_bytes(const hydro_ctx* c) {
+    if (!c) return 0;
+    return 256 + 4 * state_bytes(c);  // control block, U0, U1, U2, W
+}
+
+int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
+    if (!c || !p) return HYDRO_EINVAL;
+    if (((size_t)p & 255) != 0) return fail(c, HYDRO_EINVAL, "workspace must be 256-byte aligned");
+    if (bytes < hydro_workspace_bytes(c))
+        return fail(c, HYDRO_ENOMEM, "workspace too small: %zu < %zu", bytes, hydro_workspace_bytes(c));
+    c->ws = p;
+    c->ws_bytes = bytes;
+    char* base = (char*)p;
+    c->ctl = (Ctl*)base;
+    const size_t sb = state_bytes(c);
+    for (int i = 0; i < 3; ++i) c->U[i] = base + 256 + i * sb;
+    c->W = base + 256 + 3 * sb;
+    CUDA_OK(c, cudaMemsetAsync(p, 0, hydro_workspace_bytes(c), c->stream));
+    set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, c->t_host, 1);
+    LAUNCHED(c, "set_ctl_kernel");
+    c->fused_ready = false;
+    if (fused_supported(c->G, c->scheme, c->precision) && c->kernel != HYDRO_KERNEL_GENERIC) {
+        c->fused_ready = build_fused_plan(c->fused, c->G, c->scheme, c->precision) == 0;
+        if (!c->fused_ready && c->kernel == HYDRO_KERNEL_FUSED)
+            return fail(c, HYDRO_ECUDA, "fused plan: %s", c->fused.err);
+    }
+    return HYDRO_OK;
+}
+
+int hydro_set_state(hydro_ctx* c, const void* cons) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    if (!cons) return HYDRO_EINVAL;
+    const dim3 b = blk2d(64, 4);
+    const dim3 g = grd(c->G.n[0], c->G.n[1], c->G.n[2], b);
+    if (c->precision == HYDRO_F64) pack_kernel<double><<<g, b, 0, c->stream>>>(c->G, (const double*)cons, (double*)c->U[0]);
+    else pack_kernel<float><<<g, b, 0, c->stream>>>(c->G, (const float*)cons, (float*)c->U[0]);
+    LAUNCHED(c, "pack_kernel");
+    set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, c->t_host, 1);
+    LAUNCHED(c, "set_ctl_kernel");
+    return HYDRO_OK;
+}
+
+int hydro_get_state(hydro_ctx* c, void* out) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    if (!out) return HYDRO_EINVAL;
+    const dim3 b = blk2d(64, 4);
+    const dim3 g = grd(c->G.n[0], c->G.n[1], c->G.n[2], b);
+    if (c->precision == HYDRO_F64) unpack_kernel<double><<<g, b, 0, c->stream>>>(c->G, (const double*)c->U[0], (double*)out);
+    else unpack_kernel<float><<<g, b, 0, c->stream>>>(c->G, (const float*)c->U[0], (float*)out);
+    LAUNCHED(c, "unpack_kernel");
+    return HYDRO_OK;
+}
+
+// Host entry points: stage through the (idle between steps) second RK buffer.
+int hydro_set_state_host(hydro_ctx* c, const void* cons_host) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    if (!cons_host) return HYDRO_EINVAL;
+    const size_t bytes = (size_t)NF * c->n[0] * c->n[1] * c->n[2] * esize(c);
+    CUDA_OK(c, cudaMemcpyAsync(c->U[2], cons_host, bytes, cudaMemcpyHostToDevice, c->stream));
+    if ((rc = hydro_set_state(c, c->U[2]))) return rc;
+    CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    return HYDRO_OK;
+}
+
+int hydro_get_state_host(hydro_ctx* c, void* out_host) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    if (!out_host) return HYDRO_EINVAL;
+    const size_t bytes = (size_t)NF * c->n[0] * c->n[1] * c->n[2] * esize(c);
+    if ((rc = hydro_get_state(c, c->U[2]))) return rc;
+    CUDA_OK(c, cudaMemcpyAsync(out_host, c->U[2], bytes, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    return HYDRO_OK;
+}
+
+int hydro_step(hydro_ctx* c, double dt, int nsteps) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    if (!(dt > 0) || nsteps < 0) return fail(c, HYDRO_EINVAL, "hydro_step: dt <= 0 or nsteps < 0");
+    for (int s = 0; s < nsteps; ++s) {
+        rc = c->precision == HYDRO_F64 ? do_step<double>(c, dt, 0.0) : do_step<float>(c, dt, 0.0);
+        if (rc) return rc;
+    }
+    return HYDRO_OK;
+}
+
+int hydro_step_cfl(hydro_ctx* c, double cfl, int nsteps) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    if (!(cfl > 0) || nsteps < 0) return fail(c, HYDRO_EINVAL, "hydro_step_cfl: cfl <= 0 or nsteps < 0");
+    for (int s = 0; s < nsteps; ++s) {
+        rc = c->precision == HYDRO_F64 ? do_step<double>(c, -1.0, cfl) : do_step<float>(c, -1.0, cfl);
+        if (rc) return rc;
+    }
+    return HYDRO_OK;
+}
+
+int hydro_max_signal_speed(hydro_ctx* c, double* out_host) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    if (!out_host) return HYDRO_EINVAL;
+    reset_max_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
+    LAUNCHED(c, "reset_max_kernel");
+    rc = c->precision == HYDRO_F64 ? do_max_speed<double>(c, (const double*)c->U[0])
+                                   : do_max_speed<float>(c, (const float*)c->U[0]);
+    if (rc) return rc;
+    Ctl h;
+    CUDA_OK(c, cudaMemcpyAsync(&h, c->ctl, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    memcpy(out_host, &h.maxspeed_bits, sizeof(double));
+    reset_max_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
+    LAUNCHED(c, "reset_max_kernel");
+    return HYDRO_OK;
+}
+
+int hydro_eval_L(hydro_ctx* c, const void* cons, double t_stage, void* L_out) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    if (!cons || !L_out) return HYDRO_EINVAL;
+    return c->precision == HYDRO_F64 ? eval_L_impl<double>(c, cons, t_stage, L_out)
+                                     : eval_L_impl<float>(c, cons, t_stage, L_out);
+}
+
+int hydro_get_time(hydro_ctx* c, double* t_host) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    if (!t_host) return HYDRO_EINVAL;
+    Ctl h;
+    CUDA_OK(c, cudaMemcpyAsync(&h, c->ctl, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    *t_host = h.t;
+    return HYDRO_OK;
+}
+
+int hydro_status(hydro_ctx* c) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    Ctl h;
+    CUDA_OK(c, cudaMemcpyAsync(&h, c->ctl, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(c, HYDRO_ECUDA, "%s", cudaGetErrorString(e));
+    return h.flag ? fail(c, HYDRO_EUNPHYSICAL, "con2prim clamped at least one cell") : HYDRO_OK;
+}
+
+}  // extern "C"
+
+#include "probe.cuh"

@@ -1,0 +1,151 @@
+// iface.cuh -- one interface flux (steps a5..a7 and a7') from a stencil accessor.
+//
+// The accessor hides where the stencil lives (global memory in the generic kernel, the shared-memory
+// ring / plane in the fused kernel): acc.u(c, k) is conserved field c of stencil cell k and
+// acc.w(a, k) primitive array a (W_INV, W_P, W_AX + axis), k = 0 .. 2r-1 for cells i-r+1 .. i+r.
+#pragma once
+#include "device_math.cuh"
+
+namespace hydro {
+
+template <class T> struct is_f64 { static constexpr bool value = false; };
+template <> struct is_f64<double> { static constexpr bool value = true; };
+
+// value of (f+ reconstruction) + (f- reconstruction) from the two N/D pairs and the centre values.
+// fp64: one reciprocal for the pair.  fp32: the product of the two denominators can leave the
+// normal range, so two hardware reciprocals.
+template <class T>
+HD T combine_pair(T centre, T Np, T Dp, T Nm, T Dm) {
+    if (is_f64<T>::value) {
+        const T num = tfma(Np, Dm, Nm * Dp);
+        return tfma(num, fast_rcp(Dp * Dm), centre);
+    } else {
+        return tfma(Np, fast_rcp(Dp), tfma(Nm, fast_rcp(Dm), centre));
+    }
+}
+
+// a5-a7. Component-wise local Lax-Friedrichs flux with WENO_r reconstruction at interface i+1/2 along
+// axis DIR (O5, reading Q3):
+//   alpha = max_k a_d(k);  f+-_k = (F_d(u_k) +- alpha u_k)/2;
+//   fhat = WENO(f+ on cells 0..2r-2) + WENO(f- on cells 2r-1..1, mirrored).
+// The factor 1/2 is pulled out of the reconstruction: WENO is homogeneous of degree one when eps is
+// scaled with the square of the data, WENO_eps(g/2) = WENO_{4 eps}(g)/2, exactly in binary floating
+// point.  With v_d = M_d * winv the split fluxes are u (v_d +- alpha) for the fields that are simply
+// advected (M_j, j != d, and R), M_d (v_d +- alpha) + p for j = d, and M_d +- alpha E for E.
+template <class T, int R, int DIR, class Acc>
+HD void llf_weno_iface(const Acc& acc, T eps, T fh[NF]) {
+    constexpr int M = 2 * R;
+    constexpr int I5 = (R == 4) ? 5 : 3, I6 = (R == 4) ? 6 : 4;  // only read when R == 4
+    T md[M], vp[M], vm[M];
+    T al = acc.w(W_AX + DIR, 0);
+#pragma unroll
+    for (int k = 1; k < M; ++k) al = tmax(al, acc.w(W_AX + DIR, k));
+#pragma unroll
+    for (int k = 0; k < M; ++k) {
+        md[k] = acc.u(1 + DIR, k);
+        const T vd = md[k] * acc.w(W_INV, k);
+        vp[k] = vd + al;
+        vm[k] = vd - al;
+    }
+    // eps scale: weno5_nd works with 4*beta(g) = 16*beta(g/2); weno7_nd with beta(g) = 4*beta(g/2)
+    const T epsx = (R == 3 ? (T)16 : (T)4) * eps;
+#pragma unroll
+    for (int c = 0; c < NF; ++c) {
+        T fp[M - 1], fm[M - 1];
+        if (c == 0) {
+#pragma unroll
+            for (int k = 0; k < M - 1; ++k) {
+                fp[k] = tfma(al, acc.u(0, k), md[k]);
+                fm[k] = tfma(-al, acc.u(0, M - 1 - k), md[M - 1 - k]);
+            }
+        } else if (c == 1 + DIR) {
+#pragma unroll
+            for (int k = 0; k < M - 1; ++k) {
+                fp[k] = tfma(md[k], vp[k], acc.w(W_P, k));
+                fm[k] = tfma(md[M - 1 - k], vm[M - 1 - k], acc.w(W_P, M - 1 - k));
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < M - 1; ++k) {
+                fp[k] = acc.u(c, k) * vp[k];
+                fm[k] = acc.u(c, M - 1 - k) * vm[M - 1 - k];
+            }
+        }
+        T Np, Dp, Nm, Dm;
+        if (R == 3) {
+            weno5_nd(fp[0], fp[1], fp[2], fp[3], fp[4], epsx, Np, Dp);
+            weno5_nd(fm[0], fm[1], fm[2], fm[3], fm[4], epsx, Nm, Dm);
+        } else {
+            weno7_nd(fp[0], fp[1], fp[2], fp[3], fp[4], fp[I5], fp[I6], epsx, Np, Dp);
+            weno7_nd(fm[0], fm[1], fm[2], fm[3], fm[4], fm[I5], fm[I6], epsx, Nm, Dm);
+        }
+        fh[c] = (T)0.5 * combine_pair(fp[R - 1] + fm[R - 1], Np, Dp, Nm, Dm);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a7'. MUSTA-FORCE flux with MUSCL/minmod data (O6, O7; readings Q6-Q8).
+template <class T>
+HD T minmod(T a, T b) {
+    if (a * b <= (T)0) return (T)0;
+    const T m = tmin(tabs(a), tabs(b));
+    return a > (T)0 ? m : -m;
+}
+
+// physical flux of a conserved state along DIR plus its signal speed (every evaluation needs its own
+// con2prim, O7).  Q is modified only if the Q16 clamp fires.
+template <class T, int DIR>
+HD void flux_and_speed(const T Q[NF], T F[NF], T& a, int& flag) {
+    T winv, p, v2;
+    con2prim(Q[0], Q[1], Q[2], Q[3], winv, p, v2, flag);
+    const T vd = Q[1 + DIR] * winv;
+    F[0] = Q[1 + DIR];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) F[1 + j] = (j == DIR) ? tfma(Q[1 + j], vd, p) : Q[1 + j] * vd;
+    F[4] = Q[4] * vd;
+    a = signal_speed(vd, v2, speed_inv_den(v2));
+}
+template <class T, int DIR>
+HD void flux_only(const T Q[NF], T F[NF], int& flag) {
+    T winv, p, v2;
+    con2prim(Q[0], Q[1], Q[2], Q[3], winv, p, v2, flag);
+    const T vd = Q[1 + DIR] * winv;
+    F[0] = Q[1 + DIR];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) F[1 + j] = (j == DIR) ? tfma(Q[1 + j], vd, p) : Q[1 + j] * vd;
+    F[4] = Q[4] * vd;
+}
+
+// acc.u(c, k), k = 0..3 for cells i-1 .. i+2.  K stages, local Courant number C (tau = C/S).
+template <class T, int DIR, class Acc>
+HD void musta_force_iface(const Acc& acc, int K, T C, T fh[NF], int& flag) {
+    T QL[NF], QR[NF];
+#pragma unroll
+    for (int c = 0; c < NF; ++c) {
+        const T u0 = acc.u(c, 0), u1 = acc.u(c, 1), u2 = acc.u(c, 2), u3 = acc.u(c, 3);
+        const T dm = u1 - u0, d0 = u2 - u1, dp = u3 - u2;
+        QL[c] = tfma((T)0.5, minmod(dm, d0), u1);
+        QR[c] = tfma((T)-0.5, minmod(d0, dp), u2);
+    }
+    for (int stage = 1;; ++stage) {
+        T FL[NF], FR[NF], QM[NF], FM[NF], aL, aR;
+        flux_and_speed<T, DIR>(QL, FL, aL, flag);
+        flux_and_speed<T, DIR>(QR, FR, aR, flag);
+        const T S = tmax(aL, aR);
+        const T tau = C / S, itau = S / C;
+#pragma unroll
+        for (int c = 0; c < NF; ++c) QM[c] = (T)0.5 * ((QL[c] + QR[c]) - tau * (FR[c] - FL[c]));
+        flux_only<T, DIR>(QM, FM, flag);
+#pragma unroll
+        for (int c = 0; c < NF; ++c)
+            fh[c] = (T)0.25 * (FL[c] + (T)2 * FM[c] + FR[c] - (QR[c] - QL[c]) * itau);
+        if (stage >= K) return;
+#pragma unroll
+        for (int c = 0; c < NF; ++c) {
+            QL[c] = QL[c] - tau * (fh[c] - FL[c]);
+            QR[c] = QR[c] - tau * (FR[c] - fh[c]);
+        }
+    }
+}
+
+}  // namespace hydro
