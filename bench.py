@@ -1,0 +1,366 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path (three L(u) + SSP-RK3 combine per step) on
+BASELINE.json configs[4]: the 512^3 periodic lumpy state with 200 hotspots and blended velocities.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--scheme weno5|weno7|musta] [--precision f64|f32]
+                    [--n 512] [--no-variants] [--no-cpu-baseline] [--impl reference]
+
+One "step" is one SSP-RK3 step of the whole grid with dt = CFL dx / max signal speed taken on the device
+(hydro_step_cfl, reading Q10): ghost fill, con2prim + signal speeds + max reduction, three stage kernels.
+Prints ONE JSON line (rank 0).  N > 1 (torchrun): every rank advances its own independent 512^3 event
+(weak scaling, no data-path collective), time = max over ranks.
+
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same
+workload on the host cores; it is the only other place besides `cpu_baseline` where bench.py runs it.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1604_03360_b200 import workloads as W  # noqa: E402
+
+SCHEMES = {"weno5": W.WENO5, "weno7": W.WENO7, "musta": W.MUSTA_FORCE}
+# Algorithmic flops per cell per RK3 step and bytes per cell per RK3 step (
+# SURVEY.md 8(d)): add/mul/div/sqrt/max = 1, FMA = 2, every interface flux computed once.
+FLOPS_PER_CELL_STEP = {"weno5": 7041.0, "weno7": 14331.0, "musta": 3831.0}
+FLOPS_PER_CELL_L = {"weno5": 2327.0, "weno7": 4757.0, "musta": 1257.0}
+BYTES_PER_CELL_STEP = {"f64": 320.0, "f32": 160.0}
+# bytes one stage kernel moves per cell, averaged over the three stages of a step: 320/3 (fp64)
+METRIC = "3D cell-updates/s per RK3 step"
+UNIT = "cell-updates/s"
+CFL = 0.2
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return json.load(fh), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, power, reasons = [], None, [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for t, line in self.rows:
+            if not (t0 <= t <= t1 + 0.1):
+                continue
+            f = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(f[0]))
+                smax = float(f[1])
+                power.append(float(f[2]))
+            except Exception:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_workload(n, scheme, rank=0):
+    if n >= 64:
+        w = W.lumpy(n=n, hotspots=200, with_velocity=True, scheme=SCHEMES[scheme], nsteps=20, cfl=CFL,
+                    seed=W.SEED + rank)
+    else:
+        w = W.lumpy(n=n, hotspots=12, with_velocity=True, scheme=SCHEMES[scheme], box=n / 16.0, sigma_unit=0.12)
+    return w
+
+
+def crop_workload(w, m):
+    """m^3 corner crop of a workload, made periodic-by-fiat (the oracle sample of the same data)."""
+    cons = np.ascontiguousarray(w.cons[:, :m, :m, :m])
+    return W.Workload(w.name + "_crop%d" % m, (m, m, m), w.dx, (0.0, 0.0, 0.0), w.scheme, w.bc, cons, 0.0,
+                      cfl=w.cfl, nsteps=w.nsteps)
+
+
+def time_oracle(w, steps, warmup=0):
+    """Cell-updates/s of the oracle as it stands, single-threaded, on workload w."""
+    from oracle import oracle as O
+    o = O.from_workload(w)
+    for _ in range(warmup):
+        o.step(w.cfl * w.dx / o.max_signal_speed(), 1)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.step(w.cfl * w.dx / o.max_signal_speed(), 1)
+    dt = time.perf_counter() - t0
+    ncell = w.n[0] * w.n[1] * w.n[2]
+    o.close()
+    return ncell * steps / dt, dt
+
+
+# ----------------------------------------------------------------------------------------------
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    m = 48
+    big = make_workload(max(64, m), args.scheme)
+    w = crop_workload(big, m)
+    value, secs = time_oracle(w, args.steps, args.warmup)
+    sample = "%d^3 corner crop of the 200-hotspot lumpy state (64^3 draw), %d RK3 steps, 1 thread" % (m, args.steps)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(args.steps, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config5 lumpy periodic, %s fp64, oracle sample %s" % (args.scheme, sample),
+                   "scheme": args.scheme, "cfl": CFL},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ----------------------------------------------------------------------------------------------
+def timed_run(B, torch, w, precision, steps, warmup, dist=None, profile=True):
+    """Warm up, then time `steps` RK3 steps with CUDA events on the stream.  Returns a dict."""
+    prec = B.F32 if precision == "f32" else B.F64
+    h = B.from_workload(w, precision=prec)
+    stream = torch.cuda.current_stream()
+    h.step_cfl(CFL, warmup)
+    torch.cuda.synchronize()
+    if profile:
+        h.set_option("profile", 1)
+    l0 = h.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    e0.record(stream)
+    for _ in range(steps):
+        h.step_cfl(CFL, 1)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    if dist is not None:
+        dist.barrier()
+    ms = e0.elapsed_time(e1)
+    launches = h.launch_count - l0
+    stage_ms, stage_n = h.stage_kernel_time() if profile else (0.0, 0)
+    h.set_option("profile", 0)
+    status = h.status()
+    tnow = h.time
+    return dict(h=h, ms=ms, launches=launches, stage_ms=stage_ms, stage_n=stage_n, status=status, t=tnow,
+                wall=(t0, t1))
+
+
+def roofline(scheme, precision, ncell, stage_ms, stage_n, alu_peak_tf, peaks):
+    if stage_n == 0 or stage_ms <= 0:
+        return None
+    per_launch_s = stage_ms * 1e-3 / stage_n
+    flops = FLOPS_PER_CELL_L[scheme] * ncell
+    achieved = flops / per_launch_s / 1e12
+    byts = BYTES_PER_CELL_STEP[precision] / 3.0 * ncell
+    return {"bound": "alu", "achieved": achieved, "peak": alu_peak_tf, "unit": "TFLOP/s",
+            "frac": achieved / alu_peak_tf, "traffic": None,
+            "kernel": "stage kernel (L(u) + RK combine)", "launch_ms": per_launch_s * 1e3,
+            "hbm_gbs_achieved": byts / per_launch_s / 1e9, "hbm_frac": byts / per_launch_s / 1e9 / peaks["hbm_gbs"]}
+
+
+def run_ours(args):
+    import torch
+    if not torch.cuda.is_available():
+        print("bench.py: no CUDA device; the hot path has no CPU fallback", file=sys.stderr)
+        return 2
+    from paper_1604_03360_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist = dist_mod
+    peaks, peaks_src = measured_peaks()
+
+    n = args.n
+    ncell = n ** 3
+    w = make_workload(n, args.scheme, rank)
+
+    # ALU roofline denominator: 148 SMs x 64 fp64 (128 fp32) FMA lanes x 2 flop x
+    # the SM clock.  Nominal uses clocks.max.sm; the sustained figure is measured by the library's probe.
+    lanes = 64 if args.precision == "f64" else 128
+    sms = torch.cuda.get_device_properties(local).multi_processor_count
+    nominal_tf = sms * lanes * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+    probe_tf = B.probe_fma_peak(B.F64 if args.precision == "f64" else B.F32, 300)
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    r = timed_run(B, torch, w, args.precision, args.steps, args.warmup, dist)
+    clocks = sampler.stop(*r["wall"])
+    ms = r["ms"]
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = ncell * args.steps * world / (ms * 1e-3)
+    roof = roofline(args.scheme, args.precision, ncell, r["stage_ms"], r["stage_n"], nominal_tf, peaks)
+    if roof is not None:
+        roof["peak_source"] = ("nominal: %d SMs x %d lanes x 2 x %.0f MHz (DESIGN.md section 8); "
+                               "hbm peak %s" % (sms, lanes, peaks.get("sm_max_mhz", 1965.0), peaks_src))
+        roof["peak_probe_sustained"] = probe_tf
+        roof["frac_of_probe"] = roof["achieved"] / probe_tf if probe_tf > 0 else None
+        roof["stage_share_of_step"] = r["stage_ms"] / r["ms"]
+    # step-level roofline: cell-updates/s against min(byte roof, flop roof)
+    flop_roof = nominal_tf * 1e12 / FLOPS_PER_CELL_STEP[args.scheme]
+    byte_roof = peaks["hbm_gbs"] * 1e9 / BYTES_PER_CELL_STEP[args.precision]
+    step_roof = min(flop_roof, byte_roof)
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region
+    h = r.pop("h")
+    esz = 8 if args.precision == "f64" else 4
+    tdt = torch.float64 if args.precision == "f64" else torch.float32
+    host_in = torch.from_numpy(w.cons).to(tdt).pin_memory()
+    host_out = torch.empty_like(host_in).pin_memory()
+    h.set_state_host(host_in)          # warm the copy path
+    h.step_cfl(CFL, 1)
+    h.get_state_host(host_out)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    h.set_state_host(host_in)
+    h.step_cfl(CFL, args.steps)
+    h.get_state_host(host_out)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    state_bytes = 5 * ncell * esz
+    e2e = {"value": ncell * args.steps * world / e2e_s, "unit": UNIT,
+           "h2d_bytes_per_step": state_bytes / max(args.steps, 1),
+           "d2h_bytes_per_step": state_bytes / max(args.steps, 1),
+           "job": "hydro_set_state_host (pinned) + hydro_step_cfl(%d) + hydro_get_state_host; "
+                  "state %d bytes each way per job" % (args.steps, state_bytes),
+           "finite": bool(torch.isfinite(host_out).all().item())}
+    launches_per_step = r["launches"] / max(args.steps, 1)
+    h.close()
+    del h
+    torch.cuda.empty_cache()
+
+    # ---- the other headline variants of config 5 (same grid, fewer steps each)
+    variants = {}
+    if not args.no_variants and rank == 0 and world == 1:
+        for sch, prec in (("weno5", "f64"), ("weno7", "f64"), ("musta", "f64"), ("weno5", "f32"), ("weno7", "f32")):
+            if (sch, prec) == (args.scheme, args.precision):
+                continue
+            w.scheme = SCHEMES[sch]
+            vr = timed_run(B, torch, w, prec, max(3, args.steps // 4), 3)
+            vsteps = max(3, args.steps // 4)
+            lanes_v = 64 if prec == "f64" else 128
+            nom_v = sms * lanes_v * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+            rf = roofline(sch, prec, ncell, vr["stage_ms"], vr["stage_n"], nom_v, peaks)
+            variants["%s_%s" % (sch, prec)] = {
+                "value": ncell * vsteps / (vr["ms"] * 1e-3), "ms_per_step": vr["ms"] / vsteps, "steps": vsteps,
+                "roofline_frac": rf["frac"] if rf else None, "status": vr["status"]}
+            vr.pop("h").close()
+            torch.cuda.empty_cache()
+        w.scheme = SCHEMES[args.scheme]
+
+    # ---- the oracle beside it: bounded sample on the host cores (rank 0, N = 1 only)
+    cpu = None
+    if not args.no_cpu_baseline and rank == 0 and world == 1:
+        m = min(64, n)
+        cw = crop_workload(w, m)
+        v, secs = time_oracle(cw, 8 if m >= 64 else 20)
+        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": "%d^3 corner crop of the same state, %d RK3 steps, %.1f s, single thread" %
+                         (m, 8 if m >= 64 else 20, secs)}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / max(args.steps, 1), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
+            "config": {"workload": "BASELINE.json configs[4]: %d^3 periodic lumpy state, 200 hotspots, blended "
+                                   "velocities, %s %s, CFL %.1f (one independent event per GPU)" %
+                                   (n, args.scheme, args.precision, CFL),
+                       "grid": [n, n, n], "scheme": args.scheme, "cfl": CFL,
+                       "l2": "no flush needed: the state (%.2f GB per copy) is far larger than the 126 MB L2" %
+                             (state_bytes / 1e9)},
+            "roofline": roof,
+            "step_roofline": {"value": value / world, "roof": step_roof, "frac": value / world / step_roof,
+                              "flop_roof": flop_roof, "byte_roof": byte_roof, "unit": UNIT,
+                              "note": "min(hbm peak / 320 B, nominal ALU peak / algorithmic flops) per cell-update"},
+            "cpu_baseline": cpu,
+            "e2e": e2e,
+            "gpu_launches": int(round(launches_per_step * args.steps)),
+            "launches_per_step": launches_per_step,
+            "clocks": clocks,
+            "status": r["status"], "sim_time": r["t"],
+            "variants": variants,
+            "context": "paper: GPU ~200x one CPU thread for MUSTA-FORCE on unnamed 2016 hardware (PAPER.md:38)",
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--scheme", default="weno5", choices=sorted(SCHEMES))
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--n", type=int, default=512)
+    ap.add_argument("--no-variants", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -70,6 +70,8 @@ int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme)
  *   "x0|y0|z0"      coordinate of the low face of the domain on each axis
  *   "hubble_t0|hubble_e0|hubble_n0|hubble_bx|hubble_by|hubble_bz"  parameters of the closed-form
  *                   Hubble flow used by HYDRO_BC_HUBBLE (readings Q13, Q14)
+ *   "profile"       0 (default) | 1: record a CUDA event pair on the stream around every stage-kernel
+ *                   launch, read back with hydro_stage_kernel_time
  *   "kernel"        HYDRO_KERNEL_AUTO (default: fused stage kernel where the grid allows, else the
  *                   generic one) | HYDRO_KERNEL_GENERIC | HYDRO_KERNEL_FUSED (EINVAL at step time if
  *                   the grid does not allow it)
@@ -123,6 +125,11 @@ int hydro_status(hydro_ctx *ctx);
 
 /* Number of kernels the context has launched since creation (bench.py "gpu_launches"). */
 long long hydro_launch_count(const hydro_ctx *ctx);
+
+/* With the "profile" option on: total device time in milliseconds of the stage kernels (the L(u) +
+ * Runge-Kutta kernel, the dominant one) launched since the last call, and their number, written to HOST
+ * pointers.  Synchronises the stream and clears the record. */
+int hydro_stage_kernel_time(hydro_ctx *ctx, double *ms_total_host, long long *launches_host);
 
 /* Text of the last error on this context ("" if none).  Valid until the next call on the context. */
 const char *hydro_last_error(const hydro_ctx *ctx);

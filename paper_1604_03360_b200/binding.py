@@ -24,7 +24,7 @@ SYMBOLS = [
     "hydro_create", "hydro_set_option", "hydro_set_stream", "hydro_workspace_bytes", "hydro_bind_workspace",
     "hydro_set_state", "hydro_get_state", "hydro_set_state_host", "hydro_get_state_host", "hydro_step",
     "hydro_step_cfl", "hydro_max_signal_speed", "hydro_eval_L", "hydro_get_time", "hydro_status",
-    "hydro_launch_count", "hydro_last_error", "hydro_destroy", "hydro_probe_fma_peak",
+    "hydro_launch_count", "hydro_stage_kernel_time", "hydro_last_error", "hydro_destroy", "hydro_probe_fma_peak",
 ]
 
 
@@ -59,6 +59,7 @@ def _load():
     L.hydro_status.argtypes = [vp]
     L.hydro_launch_count.argtypes = [vp]
     L.hydro_launch_count.restype = ctypes.c_longlong
+    L.hydro_stage_kernel_time.argtypes = [vp, pd, ctypes.POINTER(ctypes.c_longlong)]
     L.hydro_last_error.argtypes = [vp]
     L.hydro_last_error.restype = ctypes.c_char_p
     L.hydro_destroy.argtypes = [vp]
@@ -172,6 +173,12 @@ class Hydro:
     @property
     def launch_count(self):
         return lib.hydro_launch_count(self._h)
+
+    def stage_kernel_time(self):
+        """(total ms, launches) of the stage kernels since the last call ("profile" option)."""
+        ms, n = ctypes.c_double(), ctypes.c_longlong()
+        self._check(lib.hydro_stage_kernel_time(self._h, ctypes.byref(ms), ctypes.byref(n)))
+        return ms.value, n.value
 
     def close(self):
         if getattr(self, "_h", None):

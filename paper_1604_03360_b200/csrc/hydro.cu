@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <vector>
 
 #include "../../include/hydro.h"
 #include "grid.cuh"
@@ -39,6 +40,9 @@ struct hydro_ctx {
     FusedPlan fused;                            // tensor maps etc. for the fused kernel
     bool fused_ready = false;
     long long launches = 0;
+    // "profile" option: CUDA events around every stage-kernel launch (bench.py roofline)
+    int profile = 0;
+    std::vector<cudaEvent_t> ev;  // pairs (start, stop), recorded on the stream
     std::string err;
 };
 
@@ -160,9 +164,26 @@ bool want_fused(const hydro_ctx* c) {
     return fused_supported(c->G, c->scheme, c->precision);
 }
 
+// records an event pair around the stage kernel when the "profile" option is on
+struct StageTimer {
+    hydro_ctx* c;
+    explicit StageTimer(hydro_ctx* c_) : c(c_) {
+        if (!c->profile) return;
+        cudaEvent_t e0, e1;
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { c->profile = 0; return; }
+        c->ev.push_back(e0);
+        c->ev.push_back(e1);
+        cudaEventRecord(e0, c->stream);
+    }
+    ~StageTimer() {
+        if (c->profile && !c->ev.empty()) cudaEventRecord(c->ev.back(), c->stream);
+    }
+};
+
 template <class T>
 int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double cb, int mode) {
     const StageArgs A = stage_args(c, ca, cb, mode);
+    StageTimer timer(c);
     if (want_fused(c)) {
         if (!c->fused_ready) return fail(c, HYDRO_ECUDA, "fused plan not built: %s", c->fused.err);
         const int rc = launch_fused<T>(c->fused, c->G, c->scheme, A, Us, (const T*)c->W, Un, Uout, c->ctl, c->stream);
@@ -256,7 +277,11 @@ int hydro_create(hydro_ctx** out, int nx, int ny, int nz, double dx, int scheme)
     return HYDRO_OK;
 }
 
-void hydro_destroy(hydro_ctx* c) { delete c; }
+void hydro_destroy(hydro_ctx* c) {
+    if (!c) return;
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    delete c;
+}
 
 const char* hydro_last_error(const hydro_ctx* c) { return c ? c->err.c_str() : "null context"; }
 
@@ -281,6 +306,8 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
         const int p = (int)v;
         if (p < 0 || p > 2) return fail(c, HYDRO_EINVAL, "kernel must be 0, 1 or 2");
         c->kernel = p;
+    } else if (k == "profile") {
+        c->profile = v != 0.0;
     } else if (k == "bc_x" || k == "bc_y" || k == "bc_z") {
         const int b = (int)v;
         if (b < 0 || b > 2) return fail(c, HYDRO_EINVAL, "unknown boundary rule %d", b);
@@ -437,6 +464,22 @@ int hydro_eval_L(hydro_ctx* c, const void* cons, double t_stage, void* L_out) {
     if (!cons || !L_out) return HYDRO_EINVAL;
     return c->precision == HYDRO_F64 ? eval_L_impl<double>(c, cons, t_stage, L_out)
                                      : eval_L_impl<float>(c, cons, t_stage, L_out);
+}
+
+int hydro_stage_kernel_time(hydro_ctx* c, double* ms_total_host, long long* launches_host) {
+    if (!c || !ms_total_host || !launches_host) return HYDRO_EINVAL;
+    CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    double total = 0.0;
+    for (size_t i = 0; i + 1 < c->ev.size(); i += 2) {
+        float ms = 0.f;
+        CUDA_OK(c, cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]));
+        total += ms;
+    }
+    *ms_total_host = total;
+    *launches_host = (long long)(c->ev.size() / 2);
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    c->ev.clear();
+    return HYDRO_OK;
 }
 
 int hydro_get_time(hydro_ctx* c, double* t_host) {

@@ -1,0 +1,347 @@
+"""Parity of the CUDA path (through the C ABI, include/hydro.h) against the CPU oracle, element by
+element on the same seeded inputs.  All tests here need a B200 (`-m gpu`).
+
+Tolerances (BASELINE.json north_star): max relative difference <= 1e-12 per RK stage and <= 1e-9 after
+100 steps in fp64; <= 1e-4 after 100 steps for the fp32 variant against the fp64 oracle (reading Q17).
+"max relative difference" is reading Q12: per field
+    max_cells |gpu - oracle| / max(max_cells |oracle|, 1e-30 + 1e-15 max_cells |E|),
+so identically-zero fields are judged against the energy scale.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1604_03360_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_STAGE = 1e-12
+TOL_100 = 1e-9
+TOL_100_F32 = 1e-4
+SCHEMES = [W.WENO5, W.WENO7, W.MUSTA_FORCE]
+NAMES = {W.WENO5: "weno5", W.WENO7: "weno7", W.MUSTA_FORCE: "musta"}
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_1604_03360_b200 import binding
+    return binding
+
+
+def reldiff(gpu, ora, scale=None):
+    """Reading Q12.  `scale` = the energy-like scale for the floor (default: max |field 0| of ora)."""
+    gpu = np.asarray(gpu, dtype=np.float64)
+    ora = np.asarray(ora, dtype=np.float64)
+    assert gpu.shape == ora.shape
+    assert np.all(np.isfinite(gpu)), "non-finite values from the CUDA path"
+    s0 = np.max(np.abs(ora[0])) if scale is None else scale
+    worst = 0.0
+    for c in range(ora.shape[0]):
+        den = max(np.max(np.abs(ora[c])), 1e-30 + 1e-15 * s0)
+        worst = max(worst, float(np.max(np.abs(gpu[c] - ora[c])) / den))
+    return worst
+
+
+def to_dev(B, a, dtype=None):
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(a)).to("cuda")
+    return t if dtype is None else t.to(dtype)
+
+
+def small_workload(scheme, n, bc=W.BC_PERIODIC, seed=W.SEED):
+    """Config-5-like lumpy state with velocities on a small, non-cubic, ragged grid (n = (nx,ny,nz))."""
+    w = W.lumpy(n=max(n), hotspots=12, with_velocity=True, scheme=scheme, box=max(n) / 16.0,
+                sigma_unit=0.12, seed=seed)
+    cons = np.ascontiguousarray(w.cons[:, :n[2], :n[1], :n[0]])
+    return W.Workload(w.name, tuple(n), w.dx, (0.0, 0.0, 0.0), scheme, (bc,) * 3, cons, 0.0, cfl=0.2, nsteps=0)
+
+
+# ------------------------------------------------------------------ a2-a4: max signal speed
+@pytest.mark.parametrize("n", [(37, 21, 19), (64, 1, 1), (1, 33, 1), (1, 1, 40), (48, 20, 1)])
+def test_max_signal_speed(B, oracle, n):
+    scheme = W.WENO5
+    cons = W.random_state((n[2], n[1], n[0]), seed=7, vmax=0.9)
+    w = W.Workload("rand", n, 0.1, (0, 0, 0), scheme, (W.BC_OUTFLOW,) * 3, cons)
+    h = B.from_workload(w)
+    o = oracle.from_workload(w)
+    a, b = h.max_signal_speed(), o.max_signal_speed()
+    assert 0.0 < b < 1.0
+    assert abs(a - b) <= 4e-16 * b + 1e-16, (a, b)
+    assert h.status() == 0
+    h.close()
+
+
+# ------------------------------------------------------------------ one L(u): every scheme, BC, shape
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("bc", [W.BC_PERIODIC, W.BC_OUTFLOW])
+@pytest.mark.parametrize("n", [(37, 21, 19), (70, 9, 13), (16, 16, 40)])
+def test_L_matches_oracle(B, oracle, scheme, bc, n):
+    w = small_workload(scheme, n, bc)
+    h = B.from_workload(w)
+    o = oracle.from_workload(w)
+    Lo = o.eval_L(w.cons)
+    Lg = h.eval_L(to_dev(B, w.cons)).cpu().numpy()
+    # natural scale of L: energy / dx
+    assert reldiff(Lg, Lo, scale=np.max(np.abs(w.cons[0])) / w.dx) <= TOL_STAGE
+    assert h.status() == 0
+    h.close()
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("n", [(50, 1, 1), (1, 50, 1), (1, 1, 50), (24, 30, 1), (1, 24, 30), (24, 1, 30)])
+def test_L_with_inactive_axes(B, oracle, scheme, n):
+    cons = W.random_state((n[2], n[1], n[0]), seed=11, vmax=0.7)
+    w = W.Workload("rand", n, 0.05, (0, 0, 0), scheme, (W.BC_OUTFLOW, W.BC_PERIODIC, W.BC_OUTFLOW), cons)
+    h = B.from_workload(w)
+    o = oracle.from_workload(w)
+    Lo = o.eval_L(w.cons)
+    Lg = h.eval_L(to_dev(B, w.cons)).cpu().numpy()
+    assert reldiff(Lg, Lo, scale=np.max(np.abs(w.cons[0])) / w.dx) <= TOL_STAGE
+    h.close()
+
+
+@pytest.mark.parametrize("scheme,g", [(W.WENO5, 3), (W.WENO7, 4), (W.MUSTA_FORCE, 2)])
+def test_L_on_the_smallest_legal_grid(B, oracle, scheme, g):
+    """Degenerate case: every active axis exactly as long as the ghost width."""
+    n = (g, g, g)
+    cons = W.random_state((g, g, g), seed=3, vmax=0.5)
+    for bc in (W.BC_PERIODIC, W.BC_OUTFLOW):
+        w = W.Workload("tiny", n, 0.1, (0, 0, 0), scheme, (bc,) * 3, cons)
+        h = B.from_workload(w)
+        o = oracle.from_workload(w)
+        Lg = h.eval_L(to_dev(B, w.cons)).cpu().numpy()
+        assert reldiff(Lg, o.eval_L(w.cons), scale=np.max(np.abs(cons[0])) / w.dx) <= TOL_STAGE
+        h.close()
+
+
+def test_single_cell_grid_is_a_fixed_point(B):
+    """1 x 1 x 1: no active axis, L = 0, stepping leaves the state alone, max speed is 0."""
+    cons = W.random_state((1, 1, 1), seed=5)
+    w = W.Workload("one", (1, 1, 1), 0.1, (0, 0, 0), W.WENO5, (W.BC_OUTFLOW,) * 3, cons)
+    h = B.from_workload(w)
+    assert np.all(h.eval_L(to_dev(B, cons)).cpu().numpy() == 0.0)
+    h.step(0.01, 2)
+    out = h.get_state().cpu().numpy()
+    assert np.max(np.abs(out - cons) / np.abs(cons)) < 1e-15
+    assert h.max_signal_speed() == 0.0
+    h.close()
+
+
+# ------------------------------------------------------------------ per-stage parity of one RK3 step
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("bc", [W.BC_PERIODIC, W.BC_OUTFLOW])
+def test_one_step_matches_oracle_per_stage_tolerance(B, oracle, scheme, bc):
+    w = small_workload(scheme, (45, 23, 18), bc)
+    h = B.from_workload(w)
+    o = oracle.from_workload(w)
+    dt = w.cfl * w.dx / o.max_signal_speed()
+    o.step(dt, 1)
+    h.step(dt, 1)
+    assert reldiff(h.get_state().cpu().numpy(), o.get_state()) <= 3 * TOL_STAGE   # three stages
+    assert abs(h.time - o.time) <= 1e-15
+    h.close()
+
+
+def test_zero_steps_is_a_no_op(B):
+    w = small_workload(W.WENO5, (20, 12, 9))
+    h = B.from_workload(w)
+    h.step(0.01, 0)
+    assert np.array_equal(h.get_state().cpu().numpy(), w.cons)
+    assert h.time == 0.0
+    h.close()
+
+
+# ------------------------------------------------------------------ state round trip, host entry points
+@pytest.mark.parametrize("prec", [0, 1])
+def test_set_get_state_round_trip_device_and_host(B, prec):
+    import torch
+    w = small_workload(W.WENO7, (33, 17, 10))
+    h = B.from_workload(w, precision=prec)
+    ref = torch.from_numpy(w.cons).to(h.dtype)
+    assert torch.equal(h.get_state().cpu(), ref)
+    host_in = ref.clone().pin_memory()
+    host_out = torch.empty_like(host_in).pin_memory()
+    h.set_state_host(host_in * 2)
+    h.get_state_host(host_out)
+    assert torch.equal(host_out, ref * 2)
+    h.close()
+
+
+# ------------------------------------------------------------------ 100 steps, fp64 and fp32
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_100_steps_fp64(B, oracle, scheme):
+    w = small_workload(scheme, (28, 20, 24))
+    o = oracle.from_workload(w)
+    w.nsteps = 100
+    dts = oracle.run(o, w)
+    h = B.from_workload(w)
+    for dt in dts:
+        h.step(dt, 1)
+    d = reldiff(h.get_state().cpu().numpy(), o.get_state())
+    assert d <= TOL_100, d
+    assert np.max(np.abs(o.get_state() - w.cons)) > 1e-3      # the state really evolved
+    assert h.status() == 0
+    h.close()
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_100_steps_fp32_against_fp64_oracle(B, oracle, scheme):
+    w = small_workload(scheme, (28, 20, 24))
+    o = oracle.from_workload(w)
+    w.nsteps = 100
+    dts = oracle.run(o, w)
+    h = B.from_workload(w, precision=B.F32)
+    for dt in dts:
+        h.step(dt, 1)
+    d = reldiff(h.get_state().cpu().numpy(), o.get_state())
+    assert d <= TOL_100_F32, d
+    h.close()
+
+
+def test_step_cfl_follows_the_oracle_dt_sequence(B, oracle):
+    """Device-resident dt = cfl dx / max speed (Q10) reproduces the oracle's host-side sequence."""
+    for sch in (W.WENO5, W.MUSTA_FORCE):
+        w2 = small_workload(sch, (30, 22, 17))
+        o2 = oracle.from_workload(w2)
+        w2.nsteps = 10
+        dts = oracle.run(o2, w2)
+        h = B.from_workload(w2)
+        h.step_cfl(w2.cfl, 10)
+        assert abs(h.time - sum(dts)) <= 1e-12 * sum(dts)
+        assert reldiff(h.get_state().cpu().numpy(), o2.get_state()) <= 1e-10
+        h.close()
+
+
+# ------------------------------------------------------------------ config 1: Sod tube, full size
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_config1_sod_full_run(B, oracle, scheme):
+    import exact
+    w = W.sod(scheme=scheme)
+    o = oracle.from_workload(w)
+    dts = oracle.run(o, w)
+    h = B.from_workload(w)
+    for dt in dts:
+        h.step(dt, 1)
+    ug = h.get_state().cpu().numpy()
+    assert reldiff(ug, o.get_state()) <= 3 * TOL_100        # 300 steps
+    # and against the exact Riemann solution (not the oracle): L1 error of the charge density
+    x = W.cell_centres(400, w.dx, -1.0)
+    t_end = sum(dts)
+    e_ex, n_ex, v_ex = exact.sod_exact(x, t_end)
+    prim = np.array([oracle.con2prim(ug[:, 0, 0, i])[0] for i in range(400)])
+    l1 = np.sum(np.abs(prim[:, 2] - n_ex)) * w.dx
+    assert l1 < (1.2e-2 if scheme == W.MUSTA_FORCE else 6e-3), l1
+    h.close()
+
+
+# ------------------------------------------------------------------ config 2: Hubble flow, analytic ghosts
+@pytest.mark.parametrize("scheme", [W.WENO5, W.WENO7])
+def test_config2_hubble_reduced(B, oracle, scheme):
+    """Config 2 at 24^3 (same domain, t0, dt/dx): analytic ghost fill at the three stage times."""
+    w = W.hubble(n=24, scheme=scheme, nsteps=12)
+    o = oracle.from_workload(w)
+    dts = oracle.run(o, w)
+    h = B.from_workload(w)
+    h.step(w.dt, w.nsteps)
+    assert abs(h.time - o.time) < 1e-12
+    assert reldiff(h.get_state().cpu().numpy(), o.get_state()) <= 1e-10
+    # per-stage operator at a stage time different from the context's
+    Lo = o.eval_L(w.cons, 8.1)
+    Lg = h.eval_L(to_dev(B, w.cons), 8.1).cpu().numpy()
+    assert reldiff(Lg, Lo, scale=np.max(np.abs(w.cons[0])) / w.dx) <= TOL_STAGE
+    h.close()
+
+
+def test_config2_hubble_full_size_against_closed_form(B):
+    """Config 2 itself (128^3, 100 steps, WENO5) against the closed form (Q13), no oracle involved."""
+    w = W.hubble()
+    h = B.from_workload(w)
+    h.step(w.dt, w.nsteps)
+    t = h.time
+    assert abs(t - (8.0 + 100 * w.dt)) < 1e-12
+    c = W.cell_centres(128, w.dx, -4.0)
+    e, n, vx, vy, vz = W.hubble_fields(c[None, None, :], c[None, :, None], c[:, None, None], t, 8.0, 1.0, 1.0)
+    exact_cons = W.prim_to_cons(e, n, vx, vy, vz)
+    ug = h.get_state().cpu().numpy()
+    err = np.max(np.abs(ug[0] - exact_cons[0]) / exact_cons[0])
+    assert err < 1e-4, err
+    assert h.status() == 0
+    h.close()
+
+
+# ------------------------------------------------------------------ config 3 reduced: WENO7, outflow
+def test_config3_ellipsoidal_reduced(B, oracle):
+    w = W.ellipsoidal(n=24, nsteps=8)
+    o = oracle.from_workload(w)
+    dts = oracle.run(o, w)
+    h = B.from_workload(w)
+    for dt in dts:
+        h.step(dt, 1)
+    assert reldiff(h.get_state().cpu().numpy(), o.get_state()) <= 1e-10
+    h.close()
+
+
+# ------------------------------------------------------------------ config 4 reduced + conservation
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_conservation_on_periodic_grid(B, scheme):
+    w = W.lumpy(n=64, hotspots=40, scheme=scheme, nsteps=10)
+    h = B.from_workload(w)
+    tot0 = [math.fsum(w.cons[c].ravel()) for c in range(5)]
+    h.step_cfl(0.2, 10)
+    u = h.get_state().cpu().numpy()
+    tot1 = [math.fsum(u[c].ravel()) for c in range(5)]
+    assert np.max(np.abs(u - w.cons)) > 1e-4
+    for a, b in zip(tot0, tot1):
+        assert abs(a - b) <= 1e-13 * tot0[0], (tot0, tot1)
+    h.close()
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_uniform_state_is_preserved(B, scheme):
+    n = (40, 24, 20)
+    u0 = W.prim_to_cons(np.array(1.7), np.array(0.3), np.array(0.31), np.array(-0.22), np.array(0.13))
+    u = np.broadcast_to(u0.reshape(5, 1, 1, 1), (5, n[2], n[1], n[0])).copy()
+    w = W.Workload("uniform", n, 0.1, (0, 0, 0), scheme, (W.BC_PERIODIC, W.BC_OUTFLOW, W.BC_PERIODIC), u)
+    h = B.from_workload(w)
+    L = h.eval_L(to_dev(B, u)).cpu().numpy()
+    # both faces of a cell evaluate identical arithmetic on identical data
+    assert np.all(L == 0.0)
+    h.step(0.02, 3)
+    out = h.get_state().cpu().numpy()
+    assert np.max(np.abs(out - u) / np.abs(u0).reshape(5, 1, 1, 1)) < 3e-15
+    h.close()
+
+
+# ------------------------------------------------------------------ Q16: unphysical cells raise the flag
+def test_unphysical_state_raises_the_sticky_flag(B, oracle):
+    w = small_workload(W.WENO5, (20, 12, 9))
+    bad = w.cons.copy()
+    bad[1, 4, 5, 6] = 5.0 * bad[0, 4, 5, 6]      # |M| > E
+    h = B.from_workload(w)
+    assert h.status() == 0
+    h.set_state(to_dev(B, bad))
+    h.step(1e-4, 1)
+    assert h.status() == B.EUNPHYSICAL
+    h.set_state(to_dev(B, w.cons))                # set_state clears it
+    h.step(1e-4, 1)
+    assert h.status() == 0
+    h.close()
+
+
+# ------------------------------------------------------------------ kernel variants agree
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("prec", [0, 1])
+def test_fused_and_generic_kernels_agree(B, scheme, prec):
+    """The tiled stage kernel against the one-thread-per-cell one on a grid spanning several tiles with
+    ragged tails in every direction."""
+    w = small_workload(scheme, (150, 37, 29))
+    outs = []
+    for kern in (B.KERNEL_GENERIC, B.KERNEL_AUTO):
+        h = B.from_workload(w, precision=prec, kernel=kern)
+        h.step_cfl(0.2, 3)
+        outs.append(h.get_state().cpu().numpy())
+        h.close()
+    assert reldiff(outs[1], outs[0]) <= (1e-12 if prec == 0 else 1e-4)
