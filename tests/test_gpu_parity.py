@@ -93,13 +93,16 @@ def test_L_matches_oracle(B, oracle, scheme, bc, n):
 @pytest.mark.parametrize("scheme", SCHEMES)
 @pytest.mark.parametrize("n", [(50, 1, 1), (1, 50, 1), (1, 1, 50), (24, 30, 1), (1, 24, 30), (24, 1, 30)])
 def test_L_with_inactive_axes(B, oracle, scheme, n):
-    cons = W.random_state((n[2], n[1], n[0]), seed=11, vmax=0.7)
+    # cell-to-cell white noise; |v| <= 0.5 keeps every MUSCL / MUSTA intermediate state admissible (with 0.7
+    # the Q16 clamp fires in the oracle too, and a clamped state is conditioned like 1/1e-12: no parity bar)
+    cons = W.random_state((n[2], n[1], n[0]), seed=11, vmax=0.5)
     w = W.Workload("rand", n, 0.05, (0, 0, 0), scheme, (W.BC_OUTFLOW, W.BC_PERIODIC, W.BC_OUTFLOW), cons)
     h = B.from_workload(w)
     o = oracle.from_workload(w)
     Lo = o.eval_L(w.cons)
     Lg = h.eval_L(to_dev(B, w.cons)).cpu().numpy()
     assert reldiff(Lg, Lo, scale=np.max(np.abs(w.cons[0])) / w.dx) <= TOL_STAGE
+    assert h.status() == 0
     h.close()
 
 
