@@ -154,10 +154,15 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------------------------
+SPLIT_Z = None  # --split-z: override the library's default stage decomposition (experiments)
+
+
 def timed_run(B, torch, w, precision, steps, warmup, dist=None, profile=True):
     """Warm up, then time `steps` RK3 steps with CUDA events on the stream.  Returns a dict."""
     prec = B.F32 if precision == "f32" else B.F64
     h = B.from_workload(w, precision=prec)
+    if SPLIT_Z is not None:
+        h.set_option("split_z", SPLIT_Z)
     stream = torch.cuda.current_stream()
     h.step_cfl(CFL, warmup)
     torch.cuda.synchronize()
@@ -356,7 +361,10 @@ def main():
     ap.add_argument("--n", type=int, default=512)
     ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--split-z", type=int, default=None, choices=[0, 1])
     args = ap.parse_args()
+    global SPLIT_Z
+    SPLIT_Z = args.split_z
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

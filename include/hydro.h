@@ -70,6 +70,8 @@ int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme)
  *   "x0|y0|z0"      coordinate of the low face of the domain on each axis
  *   "hubble_t0|hubble_e0|hubble_n0|hubble_bx|hubble_by|hubble_bz"  parameters of the closed-form
  *                   Hubble flow used by HYDRO_BC_HUBBLE (readings Q13, Q14)
+ *   "split_z"       1 (default): a stage is the x/y tiled kernel followed by the z sweep kernel;
+ *                   0: one kernel with the z register window inside
  *   "profile"       0 (default) | 1: record a CUDA event pair on the stream around every stage-kernel
  *                   launch, read back with hydro_stage_kernel_time
  *   "kernel"        HYDRO_KERNEL_AUTO (default: fused stage kernel where the grid allows, else the

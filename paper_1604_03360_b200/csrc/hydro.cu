@@ -186,9 +186,10 @@ int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double 
     StageTimer timer(c);
     if (want_fused(c)) {
         if (!c->fused_ready) return fail(c, HYDRO_ECUDA, "fused plan not built: %s", c->fused.err);
-        const int rc = launch_fused<T>(c->fused, c->G, c->scheme, A, Us, (const T*)c->W, Un, Uout, c->ctl, c->stream);
+        int nl = 0;
+        const int rc = launch_fused<T>(c->fused, c->G, c->scheme, A, Us, (const T*)c->W, Un, Uout, c->ctl, c->stream, &nl);
         if (rc != 0) return fail(c, HYDRO_ECUDA, "fused launch: %s", c->fused.err);
-        ++c->launches;
+        c->launches += nl;
         return HYDRO_OK;
     }
     if (c->kernel == HYDRO_KERNEL_FUSED)
@@ -306,6 +307,8 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
         const int p = (int)v;
         if (p < 0 || p > 2) return fail(c, HYDRO_EINVAL, "kernel must be 0, 1 or 2");
         c->kernel = p;
+    } else if (k == "split_z") {
+        c->fused.split_z = v != 0.0;
     } else if (k == "profile") {
         c->profile = v != 0.0;
     } else if (k == "bc_x" || k == "bc_y" || k == "bc_z") {

@@ -1,11 +1,347 @@
-// kernel_fused.cuh -- placeholder until the fused stage kernel lands (next commit).
+// kernel_fused.cuh -- the tiled stage kernels: L(u) of Eq. (2) fused with the SSP-RK3
+// combination (a9), every interface flux computed once.
+//
+// stage_tiled_kernel<T, SCHEME, WITH_Z>
+//   A block is 32 x TY threads over an (x, y) tile and marches along z through a chunk of planes.  Thread
+//   (lane, ty) sits on cell (i0 + lane, j0 + ty), i0 = 31 bx - 1, j0 = (TY-1) by - 1: column lane = 0 and
+//   row ty = 0 are helper positions one cell below the tile, the other 31 x (TY-1) positions own a cell.
+//   Per plane the halo'd rectangle of the tile (conserved fields, winv, p, a_x, a_y; R-1 / R cells of halo)
+//   is brought into shared memory with cp.async, double buffered one plane ahead, and a thread computes
+//   only UPPER-face fluxes from it:
+//     x: f(i+1/2) by every thread of an owning row     -> lower face from lane-1 by warp shuffle
+//     y: f(j+1/2) by every thread of an owning column  -> lower face from row ty-1 through shared memory
+//   WITH_Z: z: f(k+1/2) by owning threads from a register window of the column (cells k-R+1 .. k+R,
+//     shifted and refilled by one prefetched plane per step) -> lower face is last plane's flux.
+//   Redundant work: one column of x-fluxes per 31, one row of y-fluxes per TY-1, one z-flux per chunk.
+// z_sweep_kernel<T, SCHEME>   (used when the stage is split: tiled kernel without z, then this)
+//   thread per (i, j) column marching along z with the same register window, adds the z-flux difference
+//   to the output of the x/y kernel.  No shared memory, no barrier, no redundancy except one flux per chunk.
 #pragma once
+#include <cstdio>
+
 #include "grid.cuh"
 #include "kernel_generic.cuh"
+
 namespace hydro {
-struct FusedPlan { char err[256] = {0}; };
-inline bool fused_supported(const Geom&, int, int) { return false; }
-inline int build_fused_plan(FusedPlan&, const Geom&, int, int) { return -1; }
-template <class T>
-int launch_fused(FusedPlan&, const Geom&, int, const StageArgs&, const T*, const T*, const T*, T*, Ctl*, cudaStream_t) { return -1; }
+
+constexpr int FUSED_TY = 8;     // rows per block (one of them the helper row)
+constexpr int FUSED_ZC = 64;    // planes per z-chunk of the tiled kernel
+constexpr int ZSWEEP_ZC = 128;  // planes per z-chunk of the z sweep
+
+struct FusedPlan {
+    int split_z = 1;  // 1: x/y tiled kernel + z sweep kernel; 0: one kernel with the z window inside
+    char err[256] = {0};
+};
+
+inline bool fused_supported(const Geom& G, int /*scheme*/, int /*precision*/) {
+    return G.g[0] > 0 && G.g[1] > 0 && G.g[2] > 0;
 }
+
+template <class T>
+__device__ __forceinline__ T shfl_up1(T v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void* smem, const void* gmem) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(s), "l"(gmem), "n"(BYTES) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// z-stencil of one column held in registers while the block marches along z: cells k-R+1 .. k+R, per cell
+// the five conserved fields and (WENO only) winv, p, a_z.  All indices are compile-time constants after
+// unrolling, so the arrays live in registers.
+template <class T, int SCHEME>
+struct ZWindow {
+    static constexpr int R = SCHEME == 0 ? 3 : (SCHEME == 1 ? 4 : 2);
+    static constexpr int M = 2 * R;
+    static constexpr int NWZ = SCHEME == 2 ? 0 : 3;  // winv, p, a_z
+    static constexpr int NV = NF + NWZ;
+    T uu[NF][M];
+    T ww[NWZ > 0 ? NWZ : 1][M];
+    __device__ __forceinline__ T u(int c, int k) const { return uu[c][k]; }
+    __device__ __forceinline__ T w(int a, int k) const { return ww[a == W_INV ? 0 : (a == W_P ? 1 : 2)][k]; }
+    // values of one cell, fetched ahead of use
+    static __device__ __forceinline__ void fetch(T v[NV], const T* __restrict__ U, const T* __restrict__ W,
+                                                 long long fs, long long q) {
+#pragma unroll
+        for (int c = 0; c < NF; ++c) v[c] = __ldg(U + c * fs + q);
+        if (NWZ > 0) {
+            v[NF + 0] = __ldg(W + W_INV * fs + q);
+            v[NF + 1] = __ldg(W + W_P * fs + q);
+            v[NF + 2] = __ldg(W + (W_AX + 2) * fs + q);
+        }
+    }
+    __device__ __forceinline__ void put(int m, const T v[NV]) {
+#pragma unroll
+        for (int c = 0; c < NF; ++c) uu[c][m] = v[c];
+#pragma unroll
+        for (int a = 0; a < NWZ; ++a) ww[a][m] = v[NF + a];
+    }
+    __device__ __forceinline__ void shift() {
+#pragma unroll
+        for (int m = 0; m + 1 < M; ++m) {
+#pragma unroll
+            for (int c = 0; c < NF; ++c) uu[c][m] = uu[c][m + 1];
+#pragma unroll
+            for (int a = 0; a < NWZ; ++a) ww[a][m] = ww[a][m + 1];
+        }
+    }
+};
+
+template <class T, int SCHEME, int DIR, class Acc>
+__device__ __forceinline__ void iface_from(const Acc& acc, const StageArgs& A, T fh[NF], int& flag) {
+    constexpr int R = SCHEME == 0 ? 3 : (SCHEME == 1 ? 4 : 2);
+    if constexpr (SCHEME == 2) musta_force_iface<T, DIR>(acc, A.musta_K, (T)A.musta_C, fh, flag);
+    else llf_weno_iface<T, R, DIR>(acc, (T)A.eps, fh);
+}
+
+// stencil accessor into the shared-memory rectangle: arrays 0..4 conserved, 5 winv, 6 p, 7 a_x, 8 a_y
+template <class T>
+struct RectAcc {
+    const T* base;
+    int stride, astride;
+    __device__ __forceinline__ T u(int c, int k) const { return base[c * astride + k * stride]; }
+    __device__ __forceinline__ T w(int a, int k) const { return base[(NF + a) * astride + k * stride]; }
+};
+
+template <int SCHEME>
+struct TileShape {
+    static constexpr int R = SCHEME == 0 ? 3 : (SCHEME == 1 ? 4 : 2);
+    static constexpr int RW = 32 + 2 * R - 1;         // rectangle width  (x)
+    static constexpr int RH = FUSED_TY + 2 * R - 1;   // rectangle height (y)
+    static constexpr int NA = SCHEME == 2 ? NF : NF + 4;  // arrays staged per plane
+    static constexpr int CELLS = RW * RH;
+    template <class T>
+    static constexpr size_t smem_bytes() { return sizeof(T) * (2 * (size_t)NA * CELLS + 2 * FUSED_TY * NF * 32); }
+};
+
+// bring the halo'd rectangle of plane kp (padded z index) into shared memory: one warp per (array, row)
+template <class T, int SCHEME>
+__device__ __forceinline__ void stage_plane(const Geom& G, const T* __restrict__ Us, const T* __restrict__ W,
+                                            T* rect, int x_lo_pad, int y_lo_pad, int kp) {
+    using S = TileShape<SCHEME>;
+    const int lane = threadIdx.x, warp = threadIdx.y;
+    const long long plane = (long long)kp * G.sxy;
+    for (int r = warp; r < S::NA * S::RH; r += FUSED_TY) {
+        const int arr = r / S::RH, yy = r - arr * S::RH;
+        const int yp = y_lo_pad + yy;
+        if (yp >= G.np[1]) continue;
+        const T* src = (arr < NF ? Us + (long long)arr * G.fs : W + (long long)(arr - NF) * G.fs) + plane +
+                       (long long)yp * G.sx + x_lo_pad;
+        T* dst = rect + (arr * S::RH + yy) * S::RW;
+        if (x_lo_pad + lane < G.np[0]) cp_async<sizeof(T)>(dst + lane, src + lane);
+        if (lane + 32 < S::RW && x_lo_pad + lane + 32 < G.np[0]) cp_async<sizeof(T)>(dst + lane + 32, src + lane + 32);
+    }
+}
+
+template <class T, int SCHEME, bool WITH_Z>
+__global__ void __launch_bounds__(32 * FUSED_TY, (WITH_Z || (SCHEME == 1 && sizeof(T) == 8)) ? 1 : 2)
+stage_tiled_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, const T* Un, T* Uout,
+                   Ctl* ctl) {
+    using S = TileShape<SCHEME>;
+    constexpr int R = S::R, M = 2 * R;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* rect = reinterpret_cast<T*>(smem_raw);                   // [2][NA][RH][RW]
+    T* fy_s = rect + 2 * S::NA * S::CELLS;                      // [2][TY][NF][32]
+    const int lane = threadIdx.x, ty = threadIdx.y;
+    const int i0 = (int)blockIdx.x * 31 - 1, j0 = (int)blockIdx.y * (FUSED_TY - 1) - 1;
+    const int i = i0 + lane, j = j0 + ty;
+    const int k0 = (int)blockIdx.z * FUSED_ZC;
+    const int k1 = min(k0 + FUSED_ZC, G.n[2]);
+    const bool row_ok = ty >= 1 && j < G.n[1];
+    const bool col_ok = lane >= 1 && i < G.n[0];
+    const bool own = row_ok && col_ok;
+    const bool need_x = row_ok && i < G.n[0];  // i >= -1 always
+    const bool need_y = col_ok && j < G.n[1];  // j >= -1 always
+    const int x_lo_pad = i0 - R + 1 + G.g[0], y_lo_pad = j0 - R + 1 + G.g[1];
+    const int ic = min(i, G.n[0] - 1), jc = min(j, G.n[1] - 1);
+    long long p = G.pidx(ic, jc, k0);
+    int flag = 0;
+    const T inv_dx = (T)A.inv_dx;
+
+    stage_plane<T, SCHEME>(G, Us, W, rect, x_lo_pad, y_lo_pad, k0 + G.g[2]);
+    cp_async_commit();
+
+    T fz_lo[NF];
+    ZWindow<T, SCHEME> zw;
+    T nxt[ZWindow<T, SCHEME>::NV];
+    if (WITH_Z && own) {
+#pragma unroll
+        for (int m = 0; m < M; ++m) {  // cells k0-R .. k0+R-1
+            ZWindow<T, SCHEME>::fetch(nxt, Us, W, G.fs, p + (long long)(m - R) * G.sxy);
+            zw.put(m, nxt);
+        }
+        iface_from<T, SCHEME, 2>(zw, A, fz_lo, flag);  // face k0 - 1/2
+        ZWindow<T, SCHEME>::fetch(nxt, Us, W, G.fs, p + (long long)R * G.sxy);  // cell k0 + R
+    }
+    const T dt = (T)ctl->dt, ca = (T)A.ca, cb = (T)A.cb;
+
+    for (int k = k0; k < k1; ++k, p += G.sxy) {
+        const int b = (k - k0) & 1;
+        if (k + 1 < k1) stage_plane<T, SCHEME>(G, Us, W, rect + (b ^ 1) * S::NA * S::CELLS, x_lo_pad, y_lo_pad, k + 1 + G.g[2]);
+        cp_async_commit();
+        cp_async_wait<1>();
+        __syncthreads();  // plane k is in rect[b] for everyone
+        const T* rb = rect + b * S::NA * S::CELLS;
+        T L[NF] = {0, 0, 0, 0, 0}, us_c[NF] = {0, 0, 0, 0, 0};
+        if (WITH_Z && own) {
+            T f[NF];
+            zw.shift();
+            zw.put(M - 1, nxt);
+            if (k + 1 < k1) ZWindow<T, SCHEME>::fetch(nxt, Us, W, G.fs, p + (long long)(R + 1) * G.sxy);
+            iface_from<T, SCHEME, 2>(zw, A, f, flag);
+#pragma unroll
+            for (int c = 0; c < NF; ++c) {
+                L[c] = fz_lo[c] - f[c];
+                fz_lo[c] = f[c];
+            }
+        }
+        if (ty >= 1) {  // warp-uniform: the helper row has no x work
+            T f[NF] = {0, 0, 0, 0, 0};
+            if (need_x) {
+                RectAcc<T> acc{rb + (ty + R - 1) * S::RW + lane, 1, S::CELLS};
+                iface_from<T, SCHEME, 0>(acc, A, f, flag);
+            }
+#pragma unroll
+            for (int c = 0; c < NF; ++c) {
+                const T lo = shfl_up1<T>(f[c]);
+                if (own) L[c] += lo - f[c];
+            }
+        }
+        {
+            T f[NF] = {0, 0, 0, 0, 0};
+            if (need_y) {
+                RectAcc<T> acc{rb + ty * S::RW + lane + R - 1, S::RW, S::CELLS};
+                iface_from<T, SCHEME, 1>(acc, A, f, flag);
+            }
+            T* fy = fy_s + b * FUSED_TY * NF * 32;
+#pragma unroll
+            for (int c = 0; c < NF; ++c) fy[(ty * NF + c) * 32 + lane] = f[c];
+            // own cell's stage value (centre of the rectangle), read before rect[b] may be refilled
+            if (own && A.mode != 1) {
+                const T* uc = rb + (ty + R - 1) * S::RW + lane + R - 1;
+#pragma unroll
+                for (int c = 0; c < NF; ++c) us_c[c] = uc[c * S::CELLS];
+            }
+            __syncthreads();  // y-fluxes visible; everyone is done reading rect[b]
+            if (own) {
+#pragma unroll
+                for (int c = 0; c < NF; ++c) L[c] += fy[((ty - 1) * NF + c) * 32 + lane] - f[c];
+            }
+        }
+        if (own) {
+            if (A.mode == 1) {
+#pragma unroll
+                for (int c = 0; c < NF; ++c) Uout[c * G.fs + p] = L[c] * inv_dx;
+            } else {
+#pragma unroll
+                for (int c = 0; c < NF; ++c) {
+                    T v = tfma(dt, L[c] * inv_dx, us_c[c]);
+                    if (A.ca != 0.0) v = tfma(ca, Un[c * G.fs + p], cb * v);
+                    Uout[c * G.fs + p] = v;
+                }
+            }
+        }
+    }
+    if (flag) ctl->flag = 1;
+}
+
+// z sweep: Uout += coef * (f(k-1/2) - f(k+1/2)), coef = cb dt / dx (Runge-Kutta mode) or 1 / dx (mode 1)
+template <class T, int SCHEME>
+__global__ void __launch_bounds__(128, (SCHEME == 1 && sizeof(T) == 8) ? 2 : 3)
+z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, T* Uout, Ctl* ctl) {
+    constexpr int R = ZWindow<T, SCHEME>::R, M = 2 * R, NV = ZWindow<T, SCHEME>::NV;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= G.n[0] || j >= G.n[1]) return;
+    const int k0 = (int)blockIdx.z * ZSWEEP_ZC;
+    const int k1 = min(k0 + ZSWEEP_ZC, G.n[2]);
+    long long p = G.pidx(i, j, k0);
+    int flag = 0;
+    ZWindow<T, SCHEME> zw;
+    T nxt[NV], fz_lo[NF];
+#pragma unroll
+    for (int m = 0; m < M; ++m) {
+        ZWindow<T, SCHEME>::fetch(nxt, Us, W, G.fs, p + (long long)(m - R) * G.sxy);
+        zw.put(m, nxt);
+    }
+    iface_from<T, SCHEME, 2>(zw, A, fz_lo, flag);
+    ZWindow<T, SCHEME>::fetch(nxt, Us, W, G.fs, p + (long long)R * G.sxy);
+    const T coef = A.mode == 1 ? (T)A.inv_dx : (T)(A.cb * ctl->dt * A.inv_dx);
+    for (int k = k0; k < k1; ++k, p += G.sxy) {
+        T f[NF], o[NF];
+        zw.shift();
+        zw.put(M - 1, nxt);
+        if (k + 1 < k1) ZWindow<T, SCHEME>::fetch(nxt, Us, W, G.fs, p + (long long)(R + 1) * G.sxy);
+#pragma unroll
+        for (int c = 0; c < NF; ++c) o[c] = Uout[c * G.fs + p];
+        iface_from<T, SCHEME, 2>(zw, A, f, flag);
+#pragma unroll
+        for (int c = 0; c < NF; ++c) {
+            Uout[c * G.fs + p] = tfma(coef, fz_lo[c] - f[c], o[c]);
+            fz_lo[c] = f[c];
+        }
+    }
+    if (flag) ctl->flag = 1;
+}
+
+template <class T, int SCHEME>
+int configure_tiled(FusedPlan& P) {
+    const int bytes = (int)TileShape<SCHEME>::template smem_bytes<T>();
+    cudaError_t e = cudaFuncSetAttribute(stage_tiled_kernel<T, SCHEME, false>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(stage_tiled_kernel<T, SCHEME, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) {
+        snprintf(P.err, sizeof P.err, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+        return -1;
+    }
+    return 0;
+}
+
+inline int build_fused_plan(FusedPlan& P, const Geom&, int scheme, int precision) {
+    if (precision == 0) {
+        return scheme == 0 ? configure_tiled<double, 0>(P) : scheme == 1 ? configure_tiled<double, 1>(P)
+                                                                         : configure_tiled<double, 2>(P);
+    }
+    return scheme == 0 ? configure_tiled<float, 0>(P) : scheme == 1 ? configure_tiled<float, 1>(P)
+                                                                    : configure_tiled<float, 2>(P);
+}
+
+template <class T, int SCHEME>
+int launch_fused_scheme(FusedPlan& P, const Geom& G, const StageArgs& A, const T* Us, const T* W, const T* Un, T* Uout,
+                        Ctl* ctl, cudaStream_t st, int* launches) {
+    const dim3 b(32, FUSED_TY, 1);
+    const dim3 g((G.n[0] + 30) / 31, (G.n[1] + FUSED_TY - 2) / (FUSED_TY - 1), (G.n[2] + FUSED_ZC - 1) / FUSED_ZC);
+    const size_t smem = TileShape<SCHEME>::template smem_bytes<T>();
+    if (P.split_z) {
+        stage_tiled_kernel<T, SCHEME, false><<<g, b, smem, st>>>(G, A, Us, W, Un, Uout, ctl);
+        const dim3 bz(32, 4, 1);
+        const dim3 gz((G.n[0] + 31) / 32, (G.n[1] + 3) / 4, (G.n[2] + ZSWEEP_ZC - 1) / ZSWEEP_ZC);
+        z_sweep_kernel<T, SCHEME><<<gz, bz, 0, st>>>(G, A, Us, W, Uout, ctl);
+        *launches = 2;
+    } else {
+        stage_tiled_kernel<T, SCHEME, true><<<g, b, smem, st>>>(G, A, Us, W, Un, Uout, ctl);
+        *launches = 1;
+    }
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        snprintf(P.err, sizeof P.err, "%s", cudaGetErrorString(e));
+        return -1;
+    }
+    return 0;
+}
+
+template <class T>
+int launch_fused(FusedPlan& P, const Geom& G, int scheme, const StageArgs& A, const T* Us, const T* W, const T* Un,
+                 T* Uout, Ctl* ctl, cudaStream_t st, int* launches) {
+    switch (scheme) {
+        case 0: return launch_fused_scheme<T, 0>(P, G, A, Us, W, Un, Uout, ctl, st, launches);
+        case 1: return launch_fused_scheme<T, 1>(P, G, A, Us, W, Un, Uout, ctl, st, launches);
+        default: return launch_fused_scheme<T, 2>(P, G, A, Us, W, Un, Uout, ctl, st, launches);
+    }
+}
+
+}  // namespace hydro

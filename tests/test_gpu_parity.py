@@ -337,14 +337,20 @@ def test_unphysical_state_raises_the_sticky_flag(B, oracle):
 # ------------------------------------------------------------------ kernel variants agree
 @pytest.mark.parametrize("scheme", SCHEMES)
 @pytest.mark.parametrize("prec", [0, 1])
-def test_fused_and_generic_kernels_agree(B, scheme, prec):
-    """The tiled stage kernel against the one-thread-per-cell one on a grid spanning several tiles with
-    ragged tails in every direction."""
+@pytest.mark.parametrize("split_z", [1, 0])
+def test_tiled_and_generic_kernels_agree(B, scheme, prec, split_z):
+    """The tiled stage kernels (x/y tile kernel + z sweep, or the single kernel with the z window inside)
+    against the one-thread-per-cell kernel on a grid spanning several tiles and z-chunks with ragged tails
+    in every direction."""
     w = small_workload(scheme, (150, 37, 29))
+    w.cons = np.ascontiguousarray(np.concatenate([w.cons] * 5, axis=1)[:, :141])   # nz = 141 > two z-chunks
+    w.n = (150, 37, 141)
     outs = []
-    for kern in (B.KERNEL_GENERIC, B.KERNEL_AUTO):
+    for kern in (B.KERNEL_GENERIC, B.KERNEL_FUSED):
         h = B.from_workload(w, precision=prec, kernel=kern)
+        h.set_option("split_z", split_z)
         h.step_cfl(0.2, 3)
         outs.append(h.get_state().cpu().numpy())
+        assert h.status() == 0
         h.close()
     assert reldiff(outs[1], outs[0]) <= (1e-12 if prec == 0 else 1e-4)
