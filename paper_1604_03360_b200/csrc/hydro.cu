@@ -161,6 +161,7 @@ StageArgs stage_args(const hydro_ctx* c, double ca, double cb, int mode) {
 
 bool want_fused(const hydro_ctx* c) {
     if (c->kernel == HYDRO_KERNEL_GENERIC) return false;
+    if (c->kernel == HYDRO_KERNEL_AUTO && !c->fused_ready) return false;
     return fused_supported(c->G, c->scheme, c->precision);
 }
 
@@ -365,7 +366,8 @@ int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
     LAUNCHED(c, "set_ctl_kernel");
     c->fused_ready = false;
     if (fused_supported(c->G, c->scheme, c->precision) && c->kernel != HYDRO_KERNEL_GENERIC) {
-        c->fused_ready = build_fused_plan(c->fused, c->G, c->scheme, c->precision) == 0;
+        void* Ubuf[3] = {c->U[0], c->U[1], c->U[2]};
+        c->fused_ready = build_fused_plan(c->fused, c->G, c->scheme, c->precision, Ubuf, c->W) == 0;
         if (!c->fused_ready && c->kernel == HYDRO_KERNEL_FUSED)
             return fail(c, HYDRO_ECUDA, "fused plan: %s", c->fused.err);
     }

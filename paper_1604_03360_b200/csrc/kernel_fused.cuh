@@ -6,7 +6,8 @@
 //   (lane, ty) sits on cell (i0 + lane, j0 + ty), i0 = 31 bx - 1, j0 = (TY-1) by - 1: column lane = 0 and
 //   row ty = 0 are helper positions one cell below the tile, the other 31 x (TY-1) positions own a cell.
 //   Per plane the halo'd rectangle of the tile (conserved fields, winv, p, a_x, a_y; R-1 / R cells of halo)
-//   is brought into shared memory with cp.async, double buffered one plane ahead, and a thread computes
+//   is brought into shared memory by TMA (two cp.async.bulk.tensor boxes per plane, issued by one thread and
+//   awaited on an mbarrier), double buffered one plane ahead, and a thread computes
 //   only UPPER-face fluxes from it:
 //     x: f(i+1/2) by every thread of an owning row     -> lower face from lane-1 by warp shuffle
 //     y: f(j+1/2) by every thread of an owning column  -> lower face from row ty-1 through shared memory
@@ -17,7 +18,10 @@
 //   thread per (i, j) column marching along z with the same register window, adds the z-flux difference
 //   to the output of the x/y kernel.  No shared memory, no barrier, no redundancy except one flux per chunk.
 #pragma once
+#include <cuda.h>
+
 #include <cstdio>
+#include <cstring>
 
 #include "grid.cuh"
 #include "kernel_generic.cuh"
@@ -30,6 +34,10 @@ constexpr int ZSWEEP_ZC = 128;  // planes per z-chunk of the z sweep
 
 struct FusedPlan {
     int split_z = 1;  // 1: x/y tiled kernel + z sweep kernel; 0: one kernel with the z window inside
+    // TMA descriptors of the three padded state buffers and of the primitive arrays: 4-D tensors
+    // (x, y, z, array) with box (RW, RH, 1, 5 or 4)
+    CUtensorMap mapU[3], mapW;
+    const void* baseU[3] = {nullptr, nullptr, nullptr};
     char err[256] = {0};
 };
 
@@ -39,15 +47,6 @@ inline bool fused_supported(const Geom& G, int /*scheme*/, int /*precision*/) {
 
 template <class T>
 __device__ __forceinline__ T shfl_up1(T v) { return __shfl_up_sync(0xffffffffu, v, 1); }
-
-template <int BYTES>
-__device__ __forceinline__ void cp_async(void* smem, const void* gmem) {
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(s), "l"(gmem), "n"(BYTES) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // z-stencil of one column held in registers while the block marches along z: cells k-R+1 .. k+R, per cell
 // the five conserved fields and (WENO only) winv, p, a_z.  All indices are compile-time constants after
@@ -97,55 +96,76 @@ __device__ __forceinline__ void iface_from(const Acc& acc, const StageArgs& A, T
     else llf_weno_iface<T, R, DIR>(acc, (T)A.eps, fh);
 }
 
-// stencil accessor into the shared-memory rectangle: arrays 0..4 conserved, 5 winv, 6 p, 7 a_x, 8 a_y
+// ---- TMA (cp.async.bulk.tensor) + mbarrier, raw PTX for sm_100a -------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@!p bra WAIT_LOOP;\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+// box of a 4-D tensor (x, y, z, array) -> shared memory; out-of-bounds parts of the box are zero-filled
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, int c3,
+                                            unsigned long long* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar))
+        : "memory");
+}
+
+// stencil accessor into the shared-memory rectangle of one plane: conserved arrays at ub, (winv, p, a_x, a_y)
+// at wb, array stride astride, stencil stride `stride` (1 along x, the row pitch along y)
 template <class T>
 struct RectAcc {
-    const T* base;
+    const T* ub;
+    const T* wb;
     int stride, astride;
-    __device__ __forceinline__ T u(int c, int k) const { return base[c * astride + k * stride]; }
-    __device__ __forceinline__ T w(int a, int k) const { return base[(NF + a) * astride + k * stride]; }
+    __device__ __forceinline__ T u(int c, int k) const { return ub[c * astride + k * stride]; }
+    __device__ __forceinline__ T w(int a, int k) const { return wb[a * astride + k * stride]; }
 };
 
-template <int SCHEME>
+template <class T, int SCHEME>
 struct TileShape {
     static constexpr int R = SCHEME == 0 ? 3 : (SCHEME == 1 ? 4 : 2);
-    static constexpr int RW = 32 + 2 * R - 1;         // rectangle width  (x)
-    static constexpr int RH = FUSED_TY + 2 * R - 1;   // rectangle height (y)
-    static constexpr int NA = SCHEME == 2 ? NF : NF + 4;  // arrays staged per plane
+    static constexpr int Q = 16 / (int)sizeof(T);                       // elements per 16 bytes
+    // box width (x): 32 + 2R - 1 cells plus up to Q-1 of lead-in, because TMA wants the box to start on a
+    // 16-byte boundary of the row and to be a multiple of 16 bytes wide
+    static constexpr int RW = (32 + 2 * R - 1 + (Q - 1) + Q - 1) / Q * Q;
+    static constexpr int RH = FUSED_TY + 2 * R - 1;                     // box height (y)
+    static constexpr int NWA = SCHEME == 2 ? 0 : 4;                     // winv, p, a_x, a_y
     static constexpr int CELLS = RW * RH;
-    template <class T>
-    static constexpr size_t smem_bytes() { return sizeof(T) * (2 * (size_t)NA * CELLS + 2 * FUSED_TY * NF * 32); }
-};
-
-// bring the halo'd rectangle of plane kp (padded z index) into shared memory: one warp per (array, row)
-template <class T, int SCHEME>
-__device__ __forceinline__ void stage_plane(const Geom& G, const T* __restrict__ Us, const T* __restrict__ W,
-                                            T* rect, int x_lo_pad, int y_lo_pad, int kp) {
-    using S = TileShape<SCHEME>;
-    const int lane = threadIdx.x, warp = threadIdx.y;
-    const long long plane = (long long)kp * G.sxy;
-    for (int r = warp; r < S::NA * S::RH; r += FUSED_TY) {
-        const int arr = r / S::RH, yy = r - arr * S::RH;
-        const int yp = y_lo_pad + yy;
-        if (yp >= G.np[1]) continue;
-        const T* src = (arr < NF ? Us + (long long)arr * G.fs : W + (long long)(arr - NF) * G.fs) + plane +
-                       (long long)yp * G.sx + x_lo_pad;
-        T* dst = rect + (arr * S::RH + yy) * S::RW;
-        if (x_lo_pad + lane < G.np[0]) cp_async<sizeof(T)>(dst + lane, src + lane);
-        if (lane + 32 < S::RW && x_lo_pad + lane + 32 < G.np[0]) cp_async<sizeof(T)>(dst + lane + 32, src + lane + 32);
+    static constexpr int U_ELEMS = (NF * CELLS * (int)sizeof(T) + 127) / 128 * 128 / (int)sizeof(T);
+    static constexpr int W_ELEMS = (NWA * CELLS * (int)sizeof(T) + 127) / 128 * 128 / (int)sizeof(T);
+    static constexpr int BUF_ELEMS = U_ELEMS + W_ELEMS;
+    static constexpr unsigned TX_BYTES = (unsigned)((NF + NWA) * CELLS * sizeof(T));
+    static constexpr size_t smem_bytes() {
+        return sizeof(T) * (2 * (size_t)BUF_ELEMS + 2 * FUSED_TY * NF * 32) + 2 * sizeof(unsigned long long);
     }
-}
+};
 
 template <class T, int SCHEME, bool WITH_Z>
 __global__ void __launch_bounds__(32 * FUSED_TY, (WITH_Z || (SCHEME == 1 && sizeof(T) == 8)) ? 1 : 2)
-stage_tiled_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, const T* Un, T* Uout,
-                   Ctl* ctl) {
-    using S = TileShape<SCHEME>;
+stage_tiled_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapW, Geom G,
+                   StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, const T* Un, T* Uout, Ctl* ctl) {
+    using S = TileShape<T, SCHEME>;
     constexpr int R = S::R, M = 2 * R;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* rect = reinterpret_cast<T*>(smem_raw);                   // [2][NA][RH][RW]
-    T* fy_s = rect + 2 * S::NA * S::CELLS;                      // [2][TY][NF][32]
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    T* rect = reinterpret_cast<T*>(smem_raw);                                  // [2][BUF_ELEMS]
+    T* fy_s = rect + 2 * S::BUF_ELEMS;                                         // [2][TY][NF][32]
+    unsigned long long* bars = reinterpret_cast<unsigned long long*>(fy_s + 2 * FUSED_TY * NF * 32);
     const int lane = threadIdx.x, ty = threadIdx.y;
+    const bool leader = lane == 0 && ty == 0;
     const int i0 = (int)blockIdx.x * 31 - 1, j0 = (int)blockIdx.y * (FUSED_TY - 1) - 1;
     const int i = i0 + lane, j = j0 + ty;
     const int k0 = (int)blockIdx.z * FUSED_ZC;
@@ -155,14 +175,25 @@ stage_tiled_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __res
     const bool own = row_ok && col_ok;
     const bool need_x = row_ok && i < G.n[0];  // i >= -1 always
     const bool need_y = col_ok && j < G.n[1];  // j >= -1 always
-    const int x_lo_pad = i0 - R + 1 + G.g[0], y_lo_pad = j0 - R + 1 + G.g[1];
+    const int x_first = i0 - R + 1 + G.g[0], y_lo_pad = j0 - R + 1 + G.g[1];
+    const int x_lo_pad = x_first & ~(S::Q - 1);   // 16-byte aligned start of the box
+    const int xo = x_first - x_lo_pad + lane;      // this thread's first stencil column inside the box
     const int ic = min(i, G.n[0] - 1), jc = min(j, G.n[1] - 1);
     long long p = G.pidx(ic, jc, k0);
     int flag = 0;
     const T inv_dx = (T)A.inv_dx;
 
-    stage_plane<T, SCHEME>(G, Us, W, rect, x_lo_pad, y_lo_pad, k0 + G.g[2]);
-    cp_async_commit();
+    if (leader) {
+        mbar_init(&bars[0], 1);
+        mbar_init(&bars[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (leader) {   // plane k0 -> buffer 0
+        mbar_expect_tx(&bars[0], S::TX_BYTES);
+        tma_load_4d(rect, &mapU, x_lo_pad, y_lo_pad, k0 + G.g[2], 0, &bars[0]);
+        if (S::NWA > 0) tma_load_4d(rect + S::U_ELEMS, &mapW, x_lo_pad, y_lo_pad, k0 + G.g[2], 0, &bars[0]);
+    }
 
     T fz_lo[NF];
     ZWindow<T, SCHEME> zw;
@@ -180,11 +211,14 @@ stage_tiled_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __res
 
     for (int k = k0; k < k1; ++k, p += G.sxy) {
         const int b = (k - k0) & 1;
-        if (k + 1 < k1) stage_plane<T, SCHEME>(G, Us, W, rect + (b ^ 1) * S::NA * S::CELLS, x_lo_pad, y_lo_pad, k + 1 + G.g[2]);
-        cp_async_commit();
-        cp_async_wait<1>();
-        __syncthreads();  // plane k is in rect[b] for everyone
-        const T* rb = rect + b * S::NA * S::CELLS;
+        // plane k+1 -> the other buffer; every thread finished reading it before last plane's barrier
+        if (leader && k + 1 < k1) {
+            T* dst = rect + (b ^ 1) * S::BUF_ELEMS;
+            mbar_expect_tx(&bars[b ^ 1], S::TX_BYTES);
+            tma_load_4d(dst, &mapU, x_lo_pad, y_lo_pad, k + 1 + G.g[2], 0, &bars[b ^ 1]);
+            if (S::NWA > 0) tma_load_4d(dst + S::U_ELEMS, &mapW, x_lo_pad, y_lo_pad, k + 1 + G.g[2], 0, &bars[b ^ 1]);
+        }
+        const T* rb = rect + b * S::BUF_ELEMS;
         T L[NF] = {0, 0, 0, 0, 0}, us_c[NF] = {0, 0, 0, 0, 0};
         if (WITH_Z && own) {
             T f[NF];
@@ -198,10 +232,12 @@ stage_tiled_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __res
                 fz_lo[c] = f[c];
             }
         }
+        mbar_wait(&bars[b], ((k - k0) >> 1) & 1);   // plane k has landed in rect[b]
         if (ty >= 1) {  // warp-uniform: the helper row has no x work
             T f[NF] = {0, 0, 0, 0, 0};
             if (need_x) {
-                RectAcc<T> acc{rb + (ty + R - 1) * S::RW + lane, 1, S::CELLS};
+                const int o = (ty + R - 1) * S::RW + xo;
+                RectAcc<T> acc{rb + o, rb + S::U_ELEMS + o, 1, S::CELLS};
                 iface_from<T, SCHEME, 0>(acc, A, f, flag);
             }
 #pragma unroll
@@ -213,7 +249,8 @@ stage_tiled_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __res
         {
             T f[NF] = {0, 0, 0, 0, 0};
             if (need_y) {
-                RectAcc<T> acc{rb + ty * S::RW + lane + R - 1, S::RW, S::CELLS};
+                const int o = ty * S::RW + xo + R - 1;
+                RectAcc<T> acc{rb + o, rb + S::U_ELEMS + o, S::RW, S::CELLS};
                 iface_from<T, SCHEME, 1>(acc, A, f, flag);
             }
             T* fy = fy_s + b * FUSED_TY * NF * 32;
@@ -221,7 +258,7 @@ stage_tiled_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __res
             for (int c = 0; c < NF; ++c) fy[(ty * NF + c) * 32 + lane] = f[c];
             // own cell's stage value (centre of the rectangle), read before rect[b] may be refilled
             if (own && A.mode != 1) {
-                const T* uc = rb + (ty + R - 1) * S::RW + lane + R - 1;
+                const T* uc = rb + (ty + R - 1) * S::RW + xo + R - 1;
 #pragma unroll
                 for (int c = 0; c < NF; ++c) us_c[c] = uc[c * S::CELLS];
             }
@@ -287,9 +324,24 @@ z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restric
     if (flag) ctl->flag = 1;
 }
 
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// the driver entry point is looked up through the runtime, so the library has no link-time dependency on libcuda
+inline EncodeTiledFn encode_tiled_fn() {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+        return nullptr;
+    return (EncodeTiledFn)fn;
+}
+
 template <class T, int SCHEME>
-int configure_tiled(FusedPlan& P) {
-    const int bytes = (int)TileShape<SCHEME>::template smem_bytes<T>();
+int configure_tiled(FusedPlan& P, const Geom& G, void* const U[3], void* W) {
+    using S = TileShape<T, SCHEME>;
+    const int bytes = (int)S::smem_bytes();
     cudaError_t e = cudaFuncSetAttribute(stage_tiled_kernel<T, SCHEME, false>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e == cudaSuccess)
@@ -298,32 +350,66 @@ int configure_tiled(FusedPlan& P) {
         snprintf(P.err, sizeof P.err, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
         return -1;
     }
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) {
+        snprintf(P.err, sizeof P.err, "cuTensorMapEncodeTiled not available");
+        return -1;
+    }
+    const CUtensorMapDataType dt = sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    const cuuint64_t strides[3] = {(cuuint64_t)G.sx * sizeof(T), (cuuint64_t)G.sxy * sizeof(T), (cuuint64_t)G.fs * sizeof(T)};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    for (int m = 0; m < 4; ++m) {
+        const int narr = m < 3 ? NF : S::NWA;
+        if (narr == 0) {
+            memset(&P.mapW, 0, sizeof P.mapW);
+            continue;
+        }
+        const cuuint64_t dims[4] = {(cuuint64_t)G.sx, (cuuint64_t)G.np[1], (cuuint64_t)G.np[2], (cuuint64_t)narr};
+        const cuuint32_t box[4] = {(cuuint32_t)S::RW, (cuuint32_t)S::RH, 1, (cuuint32_t)narr};
+        CUtensorMap* map = m < 3 ? &P.mapU[m] : &P.mapW;
+        void* base = m < 3 ? U[m] : W;
+        const CUresult r = enc(map, dt, 4, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) {
+            snprintf(P.err, sizeof P.err, "cuTensorMapEncodeTiled failed: %d", (int)r);
+            return -1;
+        }
+        if (m < 3) P.baseU[m] = base;
+    }
     return 0;
 }
 
-inline int build_fused_plan(FusedPlan& P, const Geom&, int scheme, int precision) {
+inline int build_fused_plan(FusedPlan& P, const Geom& G, int scheme, int precision, void* const U[3], void* W) {
     if (precision == 0) {
-        return scheme == 0 ? configure_tiled<double, 0>(P) : scheme == 1 ? configure_tiled<double, 1>(P)
-                                                                         : configure_tiled<double, 2>(P);
+        return scheme == 0 ? configure_tiled<double, 0>(P, G, U, W)
+                           : scheme == 1 ? configure_tiled<double, 1>(P, G, U, W) : configure_tiled<double, 2>(P, G, U, W);
     }
-    return scheme == 0 ? configure_tiled<float, 0>(P) : scheme == 1 ? configure_tiled<float, 1>(P)
-                                                                    : configure_tiled<float, 2>(P);
+    return scheme == 0 ? configure_tiled<float, 0>(P, G, U, W)
+                       : scheme == 1 ? configure_tiled<float, 1>(P, G, U, W) : configure_tiled<float, 2>(P, G, U, W);
 }
 
 template <class T, int SCHEME>
 int launch_fused_scheme(FusedPlan& P, const Geom& G, const StageArgs& A, const T* Us, const T* W, const T* Un, T* Uout,
                         Ctl* ctl, cudaStream_t st, int* launches) {
+    int m = -1;
+    for (int q = 0; q < 3; ++q)
+        if (P.baseU[q] == (const void*)Us) m = q;
+    if (m < 0) {
+        snprintf(P.err, sizeof P.err, "stage input is not one of the context's state buffers");
+        return -1;
+    }
     const dim3 b(32, FUSED_TY, 1);
     const dim3 g((G.n[0] + 30) / 31, (G.n[1] + FUSED_TY - 2) / (FUSED_TY - 1), (G.n[2] + FUSED_ZC - 1) / FUSED_ZC);
-    const size_t smem = TileShape<SCHEME>::template smem_bytes<T>();
+    const size_t smem = TileShape<T, SCHEME>::smem_bytes();
     if (P.split_z) {
-        stage_tiled_kernel<T, SCHEME, false><<<g, b, smem, st>>>(G, A, Us, W, Un, Uout, ctl);
+        stage_tiled_kernel<T, SCHEME, false><<<g, b, smem, st>>>(P.mapU[m], P.mapW, G, A, Us, W, Un, Uout, ctl);
         const dim3 bz(32, 4, 1);
         const dim3 gz((G.n[0] + 31) / 32, (G.n[1] + 3) / 4, (G.n[2] + ZSWEEP_ZC - 1) / ZSWEEP_ZC);
         z_sweep_kernel<T, SCHEME><<<gz, bz, 0, st>>>(G, A, Us, W, Uout, ctl);
         *launches = 2;
     } else {
-        stage_tiled_kernel<T, SCHEME, true><<<g, b, smem, st>>>(G, A, Us, W, Un, Uout, ctl);
+        stage_tiled_kernel<T, SCHEME, true><<<g, b, smem, st>>>(P.mapU[m], P.mapW, G, A, Us, W, Un, Uout, ctl);
         *launches = 1;
     }
     const cudaError_t e = cudaGetLastError();
