@@ -54,6 +54,25 @@ HD float fast_rcp(float x) {
 #endif
 }
 
+// Square root of a positive, finite, normal number.  fp64: MUFU.RSQ64H seed plus two coupled Newton steps
+// on s = sqrt(x) (5 DFMA-pipe instructions, error about 1 ulp, no special-case path).  fp32: sqrtf.
+HD double fast_sqrt(double x) {
+#ifdef __CUDA_ARCH__
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double s = x * y;
+    const double h = 0.5 * y;
+    double e = fma(-s, s, x);
+    s = fma(e, h, s);
+    e = fma(-s, s, x);
+    s = fma(e, h, s);
+    return s;
+#else
+    return sqrt(x);
+#endif
+}
+HD float fast_sqrt(float x) { return sqrtf(x); }
+
 // ------------------------------------------------------------------------------------------------
 // a2. conserved -> primitive, closed form for p = e/3 (a2; reading Q16).
 //   s = sqrt(4E^2 - 3M^2);  v_i = 3 M_i/(2E + s);  e = 3(E^2 - M^2)/(s + E);  p = e/3.
@@ -77,9 +96,12 @@ HD void con2prim(T E, T M0, T M1, T M2, T& winv, T& p, T& v2, int& flag) {
             flag = 1;
         }
     }
-    const T s = tsqrt(tfma((T)4 * E, E, (T)-3 * m2));
-    const T w = (T)3 / ((T)2 * E + s);
-    p = tfma(E, E, -m2) / (s + E);
+    // one reciprocal serves both quotients: 1/((2E+s)(s+E))
+    const T s = fast_sqrt(tfma((T)4 * E, E, (T)-3 * m2));
+    const T d1 = tfma((T)2, E, s), d2 = s + E;
+    const T r = fast_rcp(d1 * d2);
+    const T w = (T)3 * (r * d2);
+    p = tfma(E, E, -m2) * (r * d1);
     v2 = m2 * w * w;
     winv = w * sc;
 }
@@ -91,11 +113,13 @@ HD T signal_speed(T vd, T v2, T inv_den) {
     const T cs2 = (T)(1.0 / 3.0);
     const T cs = (T)0.57735026918962576451;
     const T vd2 = vd * vd;
-    const T disc = ((T)1 - v2) * ((T)1 - vd2 - (v2 - vd2) * cs2);
-    return (tabs(vd) * ((T)1 - cs2) + cs * tsqrt(disc)) * inv_den;
+    // disc >= 0 analytically; the floor keeps the reciprocal-square-root seed finite when a clamped state
+    // (reading Q16) drives it to zero
+    const T disc = tmax(((T)1 - v2) * ((T)1 - vd2 - (v2 - vd2) * cs2), (T)1e-30);
+    return (tabs(vd) * ((T)1 - cs2) + cs * fast_sqrt(disc)) * inv_den;
 }
 template <class T>
-HD T speed_inv_den(T v2) { return (T)1 / ((T)1 - v2 * (T)(1.0 / 3.0)); }
+HD T speed_inv_den(T v2) { return fast_rcp(tfma(v2, (T)(-1.0 / 3.0), (T)1)); }
 
 // ------------------------------------------------------------------------------------------------
 // a7. WENO reconstructions in numerator/denominator form.

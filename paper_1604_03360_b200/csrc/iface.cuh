@@ -127,12 +127,13 @@ HD void musta_force_iface(const Acc& acc, int K, T C, T fh[NF], int& flag) {
         QL[c] = tfma((T)0.5, minmod(dm, d0), u1);
         QR[c] = tfma((T)-0.5, minmod(d0, dp), u2);
     }
+    const T invC = (T)1 / C;
     for (int stage = 1;; ++stage) {
         T FL[NF], FR[NF], QM[NF], FM[NF], aL, aR;
         flux_and_speed<T, DIR>(QL, FL, aL, flag);
         flux_and_speed<T, DIR>(QR, FR, aR, flag);
         const T S = tmax(aL, aR);
-        const T tau = C / S, itau = S / C;
+        const T tau = C * fast_rcp(S), itau = S * invC;
 #pragma unroll
         for (int c = 0; c < NF; ++c) QM[c] = (T)0.5 * ((QL[c] + QR[c]) - tau * (FR[c] - FL[c]));
         flux_only<T, DIR>(QM, FM, flag);

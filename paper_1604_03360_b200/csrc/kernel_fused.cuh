@@ -28,15 +28,15 @@
 
 namespace hydro {
 
-constexpr int FUSED_TY = 8;     // rows per block (one of them the helper row)
 constexpr int FUSED_ZC = 64;    // planes per z-chunk of the tiled kernel
 constexpr int ZSWEEP_ZC = 128;  // planes per z-chunk of the z sweep
 
 struct FusedPlan {
     int split_z = 1;  // 1: x/y tiled kernel + z sweep kernel; 0: one kernel with the z window inside
     // TMA descriptors of the three padded state buffers and of the primitive arrays: 4-D tensors
-    // (x, y, z, array) with box (RW, RH, 1, 5 or 4)
-    CUtensorMap mapU[3], mapW;
+    // (x, y, z, array) with box (RW, RH, 1, 5 or 4); one set per kernel variant [split, with z] because the
+    // tile height differs
+    CUtensorMap mapU[2][3], mapW[2];
     const void* baseU[3] = {nullptr, nullptr, nullptr};
     char err[256] = {0};
 };
@@ -135,14 +135,19 @@ struct RectAcc {
     __device__ __forceinline__ T w(int a, int k) const { return wb[a * astride + k * stride]; }
 };
 
-template <class T, int SCHEME>
+template <class T, int SCHEME, bool WITH_Z>
 struct TileShape {
     static constexpr int R = SCHEME == 0 ? 3 : (SCHEME == 1 ? 4 : 2);
+    // rows per block (one of them the helper row).  16 rows (512 threads, one block per SM) halve the redundant
+    // y-fluxes but measured slower than two independent 256-thread blocks per SM (18.1 vs 17.2 ms per stage,
+    // WENO5 fp64 512^3): one barrier then stalls the whole SM.
+    static constexpr int TY = 8;
+    static constexpr int MIN_BLOCKS = (TY == 16 || WITH_Z || (SCHEME == 1 && sizeof(T) == 8)) ? 1 : 2;
     static constexpr int Q = 16 / (int)sizeof(T);                       // elements per 16 bytes
     // box width (x): 32 + 2R - 1 cells plus up to Q-1 of lead-in, because TMA wants the box to start on a
     // 16-byte boundary of the row and to be a multiple of 16 bytes wide
     static constexpr int RW = (32 + 2 * R - 1 + (Q - 1) + Q - 1) / Q * Q;
-    static constexpr int RH = FUSED_TY + 2 * R - 1;                     // box height (y)
+    static constexpr int RH = TY + 2 * R - 1;                     // box height (y)
     static constexpr int NWA = SCHEME == 2 ? 0 : 4;                     // winv, p, a_x, a_y
     static constexpr int CELLS = RW * RH;
     static constexpr int U_ELEMS = (NF * CELLS * (int)sizeof(T) + 127) / 128 * 128 / (int)sizeof(T);
@@ -150,16 +155,16 @@ struct TileShape {
     static constexpr int BUF_ELEMS = U_ELEMS + W_ELEMS;
     static constexpr unsigned TX_BYTES = (unsigned)((NF + NWA) * CELLS * sizeof(T));
     static constexpr size_t smem_bytes() {
-        return sizeof(T) * (2 * (size_t)BUF_ELEMS + 2 * FUSED_TY * NF * 32) + 2 * sizeof(unsigned long long);
+        return sizeof(T) * (2 * (size_t)BUF_ELEMS + 2 * TY * NF * 32) + 2 * sizeof(unsigned long long);
     }
 };
 
 template <class T, int SCHEME, bool WITH_Z>
-__global__ void __launch_bounds__(32 * FUSED_TY, (WITH_Z || (SCHEME == 1 && sizeof(T) == 8)) ? 1 : 2)
+__global__ void __launch_bounds__(32 * TileShape<T, SCHEME, WITH_Z>::TY, TileShape<T, SCHEME, WITH_Z>::MIN_BLOCKS)
 stage_tiled_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapW, Geom G,
                    StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, const T* Un, T* Uout, Ctl* ctl) {
-    using S = TileShape<T, SCHEME>;
-    constexpr int R = S::R, M = 2 * R;
+    using S = TileShape<T, SCHEME, WITH_Z>;
+    constexpr int R = S::R, M = 2 * R, FUSED_TY = S::TY;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     T* rect = reinterpret_cast<T*>(smem_raw);                                  // [2][BUF_ELEMS]
     T* fy_s = rect + 2 * S::BUF_ELEMS;                                         // [2][TY][NF][32]
@@ -285,11 +290,30 @@ stage_tiled_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_consta
     if (flag) ctl->flag = 1;
 }
 
-// z sweep: Uout += coef * (f(k-1/2) - f(k+1/2)), coef = cb dt / dx (Runge-Kutta mode) or 1 / dx (mode 1)
+// ---- cp.async (LDGSTS) helpers: per-thread asynchronous global -> shared copies ---------------------
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void* smem, const void* gmem) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(smem_u32(smem)), "l"(gmem), "n"(BYTES) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+constexpr int ZSWEEP_THREADS = 128;
+constexpr int ZSWEEP_DEPTH = 3;   // planes in flight
+
+// z sweep: Uout += coef * (f(k-1/2) - f(k+1/2)), coef = cb dt / dx (Runge-Kutta mode) or 1 / dx (mode 1).
+// Every global read of the marching loop (the new window cell k+R and the old Uout of plane k) is a
+// cp.async into the thread's own shared-memory slots, ZSWEEP_DEPTH planes ahead: no load latency is
+// exposed and no thread reads another thread's slots, so there is no barrier.
 template <class T, int SCHEME>
-__global__ void __launch_bounds__(128, (SCHEME == 1 && sizeof(T) == 8) ? 2 : 3)
+__global__ void __launch_bounds__(ZSWEEP_THREADS, (SCHEME == 1 && sizeof(T) == 8) ? 2 : 3)
 z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, T* Uout, Ctl* ctl) {
-    constexpr int R = ZWindow<T, SCHEME>::R, M = 2 * R, NV = ZWindow<T, SCHEME>::NV;
+    constexpr int R = ZWindow<T, SCHEME>::R, M = 2 * R, NV = ZWindow<T, SCHEME>::NV, NWZ = ZWindow<T, SCHEME>::NWZ;
+    constexpr int NVO = NV + NF, D = ZSWEEP_DEPTH;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* sm = reinterpret_cast<T*>(smem_raw);   // [D][NVO][ZSWEEP_THREADS]
+    const int tid = threadIdx.x + blockDim.x * threadIdx.y;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     if (i >= G.n[0] || j >= G.n[1]) return;
@@ -297,6 +321,27 @@ z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restric
     const int k1 = min(k0 + ZSWEEP_ZC, G.n[2]);
     long long p = G.pidx(i, j, k0);
     int flag = 0;
+    // stage for plane k: window cell k+R and the old output of plane k
+    auto issue = [&](int k) {
+        if (k < k1) {
+            T* dst = sm + ((k - k0) % D) * NVO * ZSWEEP_THREADS + tid;
+            const long long q = p + (long long)(k - k0) * G.sxy;   // p stays at plane k0 in this lambda's use
+            const long long qr = q + (long long)R * G.sxy;
+#pragma unroll
+            for (int c = 0; c < NF; ++c) cp_async<sizeof(T)>(dst + c * ZSWEEP_THREADS, Us + c * G.fs + qr);
+            if (NWZ > 0) {
+                cp_async<sizeof(T)>(dst + (NF + 0) * ZSWEEP_THREADS, W + W_INV * G.fs + qr);
+                cp_async<sizeof(T)>(dst + (NF + 1) * ZSWEEP_THREADS, W + W_P * G.fs + qr);
+                cp_async<sizeof(T)>(dst + (NF + 2) * ZSWEEP_THREADS, W + (W_AX + 2) * G.fs + qr);
+            }
+#pragma unroll
+            for (int c = 0; c < NF; ++c) cp_async<sizeof(T)>(dst + (NV + c) * ZSWEEP_THREADS, Uout + c * G.fs + q);
+        }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (int d = 0; d < D; ++d) issue(k0 + d);
+
     ZWindow<T, SCHEME> zw;
     T nxt[NV], fz_lo[NF];
 #pragma unroll
@@ -305,23 +350,33 @@ z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restric
         zw.put(m, nxt);
     }
     iface_from<T, SCHEME, 2>(zw, A, fz_lo, flag);
-    ZWindow<T, SCHEME>::fetch(nxt, Us, W, G.fs, p + (long long)R * G.sxy);
     const T coef = A.mode == 1 ? (T)A.inv_dx : (T)(A.cb * ctl->dt * A.inv_dx);
-    for (int k = k0; k < k1; ++k, p += G.sxy) {
+    const long long p0 = p;
+    for (int k = k0; k < k1; ++k) {
         T f[NF], o[NF];
+        cp_async_wait<D - 1>();   // the oldest stage (plane k) has landed
+        const T* src = sm + ((k - k0) % D) * NVO * ZSWEEP_THREADS + tid;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) nxt[v] = src[v * ZSWEEP_THREADS];
+#pragma unroll
+        for (int c = 0; c < NF; ++c) o[c] = src[(NV + c) * ZSWEEP_THREADS];
+        issue(k + D);             // refill the slot just read
         zw.shift();
         zw.put(M - 1, nxt);
-        if (k + 1 < k1) ZWindow<T, SCHEME>::fetch(nxt, Us, W, G.fs, p + (long long)(R + 1) * G.sxy);
-#pragma unroll
-        for (int c = 0; c < NF; ++c) o[c] = Uout[c * G.fs + p];
         iface_from<T, SCHEME, 2>(zw, A, f, flag);
+        const long long q = p0 + (long long)(k - k0) * G.sxy;
 #pragma unroll
         for (int c = 0; c < NF; ++c) {
-            Uout[c * G.fs + p] = tfma(coef, fz_lo[c] - f[c], o[c]);
+            Uout[c * G.fs + q] = tfma(coef, fz_lo[c] - f[c], o[c]);
             fz_lo[c] = f[c];
         }
     }
     if (flag) ctl->flag = 1;
+}
+
+template <class T, int SCHEME>
+constexpr size_t zsweep_smem_bytes() {
+    return sizeof(T) * (size_t)ZSWEEP_DEPTH * (ZWindow<T, SCHEME>::NV + NF) * ZSWEEP_THREADS;
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -340,12 +395,16 @@ inline EncodeTiledFn encode_tiled_fn() {
 
 template <class T, int SCHEME>
 int configure_tiled(FusedPlan& P, const Geom& G, void* const U[3], void* W) {
-    using S = TileShape<T, SCHEME>;
-    const int bytes = (int)S::smem_bytes();
+    using S = TileShape<T, SCHEME, false>;
+    using SZ = TileShape<T, SCHEME, true>;
     cudaError_t e = cudaFuncSetAttribute(stage_tiled_kernel<T, SCHEME, false>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::smem_bytes());
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(stage_tiled_kernel<T, SCHEME, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        e = cudaFuncSetAttribute(stage_tiled_kernel<T, SCHEME, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)SZ::smem_bytes());
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(z_sweep_kernel<T, SCHEME>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)zsweep_smem_bytes<T, SCHEME>());
     if (e != cudaSuccess) {
         snprintf(P.err, sizeof P.err, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
         return -1;
@@ -358,24 +417,27 @@ int configure_tiled(FusedPlan& P, const Geom& G, void* const U[3], void* W) {
     const CUtensorMapDataType dt = sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
     const cuuint64_t strides[3] = {(cuuint64_t)G.sx * sizeof(T), (cuuint64_t)G.sxy * sizeof(T), (cuuint64_t)G.fs * sizeof(T)};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
-    for (int m = 0; m < 4; ++m) {
-        const int narr = m < 3 ? NF : S::NWA;
-        if (narr == 0) {
-            memset(&P.mapW, 0, sizeof P.mapW);
-            continue;
+    for (int v = 0; v < 2; ++v) {
+        const int RW = v == 0 ? S::RW : SZ::RW, RH = v == 0 ? S::RH : SZ::RH;
+        for (int m = 0; m < 4; ++m) {
+            const int narr = m < 3 ? NF : S::NWA;
+            if (narr == 0) {
+                memset(&P.mapW[v], 0, sizeof(CUtensorMap));
+                continue;
+            }
+            const cuuint64_t dims[4] = {(cuuint64_t)G.sx, (cuuint64_t)G.np[1], (cuuint64_t)G.np[2], (cuuint64_t)narr};
+            const cuuint32_t box[4] = {(cuuint32_t)RW, (cuuint32_t)RH, 1, (cuuint32_t)narr};
+            CUtensorMap* map = m < 3 ? &P.mapU[v][m] : &P.mapW[v];
+            void* base = m < 3 ? U[m] : W;
+            const CUresult r = enc(map, dt, 4, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) {
+                snprintf(P.err, sizeof P.err, "cuTensorMapEncodeTiled failed: %d", (int)r);
+                return -1;
+            }
+            if (m < 3) P.baseU[m] = base;
         }
-        const cuuint64_t dims[4] = {(cuuint64_t)G.sx, (cuuint64_t)G.np[1], (cuuint64_t)G.np[2], (cuuint64_t)narr};
-        const cuuint32_t box[4] = {(cuuint32_t)S::RW, (cuuint32_t)S::RH, 1, (cuuint32_t)narr};
-        CUtensorMap* map = m < 3 ? &P.mapU[m] : &P.mapW;
-        void* base = m < 3 ? U[m] : W;
-        const CUresult r = enc(map, dt, 4, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) {
-            snprintf(P.err, sizeof P.err, "cuTensorMapEncodeTiled failed: %d", (int)r);
-            return -1;
-        }
-        if (m < 3) P.baseU[m] = base;
     }
     return 0;
 }
@@ -399,17 +461,20 @@ int launch_fused_scheme(FusedPlan& P, const Geom& G, const StageArgs& A, const T
         snprintf(P.err, sizeof P.err, "stage input is not one of the context's state buffers");
         return -1;
     }
-    const dim3 b(32, FUSED_TY, 1);
-    const dim3 g((G.n[0] + 30) / 31, (G.n[1] + FUSED_TY - 2) / (FUSED_TY - 1), (G.n[2] + FUSED_ZC - 1) / FUSED_ZC);
-    const size_t smem = TileShape<T, SCHEME>::smem_bytes();
     if (P.split_z) {
-        stage_tiled_kernel<T, SCHEME, false><<<g, b, smem, st>>>(P.mapU[m], P.mapW, G, A, Us, W, Un, Uout, ctl);
+        using S = TileShape<T, SCHEME, false>;
+        const dim3 b(32, S::TY, 1);
+        const dim3 g((G.n[0] + 30) / 31, (G.n[1] + S::TY - 2) / (S::TY - 1), (G.n[2] + FUSED_ZC - 1) / FUSED_ZC);
+        stage_tiled_kernel<T, SCHEME, false><<<g, b, S::smem_bytes(), st>>>(P.mapU[0][m], P.mapW[0], G, A, Us, W, Un, Uout, ctl);
         const dim3 bz(32, 4, 1);
         const dim3 gz((G.n[0] + 31) / 32, (G.n[1] + 3) / 4, (G.n[2] + ZSWEEP_ZC - 1) / ZSWEEP_ZC);
-        z_sweep_kernel<T, SCHEME><<<gz, bz, 0, st>>>(G, A, Us, W, Uout, ctl);
+        z_sweep_kernel<T, SCHEME><<<gz, bz, zsweep_smem_bytes<T, SCHEME>(), st>>>(G, A, Us, W, Uout, ctl);
         *launches = 2;
     } else {
-        stage_tiled_kernel<T, SCHEME, true><<<g, b, smem, st>>>(P.mapU[m], P.mapW, G, A, Us, W, Un, Uout, ctl);
+        using S = TileShape<T, SCHEME, true>;
+        const dim3 b(32, S::TY, 1);
+        const dim3 g((G.n[0] + 30) / 31, (G.n[1] + S::TY - 2) / (S::TY - 1), (G.n[2] + FUSED_ZC - 1) / FUSED_ZC);
+        stage_tiled_kernel<T, SCHEME, true><<<g, b, S::smem_bytes(), st>>>(P.mapU[1][m], P.mapW[1], G, A, Us, W, Un, Uout, ctl);
         *launches = 1;
     }
     const cudaError_t e = cudaGetLastError();
