@@ -80,15 +80,28 @@ HD float fast_sqrt(float x) { return sqrtf(x); }
 // |M| <= (1-1e-12) E raises flag; the caller's E and M are left alone (the physical flux keeps using
 // them), the rescaling of M goes into winv.
 template <class T>
+HD bool below_floor(T E) { return !(E >= (T)1e-300); }
+#ifdef __CUDA_ARCH__
+// fp64: positive doubles order like their bit patterns, so the floor test is an integer compare on the high
+// word (negative E fails it through the sign bit); keeps one compare off the fp64 pipe
+template <>
+__device__ __forceinline__ bool below_floor<double>(double E) {
+    return __double2hiint(E) < 0x01a56e1f;   // high word of 1e-300 = 0x01a56e1fc2f8f359
+}
+#endif
+
+template <class T>
 HD void con2prim(T E, T M0, T M1, T M2, T& winv, T& p, T& v2, int& flag) {
-    if (!(E >= (T)1e-300)) {
+    if (below_floor(E)) {
         E = (T)1e-300;
         flag = 1;
     }
     T m2 = tfma(M0, M0, tfma(M1, M1, M2 * M2));
-    const T lim = ((T)1 - (T)1e-12) * E;
+    T t = E * E;
     T sc = (T)1;
-    if (m2 > lim * lim) {
+    const T c2 = ((T)1 - (T)1e-12) * ((T)1 - (T)1e-12);
+    if (m2 > c2 * t) {   // |M| > (1 - 1e-12) E up to rounding: settle it with the square root (rare path)
+        const T lim = ((T)1 - (T)1e-12) * E;
         const T mabs = tsqrt(m2);
         if (mabs > lim) {
             sc = lim / mabs;
@@ -97,11 +110,11 @@ HD void con2prim(T E, T M0, T M1, T M2, T& winv, T& p, T& v2, int& flag) {
         }
     }
     // one reciprocal serves both quotients: 1/((2E+s)(s+E))
-    const T s = fast_sqrt(tfma((T)4 * E, E, (T)-3 * m2));
+    const T s = fast_sqrt(tfma((T)4, t, (T)-3 * m2));
     const T d1 = tfma((T)2, E, s), d2 = s + E;
     const T r = fast_rcp(d1 * d2);
     const T w = (T)3 * (r * d2);
-    p = tfma(E, E, -m2) * (r * d1);
+    p = (t - m2) * (r * d1);
     v2 = m2 * w * w;
     winv = w * sc;
 }

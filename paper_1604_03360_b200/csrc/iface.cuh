@@ -91,6 +91,21 @@ HD T minmod(T a, T b) {
     const T m = tmin(tabs(a), tabs(b));
     return a > (T)0 ? m : -m;
 }
+#ifdef __CUDA_ARCH__
+// fp64 on the device: the same function on the bit patterns, in the integer pipe (an fp64 compare or select
+// occupies the fp64 pipe, which is the one this path is bound by).  Opposite signs -> 0; otherwise the smaller
+// magnitude with the common sign (a zero operand has magnitude 0, so the result is +-0).  Differs from the
+// product test only when a*b underflows (both |a|, |b| < 1e-154), where it returns that tiny slope instead of 0.
+template <>
+__device__ __forceinline__ double minmod<double>(double a, double b) {
+    const long long ia = __double_as_longlong(a), ib = __double_as_longlong(b);
+    if ((ia ^ ib) < 0) return 0.0;
+    const unsigned long long ma = (unsigned long long)ia & 0x7fffffffffffffffull;
+    const unsigned long long mb = (unsigned long long)ib & 0x7fffffffffffffffull;
+    const unsigned long long m = ma < mb ? ma : mb;
+    return __longlong_as_double((long long)(m | ((unsigned long long)ia & 0x8000000000000000ull)));
+}
+#endif
 
 // physical flux of a conserved state along DIR plus its signal speed (every evaluation needs its own
 // con2prim, O7).  Q is modified only if the Q16 clamp fires.
@@ -117,8 +132,10 @@ HD void flux_only(const T Q[NF], T F[NF], int& flag) {
 }
 
 // acc.u(c, k), k = 0..3 for cells i-1 .. i+2.  K stages, local Courant number C (tau = C/S).
-template <class T, int DIR, class Acc>
-HD void musta_force_iface(const Acc& acc, int K, T C, T fh[NF], int& flag) {
+// KS > 0: the number of stages is the compile-time constant KS (fully unrolled, the default K = 2 takes this
+// path); KS = 0: run-time K.
+template <class T, int DIR, int KS, class Acc>
+HD void musta_force_stages(const Acc& acc, int K, T C, T fh[NF], int& flag) {
     T QL[NF], QR[NF];
 #pragma unroll
     for (int c = 0; c < NF; ++c) {
@@ -128,7 +145,9 @@ HD void musta_force_iface(const Acc& acc, int K, T C, T fh[NF], int& flag) {
         QR[c] = tfma((T)-0.5, minmod(d0, dp), u2);
     }
     const T invC = (T)1 / C;
-    for (int stage = 1;; ++stage) {
+    const int nst = KS > 0 ? KS : K;
+#pragma unroll
+    for (int stage = 1; stage <= nst; ++stage) {
         T FL[NF], FR[NF], QM[NF], FM[NF], aL, aR;
         flux_and_speed<T, DIR>(QL, FL, aL, flag);
         flux_and_speed<T, DIR>(QR, FR, aR, flag);
@@ -140,13 +159,20 @@ HD void musta_force_iface(const Acc& acc, int K, T C, T fh[NF], int& flag) {
 #pragma unroll
         for (int c = 0; c < NF; ++c)
             fh[c] = (T)0.25 * (FL[c] + (T)2 * FM[c] + FR[c] - (QR[c] - QL[c]) * itau);
-        if (stage >= K) return;
+        if (stage < nst) {
 #pragma unroll
-        for (int c = 0; c < NF; ++c) {
-            QL[c] = QL[c] - tau * (fh[c] - FL[c]);
-            QR[c] = QR[c] - tau * (FR[c] - fh[c]);
+            for (int c = 0; c < NF; ++c) {
+                QL[c] = QL[c] - tau * (fh[c] - FL[c]);
+                QR[c] = QR[c] - tau * (FR[c] - fh[c]);
+            }
         }
     }
+}
+
+template <class T, int DIR, class Acc>
+HD void musta_force_iface(const Acc& acc, int K, T C, T fh[NF], int& flag) {
+    if (K == 2) musta_force_stages<T, DIR, 2>(acc, K, C, fh, flag);
+    else musta_force_stages<T, DIR, 0>(acc, K, C, fh, flag);
 }
 
 }  // namespace hydro
