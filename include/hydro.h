@@ -85,7 +85,7 @@ int hydro_set_option(hydro_ctx *ctx, const char *key, double value);
 int hydro_set_stream(hydro_ctx *ctx, void *cuda_stream);
 
 /* Bytes of device memory the context needs for its padded state copies (three: u^n and two RK stage
- * buffers), the per-cell primitive arrays and a small control block. */
+ * buffers), two copies of the per-cell primitive arrays and a small control block. */
 size_t hydro_workspace_bytes(const hydro_ctx *ctx);
 
 /* Hand the context its device memory (256-byte aligned, at least hydro_workspace_bytes()).  The caller

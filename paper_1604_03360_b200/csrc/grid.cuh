@@ -32,6 +32,7 @@ struct Ctl {
     unsigned long long maxspeed_bits;
     int flag;
     int pad;
+    unsigned long long maxspeed_next_bits;  // max speed of the state the running step is producing (stage-3 epilogue)
 };
 
 struct HubbleParams {  // closed-form ghost fill (readings Q13, Q14)

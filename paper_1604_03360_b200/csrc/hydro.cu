@@ -36,7 +36,10 @@ struct hydro_ctx {
     size_t ws_bytes = 0;
     Ctl* ctl = nullptr;
     char* U[3] = {nullptr, nullptr, nullptr};  // u^n and two stage buffers (padded, 5 fields each)
-    char* W = nullptr;                          // primitives (padded, 5 arrays)
+    char* Wb[2] = {nullptr, nullptr};           // primitives (padded, 5 arrays), two buffers: the z sweep's epilogue
+                                                // writes the next stage's while this stage's are still read
+    int wcur = 0;                               // buffer holding the primitives of the stage input
+    bool w_ready = false;                       // interior of Wb[wcur] already holds the primitives of u^n
     FusedPlan fused;                            // tensor maps etc. for the fused kernel
     bool fused_ready = false;
     long long launches = 0;
@@ -100,6 +103,7 @@ __global__ void set_ctl_kernel(Ctl* ctl, double t, int reset_flag) {
     if (reset_flag) {
         ctl->flag = 0;
         ctl->maxspeed_bits = 0ull;
+        ctl->maxspeed_next_bits = 0ull;
         ctl->dt = 0.0;
     }
 }
@@ -111,7 +115,7 @@ int need_ws(hydro_ctx* c) {
 }
 
 template <class T>
-int do_halo(hydro_ctx* c, T* pad, double tfrac, bool use_abs, double t_abs) {
+int do_halo(hydro_ctx* c, T* pad, double tfrac, bool use_abs, double t_abs, T* Wghost = nullptr) {
     HaloArgs A;
     long long total = 0;
     for (int a = 0; a < 3; ++a) {
@@ -125,7 +129,7 @@ int do_halo(hydro_ctx* c, T* pad, double tfrac, bool use_abs, double t_abs) {
     if (total == 0) return HYDRO_OK;
     const int tb = 256;
     halo_fill_kernel<T><<<(unsigned)((total + tb - 1) / tb), tb, 0, c->stream>>>(c->G, A, c->ctl, tfrac, t_abs,
-                                                                                   use_abs ? 1 : 0, pad);
+                                                                                   use_abs ? 1 : 0, pad, Wghost);
     LAUNCHED(c, "halo_fill_kernel");
     return HYDRO_OK;
 }
@@ -133,7 +137,7 @@ int do_halo(hydro_ctx* c, T* pad, double tfrac, bool use_abs, double t_abs) {
 template <class T>
 int do_prim(hydro_ctx* c, const T* pad, int do_max) {
     const dim3 b = blk2d(64, 4);
-    prim_kernel<T><<<grd(c->G.np[0], c->G.np[1], c->G.np[2], b), b, 0, c->stream>>>(c->G, pad, (T*)c->W, c->ctl,
+    prim_kernel<T><<<grd(c->G.np[0], c->G.np[1], c->G.np[2], b), b, 0, c->stream>>>(c->G, pad, (T*)c->Wb[c->wcur], c->ctl,
                                                                                       do_max);
     LAUNCHED(c, "prim_kernel");
     return HYDRO_OK;
@@ -156,6 +160,7 @@ StageArgs stage_args(const hydro_ctx* c, double ca, double cb, int mode) {
     A.eps = c->eps;
     A.musta_K = c->musta_stages;
     A.musta_C = c->musta_cfl;
+    A.epi_max = 0;
     return A;
 }
 
@@ -182,13 +187,16 @@ struct StageTimer {
 };
 
 template <class T>
-int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double cb, int mode) {
-    const StageArgs A = stage_args(c, ca, cb, mode);
+int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double cb, int mode, T* Wnext = nullptr,
+             int epi_max = 0) {
+    StageArgs A = stage_args(c, ca, cb, mode);
+    A.epi_max = epi_max;
     StageTimer timer(c);
     if (want_fused(c)) {
         if (!c->fused_ready) return fail(c, HYDRO_ECUDA, "fused plan not built: %s", c->fused.err);
         int nl = 0;
-        const int rc = launch_fused<T>(c->fused, c->G, c->scheme, A, Us, (const T*)c->W, Un, Uout, c->ctl, c->stream, &nl);
+        const int rc = launch_fused<T>(c->fused, c->G, c->scheme, A, Us, (const T*)c->Wb[c->wcur], Un, Uout, Wnext,
+                                       c->ctl, c->stream, &nl);
         if (rc != 0) return fail(c, HYDRO_ECUDA, "fused launch: %s", c->fused.err);
         c->launches += nl;
         return HYDRO_OK;
@@ -197,7 +205,7 @@ int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double 
         return fail(c, HYDRO_EINVAL, "kernel=fused requested but the grid/scheme does not allow it");
     const dim3 b = blk2d(32, 4);
     const dim3 g = grd(c->G.n[0], c->G.n[1], c->G.n[2], b);
-    const T* W = (const T*)c->W;
+    const T* W = (const T*)c->Wb[c->wcur];
     switch (c->scheme) {
         case HYDRO_WENO5: stage_generic_kernel<T, 0><<<g, b, 0, c->stream>>>(c->G, A, Us, W, Un, Uout, c->ctl); break;
         case HYDRO_WENO7: stage_generic_kernel<T, 1><<<g, b, 0, c->stream>>>(c->G, A, Us, W, Un, Uout, c->ctl); break;
@@ -209,32 +217,38 @@ int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double 
 
 // One SSP-RK3 step (a9, O8):  u1 = u + dt L(u);  u2 = 3/4 u + 1/4 (u1 + dt L(u1));
 // u' = 1/3 u + 2/3 (u2 + dt L(u2)), ghosts at t, t+dt, t+dt/2.  dt_fixed > 0, or CFL mode.
+// WENO with the split tiled kernels: the z sweep of every stage leaves the primitives of its output in the
+// other W buffer (and stage 3 the max signal speed), so con2prim runs as a separate pass only for the first
+// step after hydro_set_state / hydro_eval_L; the ghost cells' primitives come from the halo kernel.
 template <class T>
 int do_step(hydro_ctx* c, double dt_fixed, double cfl) {
-    T* U0 = (T*)c->U[0];
-    T* U1 = (T*)c->U[1];
-    T* U2 = (T*)c->U[2];
+    T* U[3] = {(T*)c->U[0], (T*)c->U[1], (T*)c->U[2]};
     const bool weno = c->scheme != HYDRO_MUSTA_FORCE;
     const bool cflmode = !(dt_fixed > 0.0);
+    const bool epi = weno && want_fused(c) && c->fused.split_z;
+    const double tfrac[3] = {0.0, 1.0, 0.5};
+    const double ca[3] = {0.0, 0.75, 1.0 / 3.0}, cb[3] = {1.0, 0.25, 2.0 / 3.0};
+    T* const in[3] = {U[0], U[1], U[2]};
+    T* const out[3] = {U[1], U[2], U[0]};   // stage 3 writes u^n in place: each cell reads only its own u^n
     int rc;
-    // stage 1
-    if ((rc = do_halo<T>(c, U0, 0.0, false, 0.0))) return rc;
-    if (weno) {
-        if ((rc = do_prim<T>(c, U0, cflmode ? 1 : 0))) return rc;
-    } else if (cflmode) {
-        if ((rc = do_max_speed<T>(c, U0))) return rc;
+    bool have_w = c->w_ready;
+    for (int s = 0; s < 3; ++s) {
+        if ((rc = do_halo<T>(c, in[s], tfrac[s], false, 0.0, (weno && have_w) ? (T*)c->Wb[c->wcur] : nullptr))) return rc;
+        if (weno && !have_w) {
+            if ((rc = do_prim<T>(c, in[s], (s == 0 && cflmode) ? 1 : 0))) return rc;
+        } else if (!weno && s == 0 && cflmode) {
+            if ((rc = do_max_speed<T>(c, in[s]))) return rc;
+        }
+        if (s == 0) {
+            begin_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl, dt_fixed, cfl, c->dx);
+            LAUNCHED(c, "begin_step_kernel");
+        }
+        T* Wnext = epi ? (T*)c->Wb[c->wcur ^ 1] : nullptr;
+        if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, Wnext, s == 2 ? 1 : 0))) return rc;
+        if (epi) c->wcur ^= 1;
+        have_w = epi;
     }
-    begin_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl, dt_fixed, cfl, c->dx);
-    LAUNCHED(c, "begin_step_kernel");
-    if ((rc = do_stage<T>(c, U0, U0, U1, 0.0, 1.0, 0))) return rc;
-    // stage 2
-    if ((rc = do_halo<T>(c, U1, 1.0, false, 0.0))) return rc;
-    if (weno && (rc = do_prim<T>(c, U1, 0))) return rc;
-    if ((rc = do_stage<T>(c, U1, U0, U2, 0.75, 0.25, 0))) return rc;
-    // stage 3 (writes u^n in place: each cell reads only its own u^n)
-    if ((rc = do_halo<T>(c, U2, 0.5, false, 0.0))) return rc;
-    if (weno && (rc = do_prim<T>(c, U2, 0))) return rc;
-    if ((rc = do_stage<T>(c, U2, U0, U0, 1.0 / 3.0, 2.0 / 3.0, 0))) return rc;
+    c->w_ready = have_w;
     end_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
     LAUNCHED(c, "end_step_kernel");
     return HYDRO_OK;
@@ -247,6 +261,7 @@ int eval_L_impl(hydro_ctx* c, const void* cons, double t_stage, void* L_out) {
     const dim3 b = blk2d(64, 4);
     const dim3 g = grd(c->G.n[0], c->G.n[1], c->G.n[2], b);
     int rc;
+    c->w_ready = false;   // the primitive buffer is used as scratch
     pack_kernel<T><<<g, b, 0, c->stream>>>(c->G, (const T*)cons, U1);
     LAUNCHED(c, "pack_kernel");
     if ((rc = do_halo<T>(c, U1, 0.0, true, t_stage))) return rc;
@@ -346,7 +361,7 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
 
 size_t hydro_workspace_bytes(const hydro_ctx* c) {
     if (!c) return 0;
-    return 256 + 4 * state_bytes(c);  // control block, U0, U1, U2, W
+    return 256 + 5 * state_bytes(c);  // control block, U0, U1, U2, W (two buffers)
 }
 
 int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
@@ -360,14 +375,18 @@ int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
     c->ctl = (Ctl*)base;
     const size_t sb = state_bytes(c);
     for (int i = 0; i < 3; ++i) c->U[i] = base + 256 + i * sb;
-    c->W = base + 256 + 3 * sb;
+    c->Wb[0] = base + 256 + 3 * sb;
+    c->Wb[1] = base + 256 + 4 * sb;
+    c->wcur = 0;
+    c->w_ready = false;
     CUDA_OK(c, cudaMemsetAsync(p, 0, hydro_workspace_bytes(c), c->stream));
     set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, c->t_host, 1);
     LAUNCHED(c, "set_ctl_kernel");
     c->fused_ready = false;
     if (fused_supported(c->G, c->scheme, c->precision) && c->kernel != HYDRO_KERNEL_GENERIC) {
         void* Ubuf[3] = {c->U[0], c->U[1], c->U[2]};
-        c->fused_ready = build_fused_plan(c->fused, c->G, c->scheme, c->precision, Ubuf, c->W) == 0;
+        void* Wbuf[2] = {c->Wb[0], c->Wb[1]};
+        c->fused_ready = build_fused_plan(c->fused, c->G, c->scheme, c->precision, Ubuf, Wbuf) == 0;
         if (!c->fused_ready && c->kernel == HYDRO_KERNEL_FUSED)
             return fail(c, HYDRO_ECUDA, "fused plan: %s", c->fused.err);
     }
@@ -383,6 +402,7 @@ int hydro_set_state(hydro_ctx* c, const void* cons) {
     if (c->precision == HYDRO_F64) pack_kernel<double><<<g, b, 0, c->stream>>>(c->G, (const double*)cons, (double*)c->U[0]);
     else pack_kernel<float><<<g, b, 0, c->stream>>>(c->G, (const float*)cons, (float*)c->U[0]);
     LAUNCHED(c, "pack_kernel");
+    c->w_ready = false;
     set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, c->t_host, 1);
     LAUNCHED(c, "set_ctl_kernel");
     return HYDRO_OK;
@@ -458,8 +478,7 @@ int hydro_max_signal_speed(hydro_ctx* c, double* out_host) {
     CUDA_OK(c, cudaMemcpyAsync(&h, c->ctl, sizeof h, cudaMemcpyDeviceToHost, c->stream));
     CUDA_OK(c, cudaStreamSynchronize(c->stream));
     memcpy(out_host, &h.maxspeed_bits, sizeof(double));
-    reset_max_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
-    LAUNCHED(c, "reset_max_kernel");
+    // the value stays in the control block: it is the max speed of u^n, which is what the next CFL step needs
     return HYDRO_OK;
 }
 

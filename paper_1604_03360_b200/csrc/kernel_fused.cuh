@@ -25,6 +25,7 @@
 
 #include "grid.cuh"
 #include "kernel_generic.cuh"
+#include "kernels_aux.cuh"
 
 namespace hydro {
 
@@ -36,8 +37,9 @@ struct FusedPlan {
     // TMA descriptors of the three padded state buffers and of the primitive arrays: 4-D tensors
     // (x, y, z, array) with box (RW, RH, 1, 5 or 4); one set per kernel variant [split, with z] because the
     // tile height differs
-    CUtensorMap mapU[2][3], mapW[2];
+    CUtensorMap mapU[2][3], mapW[2][2];
     const void* baseU[3] = {nullptr, nullptr, nullptr};
+    const void* baseW[2] = {nullptr, nullptr};
     char err[256] = {0};
 };
 
@@ -306,9 +308,13 @@ constexpr int ZSWEEP_DEPTH = 3;   // planes in flight
 // Every global read of the marching loop (the new window cell k+R and the old Uout of plane k) is a
 // cp.async into the thread's own shared-memory slots, ZSWEEP_DEPTH planes ahead: no load latency is
 // exposed and no thread reads another thread's slots, so there is no barrier.
-template <class T, int SCHEME>
+// EPI (WENO schemes, Runge-Kutta mode): the thread holds the finished stage value of its cell, so it also makes
+// the next stage's primitives W' = (winv, p, a_x, a_y, a_z) of that cell (a2-a3; written to the OTHER W buffer,
+// this stage's W is still being read by neighbouring chunks) and, in stage 3, the max signal speed of the new
+// state (a4): the separate con2prim pass over the grid disappears from the step.
+template <class T, int SCHEME, bool EPI>
 __global__ void __launch_bounds__(ZSWEEP_THREADS, (SCHEME == 1 && sizeof(T) == 8) ? 2 : 3)
-z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, T* Uout, Ctl* ctl) {
+z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, T* Uout, T* Wnext, Ctl* ctl) {
     constexpr int R = ZWindow<T, SCHEME>::R, M = 2 * R, NV = ZWindow<T, SCHEME>::NV, NWZ = ZWindow<T, SCHEME>::NWZ;
     constexpr int NVO = NV + NF, D = ZSWEEP_DEPTH;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -352,6 +358,7 @@ z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restric
     iface_from<T, SCHEME, 2>(zw, A, fz_lo, flag);
     const T coef = A.mode == 1 ? (T)A.inv_dx : (T)(A.cb * ctl->dt * A.inv_dx);
     const long long p0 = p;
+    double amax = 0.0;
     for (int k = k0; k < k1; ++k) {
         T f[NF], o[NF];
         cp_async_wait<D - 1>();   // the oldest stage (plane k) has landed
@@ -367,9 +374,27 @@ z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restric
         const long long q = p0 + (long long)(k - k0) * G.sxy;
 #pragma unroll
         for (int c = 0; c < NF; ++c) {
-            Uout[c * G.fs + q] = tfma(coef, fz_lo[c] - f[c], o[c]);
+            o[c] = tfma(coef, fz_lo[c] - f[c], o[c]);
+            Uout[c * G.fs + q] = o[c];
             fz_lo[c] = f[c];
         }
+        if (EPI) {
+            T w[NW];
+            prim_of_cell(o, w, flag);
+#pragma unroll
+            for (int a = 0; a < NW; ++a) Wnext[a * G.fs + q] = w[a];
+            if (A.epi_max) amax = fmax(amax, fmax((double)w[W_AX], fmax((double)w[W_AX + 1], (double)w[W_AX + 2])));
+        }
+    }
+    if (EPI && A.epi_max) {   // all three axes are active whenever this kernel runs
+        const unsigned mask = __activemask();
+#pragma unroll
+        for (int o2 = 16; o2 > 0; o2 >>= 1) {
+            const double other = __shfl_xor_sync(mask, amax, o2);
+            if ((mask >> ((threadIdx.x & 31) ^ o2)) & 1u) amax = fmax(amax, other);   // partner lane exists
+        }
+        if ((threadIdx.x & 31) == 0 && amax > 0.0)
+            atomicMax(&ctl->maxspeed_next_bits, (unsigned long long)__double_as_longlong(amax));
     }
     if (flag) ctl->flag = 1;
 }
@@ -394,7 +419,7 @@ inline EncodeTiledFn encode_tiled_fn() {
 }
 
 template <class T, int SCHEME>
-int configure_tiled(FusedPlan& P, const Geom& G, void* const U[3], void* W) {
+int configure_tiled(FusedPlan& P, const Geom& G, void* const U[3], void* const W[2]) {
     using S = TileShape<T, SCHEME, false>;
     using SZ = TileShape<T, SCHEME, true>;
     cudaError_t e = cudaFuncSetAttribute(stage_tiled_kernel<T, SCHEME, false>,
@@ -403,7 +428,10 @@ int configure_tiled(FusedPlan& P, const Geom& G, void* const U[3], void* W) {
         e = cudaFuncSetAttribute(stage_tiled_kernel<T, SCHEME, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)SZ::smem_bytes());
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(z_sweep_kernel<T, SCHEME>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        e = cudaFuncSetAttribute(z_sweep_kernel<T, SCHEME, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)zsweep_smem_bytes<T, SCHEME>());
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(z_sweep_kernel<T, SCHEME, (SCHEME != 2)>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)zsweep_smem_bytes<T, SCHEME>());
     if (e != cudaSuccess) {
         snprintf(P.err, sizeof P.err, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
@@ -419,16 +447,16 @@ int configure_tiled(FusedPlan& P, const Geom& G, void* const U[3], void* W) {
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     for (int v = 0; v < 2; ++v) {
         const int RW = v == 0 ? S::RW : SZ::RW, RH = v == 0 ? S::RH : SZ::RH;
-        for (int m = 0; m < 4; ++m) {
+        for (int m = 0; m < 5; ++m) {   // three state buffers, two primitive buffers
             const int narr = m < 3 ? NF : S::NWA;
             if (narr == 0) {
-                memset(&P.mapW[v], 0, sizeof(CUtensorMap));
+                memset(&P.mapW[v][m - 3], 0, sizeof(CUtensorMap));
                 continue;
             }
             const cuuint64_t dims[4] = {(cuuint64_t)G.sx, (cuuint64_t)G.np[1], (cuuint64_t)G.np[2], (cuuint64_t)narr};
             const cuuint32_t box[4] = {(cuuint32_t)RW, (cuuint32_t)RH, 1, (cuuint32_t)narr};
-            CUtensorMap* map = m < 3 ? &P.mapU[v][m] : &P.mapW[v];
-            void* base = m < 3 ? U[m] : W;
+            CUtensorMap* map = m < 3 ? &P.mapU[v][m] : &P.mapW[v][m - 3];
+            void* base = m < 3 ? U[m] : W[m - 3];
             const CUresult r = enc(map, dt, 4, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -437,12 +465,13 @@ int configure_tiled(FusedPlan& P, const Geom& G, void* const U[3], void* W) {
                 return -1;
             }
             if (m < 3) P.baseU[m] = base;
+            else P.baseW[m - 3] = base;
         }
     }
     return 0;
 }
 
-inline int build_fused_plan(FusedPlan& P, const Geom& G, int scheme, int precision, void* const U[3], void* W) {
+inline int build_fused_plan(FusedPlan& P, const Geom& G, int scheme, int precision, void* const U[3], void* const W[2]) {
     if (precision == 0) {
         return scheme == 0 ? configure_tiled<double, 0>(P, G, U, W)
                            : scheme == 1 ? configure_tiled<double, 1>(P, G, U, W) : configure_tiled<double, 2>(P, G, U, W);
@@ -453,10 +482,11 @@ inline int build_fused_plan(FusedPlan& P, const Geom& G, int scheme, int precisi
 
 template <class T, int SCHEME>
 int launch_fused_scheme(FusedPlan& P, const Geom& G, const StageArgs& A, const T* Us, const T* W, const T* Un, T* Uout,
-                        Ctl* ctl, cudaStream_t st, int* launches) {
+                        T* Wnext, Ctl* ctl, cudaStream_t st, int* launches) {
     int m = -1;
     for (int q = 0; q < 3; ++q)
         if (P.baseU[q] == (const void*)Us) m = q;
+    const int mw = P.baseW[1] == (const void*)W ? 1 : 0;
     if (m < 0) {
         snprintf(P.err, sizeof P.err, "stage input is not one of the context's state buffers");
         return -1;
@@ -465,16 +495,19 @@ int launch_fused_scheme(FusedPlan& P, const Geom& G, const StageArgs& A, const T
         using S = TileShape<T, SCHEME, false>;
         const dim3 b(32, S::TY, 1);
         const dim3 g((G.n[0] + 30) / 31, (G.n[1] + S::TY - 2) / (S::TY - 1), (G.n[2] + FUSED_ZC - 1) / FUSED_ZC);
-        stage_tiled_kernel<T, SCHEME, false><<<g, b, S::smem_bytes(), st>>>(P.mapU[0][m], P.mapW[0], G, A, Us, W, Un, Uout, ctl);
+        stage_tiled_kernel<T, SCHEME, false><<<g, b, S::smem_bytes(), st>>>(P.mapU[0][m], P.mapW[0][mw], G, A, Us, W, Un, Uout, ctl);
         const dim3 bz(32, 4, 1);
         const dim3 gz((G.n[0] + 31) / 32, (G.n[1] + 3) / 4, (G.n[2] + ZSWEEP_ZC - 1) / ZSWEEP_ZC);
-        z_sweep_kernel<T, SCHEME><<<gz, bz, zsweep_smem_bytes<T, SCHEME>(), st>>>(G, A, Us, W, Uout, ctl);
+        if (SCHEME != 2 && Wnext != nullptr)
+            z_sweep_kernel<T, SCHEME, (SCHEME != 2)><<<gz, bz, zsweep_smem_bytes<T, SCHEME>(), st>>>(G, A, Us, W, Uout, Wnext, ctl);
+        else
+            z_sweep_kernel<T, SCHEME, false><<<gz, bz, zsweep_smem_bytes<T, SCHEME>(), st>>>(G, A, Us, W, Uout, nullptr, ctl);
         *launches = 2;
     } else {
         using S = TileShape<T, SCHEME, true>;
         const dim3 b(32, S::TY, 1);
         const dim3 g((G.n[0] + 30) / 31, (G.n[1] + S::TY - 2) / (S::TY - 1), (G.n[2] + FUSED_ZC - 1) / FUSED_ZC);
-        stage_tiled_kernel<T, SCHEME, true><<<g, b, S::smem_bytes(), st>>>(P.mapU[1][m], P.mapW[1], G, A, Us, W, Un, Uout, ctl);
+        stage_tiled_kernel<T, SCHEME, true><<<g, b, S::smem_bytes(), st>>>(P.mapU[1][m], P.mapW[1][mw], G, A, Us, W, Un, Uout, ctl);
         *launches = 1;
     }
     const cudaError_t e = cudaGetLastError();
@@ -487,11 +520,11 @@ int launch_fused_scheme(FusedPlan& P, const Geom& G, const StageArgs& A, const T
 
 template <class T>
 int launch_fused(FusedPlan& P, const Geom& G, int scheme, const StageArgs& A, const T* Us, const T* W, const T* Un,
-                 T* Uout, Ctl* ctl, cudaStream_t st, int* launches) {
+                 T* Uout, T* Wnext, Ctl* ctl, cudaStream_t st, int* launches) {
     switch (scheme) {
-        case 0: return launch_fused_scheme<T, 0>(P, G, A, Us, W, Un, Uout, ctl, st, launches);
-        case 1: return launch_fused_scheme<T, 1>(P, G, A, Us, W, Un, Uout, ctl, st, launches);
-        default: return launch_fused_scheme<T, 2>(P, G, A, Us, W, Un, Uout, ctl, st, launches);
+        case 0: return launch_fused_scheme<T, 0>(P, G, A, Us, W, Un, Uout, Wnext, ctl, st, launches);
+        case 1: return launch_fused_scheme<T, 1>(P, G, A, Us, W, Un, Uout, Wnext, ctl, st, launches);
+        default: return launch_fused_scheme<T, 2>(P, G, A, Us, W, Un, Uout, Wnext, ctl, st, launches);
     }
 }
 

@@ -25,6 +25,7 @@ struct StageArgs {
     double eps;         // WENO epsilon (Q5)
     int musta_K;        // Q8
     double musta_C;     // Q7
+    int epi_max;        // z-sweep epilogue: also reduce the max signal speed of the new state (stage 3)
 };
 
 // flux at interface (cell p) + 1/2 along DIR; p = padded index of the cell on the low side

@@ -25,9 +25,22 @@ __global__ void begin_step_kernel(Ctl* ctl, double dt_fixed, double cfl, double 
 }
 __global__ void end_step_kernel(Ctl* ctl) {
     ctl->t += ctl->dt;
-    ctl->maxspeed_bits = 0ull;
+    // the stage-3 epilogue of the z sweep (when it ran) left the max signal speed of the new state here
+    ctl->maxspeed_bits = ctl->maxspeed_next_bits;
+    ctl->maxspeed_next_bits = 0ull;
 }
 __global__ void reset_max_kernel(Ctl* ctl) { ctl->maxspeed_bits = 0ull; }
+
+// W = (winv, p, a_x, a_y, a_z) of one cell from its conserved values (a2-a3); returns the three speeds too
+template <class T>
+__device__ __forceinline__ void prim_of_cell(const T u[NF], T w[NW], int& flag) {
+    T v2;
+    con2prim(u[0], u[1], u[2], u[3], w[W_INV], w[W_P], v2, flag);
+    const T id = speed_inv_den(v2);
+    w[W_AX + 0] = signal_speed(u[1] * w[W_INV], v2, id);
+    w[W_AX + 1] = signal_speed(u[2] * w[W_INV], v2, id);
+    w[W_AX + 2] = signal_speed(u[3] * w[W_INV], v2, id);
+}
 
 // ------------------------------------------------------------------------------------------------
 // pack: interior [5][nz][ny][nx] -> padded;  unpack: the reverse.  One thread per interior cell.
@@ -93,8 +106,8 @@ struct HaloArgs {
 };
 
 template <class T>
-__global__ void halo_fill_kernel(Geom G, HaloArgs A, const Ctl* __restrict__ ctl, double tfrac, double t_abs,
-                                 int use_abs, T* __restrict__ pad) {
+__global__ void halo_fill_kernel(Geom G, HaloArgs A, Ctl* ctl, double tfrac, double t_abs,
+                                 int use_abs, T* __restrict__ pad, T* __restrict__ Wghost) {
     long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     int a = 0;
     for (; a < 3; ++a) {
@@ -134,6 +147,15 @@ __global__ void halo_fill_kernel(Geom G, HaloArgs A, const Ctl* __restrict__ ctl
     const long long p = G.pidx(ix[0], ix[1], ix[2]);
 #pragma unroll
     for (int c = 0; c < NF; ++c) pad[c * G.fs + p] = val[c];
+    // when the interior primitives came from the previous stage's z-sweep epilogue, the ghost cells' are made here
+    if (Wghost != nullptr) {
+        T w[NW];
+        int flag = 0;
+        prim_of_cell(val, w, flag);
+#pragma unroll
+        for (int a = 0; a < NW; ++a) Wghost[a * G.fs + p] = w[a];
+        if (flag) ctl->flag = 1;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
