@@ -325,6 +325,9 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
         c->kernel = p;
     } else if (k == "split_z") {
         c->fused.split_z = v != 0.0;
+    } else if (k == "tile_zc" || k == "sweep_zc") {
+        if (v < 1) return fail(c, HYDRO_EINVAL, "%s < 1", key);
+        (k == "tile_zc" ? c->fused.tile_zc : c->fused.sweep_zc) = (int)v;
     } else if (k == "profile") {
         c->profile = v != 0.0;
     } else if (k == "bc_x" || k == "bc_y" || k == "bc_z") {

@@ -29,11 +29,12 @@
 
 namespace hydro {
 
-constexpr int FUSED_ZC = 64;    // planes per z-chunk of the tiled kernel
-constexpr int ZSWEEP_ZC = 128;  // planes per z-chunk of the z sweep
+constexpr int FUSED_ZC = 64;    // default planes per z-chunk of the tiled kernel ("tile_zc" option)
+constexpr int ZSWEEP_ZC = 128;  // default planes per z-chunk of the z sweep ("sweep_zc" option)
 
 struct FusedPlan {
     int split_z = 1;  // 1: x/y tiled kernel + z sweep kernel; 0: one kernel with the z window inside
+    int tile_zc = FUSED_ZC, sweep_zc = ZSWEEP_ZC;
     // TMA descriptors of the three padded state buffers and of the primitive arrays: 4-D tensors
     // (x, y, z, array) with box (RW, RH, 1, 5 or 4); one set per kernel variant [split, with z] because the
     // tile height differs
@@ -164,7 +165,8 @@ struct TileShape {
 template <class T, int SCHEME, bool WITH_Z>
 __global__ void __launch_bounds__(32 * TileShape<T, SCHEME, WITH_Z>::TY, TileShape<T, SCHEME, WITH_Z>::MIN_BLOCKS)
 stage_tiled_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapW, Geom G,
-                   StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, const T* Un, T* Uout, Ctl* ctl) {
+                   StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, const T* Un, T* Uout, Ctl* ctl,
+                   int zc) {
     using S = TileShape<T, SCHEME, WITH_Z>;
     constexpr int R = S::R, M = 2 * R, FUSED_TY = S::TY;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -175,8 +177,8 @@ stage_tiled_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_consta
     const bool leader = lane == 0 && ty == 0;
     const int i0 = (int)blockIdx.x * 31 - 1, j0 = (int)blockIdx.y * (FUSED_TY - 1) - 1;
     const int i = i0 + lane, j = j0 + ty;
-    const int k0 = (int)blockIdx.z * FUSED_ZC;
-    const int k1 = min(k0 + FUSED_ZC, G.n[2]);
+    const int k0 = (int)blockIdx.z * zc;
+    const int k1 = min(k0 + zc, G.n[2]);
     const bool row_ok = ty >= 1 && j < G.n[1];
     const bool col_ok = lane >= 1 && i < G.n[0];
     const bool own = row_ok && col_ok;
@@ -314,7 +316,8 @@ constexpr int ZSWEEP_DEPTH = 3;   // planes in flight
 // state (a4): the separate con2prim pass over the grid disappears from the step.
 template <class T, int SCHEME, bool EPI>
 __global__ void __launch_bounds__(ZSWEEP_THREADS, (SCHEME == 1 && sizeof(T) == 8) ? 2 : 3)
-z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, T* Uout, T* Wnext, Ctl* ctl) {
+z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, T* Uout, T* Wnext, Ctl* ctl,
+               int zc) {
     constexpr int R = ZWindow<T, SCHEME>::R, M = 2 * R, NV = ZWindow<T, SCHEME>::NV, NWZ = ZWindow<T, SCHEME>::NWZ;
     constexpr int NVO = NV + NF, D = ZSWEEP_DEPTH;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -323,8 +326,8 @@ z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restric
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     if (i >= G.n[0] || j >= G.n[1]) return;
-    const int k0 = (int)blockIdx.z * ZSWEEP_ZC;
-    const int k1 = min(k0 + ZSWEEP_ZC, G.n[2]);
+    const int k0 = (int)blockIdx.z * zc;
+    const int k1 = min(k0 + zc, G.n[2]);
     long long p = G.pidx(i, j, k0);
     int flag = 0;
     // stage for plane k: window cell k+R and the old output of plane k
@@ -494,20 +497,20 @@ int launch_fused_scheme(FusedPlan& P, const Geom& G, const StageArgs& A, const T
     if (P.split_z) {
         using S = TileShape<T, SCHEME, false>;
         const dim3 b(32, S::TY, 1);
-        const dim3 g((G.n[0] + 30) / 31, (G.n[1] + S::TY - 2) / (S::TY - 1), (G.n[2] + FUSED_ZC - 1) / FUSED_ZC);
-        stage_tiled_kernel<T, SCHEME, false><<<g, b, S::smem_bytes(), st>>>(P.mapU[0][m], P.mapW[0][mw], G, A, Us, W, Un, Uout, ctl);
+        const dim3 g((G.n[0] + 30) / 31, (G.n[1] + S::TY - 2) / (S::TY - 1), (G.n[2] + P.tile_zc - 1) / P.tile_zc);
+        stage_tiled_kernel<T, SCHEME, false><<<g, b, S::smem_bytes(), st>>>(P.mapU[0][m], P.mapW[0][mw], G, A, Us, W, Un, Uout, ctl, P.tile_zc);
         const dim3 bz(32, 4, 1);
-        const dim3 gz((G.n[0] + 31) / 32, (G.n[1] + 3) / 4, (G.n[2] + ZSWEEP_ZC - 1) / ZSWEEP_ZC);
+        const dim3 gz((G.n[0] + 31) / 32, (G.n[1] + 3) / 4, (G.n[2] + P.sweep_zc - 1) / P.sweep_zc);
         if (SCHEME != 2 && Wnext != nullptr)
-            z_sweep_kernel<T, SCHEME, (SCHEME != 2)><<<gz, bz, zsweep_smem_bytes<T, SCHEME>(), st>>>(G, A, Us, W, Uout, Wnext, ctl);
+            z_sweep_kernel<T, SCHEME, (SCHEME != 2)><<<gz, bz, zsweep_smem_bytes<T, SCHEME>(), st>>>(G, A, Us, W, Uout, Wnext, ctl, P.sweep_zc);
         else
-            z_sweep_kernel<T, SCHEME, false><<<gz, bz, zsweep_smem_bytes<T, SCHEME>(), st>>>(G, A, Us, W, Uout, nullptr, ctl);
+            z_sweep_kernel<T, SCHEME, false><<<gz, bz, zsweep_smem_bytes<T, SCHEME>(), st>>>(G, A, Us, W, Uout, nullptr, ctl, P.sweep_zc);
         *launches = 2;
     } else {
         using S = TileShape<T, SCHEME, true>;
         const dim3 b(32, S::TY, 1);
-        const dim3 g((G.n[0] + 30) / 31, (G.n[1] + S::TY - 2) / (S::TY - 1), (G.n[2] + FUSED_ZC - 1) / FUSED_ZC);
-        stage_tiled_kernel<T, SCHEME, true><<<g, b, S::smem_bytes(), st>>>(P.mapU[1][m], P.mapW[1][mw], G, A, Us, W, Un, Uout, ctl);
+        const dim3 g((G.n[0] + 30) / 31, (G.n[1] + S::TY - 2) / (S::TY - 1), (G.n[2] + P.tile_zc - 1) / P.tile_zc);
+        stage_tiled_kernel<T, SCHEME, true><<<g, b, S::smem_bytes(), st>>>(P.mapU[1][m], P.mapW[1][mw], G, A, Us, W, Un, Uout, ctl, P.tile_zc);
         *launches = 1;
     }
     const cudaError_t e = cudaGetLastError();
