@@ -6,7 +6,8 @@ BASELINE.json configs[4]: the 512^3 periodic lumpy state with 200 hotspots and b
                     [--n 512] [--no-variants] [--no-cpu-baseline] [--impl reference]
 
 One "step" is one SSP-RK3 step of the whole grid with dt = CFL dx / max signal speed taken on the device
-(hydro_step_cfl, reading Q10): ghost fill, con2prim + signal speeds + max reduction, three stage kernels.
+(hydro_step_cfl, reading Q10): per stage the ghost fill, the x/y tile kernel and the z sweep, whose epilogue
+also does con2prim + signal speeds + the CFL max for the next stage.
 Prints ONE JSON line (rank 0).  N > 1 (torchrun): every rank advances its own independent 512^3 event
 (weak scaling, no data-path collective), time = max over ranks.
 
@@ -38,6 +39,9 @@ FLOPS_PER_CELL_STEP = {"weno5": 7041.0, "weno7": 14331.0, "musta": 3831.0}
 FLOPS_PER_CELL_L = {"weno5": 2327.0, "weno7": 4757.0, "musta": 1257.0}
 BYTES_PER_CELL_STEP = {"f64": 320.0, "f32": 160.0}
 # bytes one stage kernel moves per cell, averaged over the three stages of a step: 320/3 (fp64)
+# DRAM bytes of one stage (tile kernel + z sweep), dram__bytes_read.sum + dram__bytes_write.sum of one
+# `ncu --set full` capture each at 512^3: profiles/r01_tiled_ncu.txt, profiles/r01_zsweep_ncu.txt
+TRAFFIC_BYTES_PER_STAGE = {("weno5", "f64", 512): 10.942e9 + 5.393e9 + 14.678e9 + 10.783e9}
 METRIC = "3D cell-updates/s per RK3 step"
 UNIT = "cell-updates/s"
 CFL = 0.2
@@ -192,6 +196,21 @@ def timed_run(B, torch, w, precision, steps, warmup, dist=None, profile=True):
                 wall=(t0, t1))
 
 
+def max_over_ranks(value, dist=None, device="cpu"):
+    """Max of a scalar over all ranks (the multi-GPU timing rule); identity without a process group."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(ncell, steps, world, ms):
+    """Whole-job cell-updates/s: every rank advances its own event of ncell cells (weak scaling)."""
+    return ncell * steps * world / (ms * 1e-3)
+
+
 def roofline(scheme, precision, ncell, stage_ms, stage_n, alu_peak_tf, peaks):
     if stage_n == 0 or stage_ms <= 0:
         return None
@@ -200,8 +219,13 @@ def roofline(scheme, precision, ncell, stage_ms, stage_n, alu_peak_tf, peaks):
     achieved = flops / per_launch_s / 1e12
     byts = BYTES_PER_CELL_STEP[precision] / 3.0 * ncell
     return {"bound": "alu", "achieved": achieved, "peak": alu_peak_tf, "unit": "TFLOP/s",
-            "frac": achieved / alu_peak_tf, "traffic": None,
-            "kernel": "stage kernel (L(u) + RK combine)", "launch_ms": per_launch_s * 1e3,
+            "frac": achieved / alu_peak_tf,
+            "traffic": TRAFFIC_BYTES_PER_STAGE.get((scheme, precision, round(ncell ** (1.0 / 3.0)))),
+            "traffic_note": "DRAM bytes of one stage from profiles/r01_*_ncu.txt; algorithmic bytes of one stage: %.3g"
+                            % (BYTES_PER_CELL_STEP[precision] / 3.0 * ncell),
+            "kernel": "one RK stage = stage_tiled_kernel (x/y fluxes + combine) + z_sweep_kernel (z fluxes, con2prim "
+                      "epilogue), timed together with one CUDA-event pair on the stream",
+            "launch_ms": per_launch_s * 1e3,
             "hbm_gbs_achieved": byts / per_launch_s / 1e9, "hbm_frac": byts / per_launch_s / 1e9 / peaks["hbm_gbs"]}
 
 
@@ -238,12 +262,8 @@ def run_ours(args):
     sampler.start()
     r = timed_run(B, torch, w, args.precision, args.steps, args.warmup, dist)
     clocks = sampler.stop(*r["wall"])
-    ms = r["ms"]
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = ncell * args.steps * world / (ms * 1e-3)
+    ms = max_over_ranks(r["ms"], dist, "cuda")
+    value = aggregate_value(ncell, args.steps, world, ms)
     roof = roofline(args.scheme, args.precision, ncell, r["stage_ms"], r["stage_n"], nominal_tf, peaks)
     if roof is not None:
         roof["peak_source"] = ("nominal: %d SMs x %d lanes x 2 x %.0f MHz (DESIGN.md section 8); "
@@ -273,11 +293,7 @@ def run_ours(args):
     h.step_cfl(CFL, args.steps)
     h.get_state_host(host_out)
     torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(time.perf_counter() - t0, dist, "cuda")
     state_bytes = 5 * ncell * esz
     e2e = {"value": ncell * args.steps * world / e2e_s, "unit": UNIT,
            "h2d_bytes_per_step": state_bytes / max(args.steps, 1),

@@ -354,3 +354,49 @@ def test_tiled_and_generic_kernels_agree(B, scheme, prec, split_z):
         assert h.status() == 0
         h.close()
     assert reldiff(outs[1], outs[0]) <= (1e-12 if prec == 0 else 1e-4)
+
+
+# ------------------------------------------------------------------ full size, the launch configuration bench.py times
+def _crop_periodic(cons, centre, half):
+    """(2 half + 1)^3 block of a periodic state around cell `centre` = (i, j, k)."""
+    idx = [np.arange(c - half, c + half + 1) for c in centre]
+    nz, ny, nx = cons.shape[1:]
+    return np.ascontiguousarray(cons[:, idx[2] % nz][:, :, idx[1] % ny][:, :, :, idx[0] % nx])
+
+
+@pytest.mark.parametrize("scheme,prec,n", [(W.WENO5, 0, 512), (W.WENO7, 0, 256), (W.MUSTA_FORCE, 0, 256), (W.WENO5, 1, 256)])
+def test_full_size_step_on_sampled_cells(B, oracle, scheme, prec, n):
+    """BASELINE configs[4] (configs[3]-size for the other variants) through the kernels bench.py times.  One full
+    RK3 step depends on the cells within 3 r of a cell, so the oracle can recompute any single output cell from
+    a (6 r + 1)^3 crop of the input: sampled cells (tile and z-chunk corners, interior points, the periodic
+    seam) are compared one by one, and the whole grid is checked for the conservation invariant."""
+    w = W.lumpy(n=n, hotspots=200, with_velocity=True, scheme=scheme, nsteps=1, cfl=0.2)
+    h = B.from_workload(w, precision=prec)
+    dt = 0.2 * w.dx / h.max_signal_speed()
+    h.step(dt, 1)
+    ug = h.get_state().cpu().numpy().astype(np.float64)
+    assert h.status() == 0
+    r = {W.WENO5: 3, W.WENO7: 4, W.MUSTA_FORCE: 2}[scheme]
+    half = 3 * r
+    samples = [(0, 0, 0), (n - 1, n - 1, n - 1), (30, 6, 63), (31, 7, 64), (62, 13, 127), (n // 2, n // 2, n // 2),
+               (n - 1, 0, 128), (17, n - 1, 1), (333 % n, 222 % n, 111 % n)]
+    worst = 0.0
+    scale = np.max(np.abs(w.cons[0]))
+    for (i, j, k) in samples:
+        crop = _crop_periodic(w.cons, (i, j, k), half)
+        m = 2 * half + 1
+        wc = W.Workload("crop", (m, m, m), w.dx, (0, 0, 0), scheme, (W.BC_PERIODIC,) * 3, crop)
+        o = oracle.from_workload(wc)
+        o.step(dt, 1)
+        ref = o.get_state()[:, half, half, half]
+        got = ug[:, k, j, i]
+        for c in range(5):
+            den = max(abs(ref[c]), 1e-15 * scale) if c == 0 else max(np.max(np.abs(w.cons[c])), 1e-15 * scale)
+            worst = max(worst, abs(got[c] - ref[c]) / den)
+    assert worst <= (3e-12 if prec == 0 else 1e-5), worst
+    # invariant at any size: the totals are conserved on the periodic grid
+    tot0 = [math.fsum(w.cons[c].ravel()[::1]) for c in range(5)]
+    tot1 = [math.fsum(ug[c].ravel()) for c in range(5)]
+    for a, b in zip(tot0, tot1):
+        assert abs(a - b) <= (1e-13 if prec == 0 else 2e-6) * tot0[0], (tot0, tot1)
+    h.close()
