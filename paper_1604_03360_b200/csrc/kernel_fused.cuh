@@ -145,7 +145,11 @@ struct TileShape {
     // y-fluxes but measured slower than two independent 256-thread blocks per SM (18.1 vs 17.2 ms per stage,
     // WENO5 fp64 512^3): one barrier then stalls the whole SM.
     static constexpr int TY = 8;
-    static constexpr int MIN_BLOCKS = (TY == 16 || WITH_Z || (SCHEME == 1 && sizeof(T) == 8)) ? 1 : 2;
+    // resident blocks per SM the register budget is sized for: fp64 WENO5/MUSTA 2 (128 registers), fp64 WENO7
+    // and the variant with the z window inside 1, fp32 WENO5/MUSTA 3 (80 registers suffice; left free the
+    // compiler takes 126 and the fp32 step is 25 % slower)
+    static constexpr int MIN_BLOCKS = (TY == 16 || WITH_Z || (SCHEME == 1 && sizeof(T) == 8)) ? 1
+                                      : (sizeof(T) == 4 && SCHEME != 1) ? 3 : 2;
     static constexpr int Q = 16 / (int)sizeof(T);                       // elements per 16 bytes
     // box width (x): 32 + 2R - 1 cells plus up to Q-1 of lead-in, because TMA wants the box to start on a
     // 16-byte boundary of the row and to be a multiple of 16 bytes wide
