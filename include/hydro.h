@@ -72,6 +72,7 @@ int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme)
  *                   Hubble flow used by HYDRO_BC_HUBBLE (readings Q13, Q14)
  *   "split_z"       1 (default): a stage is the x/y tiled kernel followed by the z sweep kernel;
  *                   0: one kernel with the z register window inside
+ *   "layout"        with split_z = 1: 1 (default) = x/z marching kernel + y sweep, 0 = x/y tile kernel + z sweep
  *   "tile_zc", "sweep_zc"  planes a block of the tile kernel / of the z sweep marches through (defaults 64 / 128;
  *                   tuning knobs: a longer march amortises the one redundant z-flux and the pipeline fill)
  *   "profile"       0 (default) | 1: record a CUDA event pair on the stream around every stage-kernel

@@ -13,6 +13,7 @@
 #include "../../include/hydro.h"
 #include "grid.cuh"
 #include "kernel_fused.cuh"
+#include "kernel_xz.cuh"
 #include "kernel_generic.cuh"
 #include "kernels_aux.cuh"
 
@@ -323,6 +324,9 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
         const int p = (int)v;
         if (p < 0 || p > 2) return fail(c, HYDRO_EINVAL, "kernel must be 0, 1 or 2");
         c->kernel = p;
+    } else if (k == "layout") {
+        if (v != 0.0 && v != 1.0) return fail(c, HYDRO_EINVAL, "layout must be 0 or 1");
+        c->fused.layout = (int)v;
     } else if (k == "split_z") {
         c->fused.split_z = v != 0.0;
     } else if (k == "tile_zc" || k == "sweep_zc") {

@@ -35,6 +35,7 @@ constexpr int ZSWEEP_ZC = 128;  // default planes per z-chunk of the z sweep ("s
 struct FusedPlan {
     int split_z = 1;  // 1: x/y tiled kernel + z sweep kernel; 0: one kernel with the z window inside
     int tile_zc = FUSED_ZC, sweep_zc = ZSWEEP_ZC;
+    int layout = 1;   // split stage: 1 = x/z marching kernel + y sweep (default), 0 = x/y tile kernel + z sweep
     // TMA descriptors of the three padded state buffers and of the primitive arrays: 4-D tensors
     // (x, y, z, array) with box (RW, RH, 1, 5 or 4); one set per kernel variant [split, with z] because the
     // tile height differs
@@ -54,7 +55,7 @@ __device__ __forceinline__ T shfl_up1(T v) { return __shfl_up_sync(0xffffffffu, 
 // z-stencil of one column held in registers while the block marches along z: cells k-R+1 .. k+R, per cell
 // the five conserved fields and (WENO only) winv, p, a_z.  All indices are compile-time constants after
 // unrolling, so the arrays live in registers.
-template <class T, int SCHEME>
+template <class T, int SCHEME, int DIR = 2>
 struct ZWindow {
     static constexpr int R = SCHEME == 0 ? 3 : (SCHEME == 1 ? 4 : 2);
     static constexpr int M = 2 * R;
@@ -72,7 +73,7 @@ struct ZWindow {
         if (NWZ > 0) {
             v[NF + 0] = __ldg(W + W_INV * fs + q);
             v[NF + 1] = __ldg(W + W_P * fs + q);
-            v[NF + 2] = __ldg(W + (W_AX + 2) * fs + q);
+            v[NF + 2] = __ldg(W + (W_AX + DIR) * fs + q);
         }
     }
     __device__ __forceinline__ void put(int m, const T v[NV]) {
@@ -310,42 +311,47 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 constexpr int ZSWEEP_THREADS = 128;
 constexpr int ZSWEEP_DEPTH = 3;   // planes in flight
 
-// z sweep: Uout += coef * (f(k-1/2) - f(k+1/2)), coef = cb dt / dx (Runge-Kutta mode) or 1 / dx (mode 1).
-// Every global read of the marching loop (the new window cell k+R and the old Uout of plane k) is a
-// cp.async into the thread's own shared-memory slots, ZSWEEP_DEPTH planes ahead: no load latency is
+// Marching sweep along axis DIR (2: z, 1: y): Uout += coef * (f(m-1/2) - f(m+1/2)), coef = cb dt / dx
+// (Runge-Kutta mode) or 1 / dx (mode 1).  One thread per (x, other axis) column, threads of a warp along x (so
+// every access is coalesced whichever axis is marched), the 2r-cell stencil in a register window.
+// Every global read of the marching loop (the new window cell m+R and the old Uout of cell m) is a
+// cp.async into the thread's own shared-memory slots, ZSWEEP_DEPTH cells ahead: no load latency is
 // exposed and no thread reads another thread's slots, so there is no barrier.
 // EPI (WENO schemes, Runge-Kutta mode): the thread holds the finished stage value of its cell, so it also makes
 // the next stage's primitives W' = (winv, p, a_x, a_y, a_z) of that cell (a2-a3; written to the OTHER W buffer,
 // this stage's W is still being read by neighbouring chunks) and, in stage 3, the max signal speed of the new
 // state (a4): the separate con2prim pass over the grid disappears from the step.
-template <class T, int SCHEME, bool EPI>
+template <class T, int SCHEME, bool EPI, int DIR = 2>
 __global__ void __launch_bounds__(ZSWEEP_THREADS, (SCHEME == 1 && sizeof(T) == 8) ? 2 : 3)
 z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, T* Uout, T* Wnext, Ctl* ctl,
                int zc) {
-    constexpr int R = ZWindow<T, SCHEME>::R, M = 2 * R, NV = ZWindow<T, SCHEME>::NV, NWZ = ZWindow<T, SCHEME>::NWZ;
+    using Win = ZWindow<T, SCHEME, DIR>;
+    constexpr int R = Win::R, M = 2 * R, NV = Win::NV, NWZ = Win::NWZ;
     constexpr int NVO = NV + NF, D = ZSWEEP_DEPTH;
+    constexpr int OTHER = DIR == 2 ? 1 : 2;   // the axis blockIdx.y / threadIdx.y run over
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* sm = reinterpret_cast<T*>(smem_raw);   // [D][NVO][ZSWEEP_THREADS]
     const int tid = threadIdx.x + blockDim.x * threadIdx.y;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    if (i >= G.n[0] || j >= G.n[1]) return;
+    if (i >= G.n[0] || j >= G.n[OTHER]) return;
+    const long long ms = DIR == 2 ? G.sxy : G.sx;   // stride of the marched axis
     const int k0 = (int)blockIdx.z * zc;
-    const int k1 = min(k0 + zc, G.n[2]);
-    long long p = G.pidx(i, j, k0);
+    const int k1 = min(k0 + zc, G.n[DIR]);
+    long long p = DIR == 2 ? G.pidx(i, j, k0) : G.pidx(i, k0, j);
     int flag = 0;
-    // stage for plane k: window cell k+R and the old output of plane k
+    // stage for cell k of the march: window cell k+R and the old output of cell k
     auto issue = [&](int k) {
         if (k < k1) {
             T* dst = sm + ((k - k0) % D) * NVO * ZSWEEP_THREADS + tid;
-            const long long q = p + (long long)(k - k0) * G.sxy;   // p stays at plane k0 in this lambda's use
-            const long long qr = q + (long long)R * G.sxy;
+            const long long q = p + (long long)(k - k0) * ms;
+            const long long qr = q + (long long)R * ms;
 #pragma unroll
             for (int c = 0; c < NF; ++c) cp_async<sizeof(T)>(dst + c * ZSWEEP_THREADS, Us + c * G.fs + qr);
             if (NWZ > 0) {
                 cp_async<sizeof(T)>(dst + (NF + 0) * ZSWEEP_THREADS, W + W_INV * G.fs + qr);
                 cp_async<sizeof(T)>(dst + (NF + 1) * ZSWEEP_THREADS, W + W_P * G.fs + qr);
-                cp_async<sizeof(T)>(dst + (NF + 2) * ZSWEEP_THREADS, W + (W_AX + 2) * G.fs + qr);
+                cp_async<sizeof(T)>(dst + (NF + 2) * ZSWEEP_THREADS, W + (W_AX + DIR) * G.fs + qr);
             }
 #pragma unroll
             for (int c = 0; c < NF; ++c) cp_async<sizeof(T)>(dst + (NV + c) * ZSWEEP_THREADS, Uout + c * G.fs + q);
@@ -355,36 +361,34 @@ z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restric
 #pragma unroll
     for (int d = 0; d < D; ++d) issue(k0 + d);
 
-    ZWindow<T, SCHEME> zw;
+    Win zw;
     T nxt[NV], fz_lo[NF];
 #pragma unroll
     for (int m = 0; m < M; ++m) {
-        ZWindow<T, SCHEME>::fetch(nxt, Us, W, G.fs, p + (long long)(m - R) * G.sxy);
+        Win::fetch(nxt, Us, W, G.fs, p + (long long)(m - R) * ms);
         zw.put(m, nxt);
     }
-    iface_from<T, SCHEME, 2>(zw, A, fz_lo, flag);
+    iface_from<T, SCHEME, DIR>(zw, A, fz_lo, flag);
     const T coef = A.mode == 1 ? (T)A.inv_dx : (T)(A.cb * ctl->dt * A.inv_dx);
     const long long p0 = p;
     double amax = 0.0;
     for (int k = k0; k < k1; ++k) {
         T f[NF], o[NF];
-        cp_async_wait<D - 1>();   // the oldest stage (plane k) has landed
+        cp_async_wait<D - 1>();   // the oldest stage (cell k) has landed
         const T* src = sm + ((k - k0) % D) * NVO * ZSWEEP_THREADS + tid;
 #pragma unroll
         for (int v = 0; v < NV; ++v) nxt[v] = src[v * ZSWEEP_THREADS];
-#pragma unroll
-        for (int c = 0; c < NF; ++c) o[c] = src[(NV + c) * ZSWEEP_THREADS];
-        issue(k + D);             // refill the slot just read
         zw.shift();
         zw.put(M - 1, nxt);
-        iface_from<T, SCHEME, 2>(zw, A, f, flag);
-        const long long q = p0 + (long long)(k - k0) * G.sxy;
+        iface_from<T, SCHEME, DIR>(zw, A, f, flag);
+        const long long q = p0 + (long long)(k - k0) * ms;
 #pragma unroll
         for (int c = 0; c < NF; ++c) {
-            o[c] = tfma(coef, fz_lo[c] - f[c], o[c]);
+            o[c] = tfma(coef, fz_lo[c] - f[c], src[(NV + c) * ZSWEEP_THREADS]);   // old output: read late
             Uout[c * G.fs + q] = o[c];
             fz_lo[c] = f[c];
         }
+        issue(k + D);             // refill the slot just consumed
         if (EPI) {
             T w[NW];
             prim_of_cell(o, w, flag);
@@ -410,6 +414,12 @@ template <class T, int SCHEME>
 constexpr size_t zsweep_smem_bytes() {
     return sizeof(T) * (size_t)ZSWEEP_DEPTH * (ZWindow<T, SCHEME>::NV + NF) * ZSWEEP_THREADS;
 }
+
+template <class T, int SCHEME>
+int configure_xz(FusedPlan& P);
+template <class T, int SCHEME>
+int launch_xz_y(FusedPlan& P, const Geom& G, const StageArgs& A, const T* Us, const T* W, const T* Un, T* Uout,
+                T* Wnext, Ctl* ctl, cudaStream_t st, int* launches);
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -444,6 +454,7 @@ int configure_tiled(FusedPlan& P, const Geom& G, void* const U[3], void* const W
         snprintf(P.err, sizeof P.err, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
         return -1;
     }
+    if (configure_xz<T, SCHEME>(P) != 0) return -1;
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) {
         snprintf(P.err, sizeof P.err, "cuTensorMapEncodeTiled not available");
@@ -498,6 +509,7 @@ int launch_fused_scheme(FusedPlan& P, const Geom& G, const StageArgs& A, const T
         snprintf(P.err, sizeof P.err, "stage input is not one of the context's state buffers");
         return -1;
     }
+    if (P.split_z && P.layout == 1) return launch_xz_y<T, SCHEME>(P, G, A, Us, W, Un, Uout, Wnext, ctl, st, launches);
     if (P.split_z) {
         using S = TileShape<T, SCHEME, false>;
         const dim3 b(32, S::TY, 1);

@@ -337,9 +337,10 @@ def test_unphysical_state_raises_the_sticky_flag(B, oracle):
 # ------------------------------------------------------------------ kernel variants agree
 @pytest.mark.parametrize("scheme", SCHEMES)
 @pytest.mark.parametrize("prec", [0, 1])
-@pytest.mark.parametrize("split_z", [1, 0])
-def test_tiled_and_generic_kernels_agree(B, scheme, prec, split_z):
-    """The tiled stage kernels (x/y tile kernel + z sweep, or the single kernel with the z window inside)
+@pytest.mark.parametrize("split_z,layout", [(1, 0), (1, 1), (0, 0)])
+def test_tiled_and_generic_kernels_agree(B, scheme, prec, split_z, layout):
+    """The tiled stage kernels (x/y tile kernel + z sweep, x/z marching kernel + y sweep, or the single kernel
+    with the z window inside)
     against the one-thread-per-cell kernel on a grid spanning several tiles and z-chunks with ragged tails
     in every direction."""
     w = small_workload(scheme, (150, 37, 29))
@@ -349,6 +350,7 @@ def test_tiled_and_generic_kernels_agree(B, scheme, prec, split_z):
     for kern in (B.KERNEL_GENERIC, B.KERNEL_FUSED):
         h = B.from_workload(w, precision=prec, kernel=kern)
         h.set_option("split_z", split_z)
+        h.set_option("layout", layout)
         h.step_cfl(0.2, 3)
         outs.append(h.get_state().cpu().numpy())
         assert h.status() == 0
