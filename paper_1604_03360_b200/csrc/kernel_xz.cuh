@@ -31,7 +31,11 @@ struct XZShape {
     static constexpr int NHL = 2 * R - 1;                     // halo lanes: R-1 cells below, R cells above the row
     static constexpr int RWX = 32 + 2 * R - 1;                // cells of a row with halo
     static constexpr int STAGE = NS * 32 * XZ_ROWS + XZ_ROWS * NHL * NH;
-    static constexpr size_t smem_bytes() { return sizeof(T) * ((size_t)XZ_DEPTH * STAGE + XZ_ROWS * NH * RWX); }
+    // pipeline stages, the warps' rows, and one parking slot per thread and field for the last z-flux (it is
+    // only needed once per plane; parked, the kernel fits its register budget without spilling)
+    static constexpr size_t smem_bytes() {
+        return sizeof(T) * ((size_t)XZ_DEPTH * STAGE + XZ_ROWS * NH * RWX + NF * 32 * XZ_ROWS);
+    }
 };
 
 template <class T, int SCHEME>
@@ -48,6 +52,7 @@ xz_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restri
     const int j = (int)blockIdx.y * XZ_ROWS + wy;
     if (j >= G.n[1]) return;   // whole warp
     T* row = sm + D * S::STAGE + wy * NH * RWX;            // [NH][RWX], this warp's
+    T* park = sm + D * S::STAGE + XZ_ROWS * NH * RWX + tid; // [NF][128]: this thread's last z-flux
     const bool own = lane >= 1 && i < G.n[0];
     const bool need_x = i < G.n[0];                        // i >= -1 always
     const int imax = G.n[0] - 1 + G.g[0];
@@ -96,7 +101,7 @@ xz_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restri
     for (int d = 0; d < D; ++d) issue(k0 + d);
 
     Win zw;
-    T nxt[NV], fz_lo[NF];
+    T nxt[NV];
 #pragma unroll
     for (int m = 0; m < M; ++m) {   // cells k0-R .. k0+R-1
         Win::fetch(nxt, Us, W, G.fs, p0 + (long long)(m - R) * G.sxy);
@@ -105,7 +110,12 @@ xz_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restri
     // the helper lane and the idle lanes of a ragged last tile march through x-ghost columns, whose z-ghost cells
     // are edge ghosts nobody fills: their z-fluxes are discarded, and so must be their unphysical-state flag
     int zflag = 0;
-    iface_from<T, SCHEME, 2>(zw, A, fz_lo, zflag);   // face k0 - 1/2
+    {
+        T f0[NF];
+        iface_from<T, SCHEME, 2>(zw, A, f0, zflag);   // face k0 - 1/2
+#pragma unroll
+        for (int c = 0; c < NF; ++c) park[c * 128] = f0[c];
+    }
     const T dt = (T)ctl->dt, ca = (T)A.ca, cb = (T)A.cb, inv_dx = (T)A.inv_dx;
 
     for (int k = k0; k < k1; ++k) {
@@ -140,8 +150,8 @@ xz_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restri
         iface_from<T, SCHEME, 2>(zw, A, f, zflag);
 #pragma unroll
         for (int c = 0; c < NF; ++c) {
-            L[c] = fz_lo[c] - f[c];
-            fz_lo[c] = f[c];
+            L[c] = park[c * 128] - f[c];
+            park[c * 128] = f[c];
         }
 #pragma unroll
         for (int c = 0; c < NF; ++c) f[c] = (T)0;
