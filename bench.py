@@ -6,7 +6,7 @@ BASELINE.json configs[4]: the 512^3 periodic lumpy state with 200 hotspots and b
                     [--n 512] [--no-variants] [--no-cpu-baseline] [--impl reference]
 
 One "step" is one SSP-RK3 step of the whole grid with dt = CFL dx / max signal speed taken on the device
-(hydro_step_cfl, reading Q10): per stage the ghost fill, the x/y tile kernel and the z sweep, whose epilogue
+(hydro_step_cfl, reading Q10): per stage the ghost fill, the x/z marching kernel and the y sweep, whose epilogue
 also does con2prim + signal speeds + the CFL max for the next stage.
 Prints ONE JSON line (rank 0).  N > 1 (torchrun): every rank advances its own independent 512^3 event
 (weak scaling, no data-path collective), time = max over ranks.
@@ -39,9 +39,9 @@ FLOPS_PER_CELL_STEP = {"weno5": 7041.0, "weno7": 14331.0, "musta": 3831.0}
 FLOPS_PER_CELL_L = {"weno5": 2327.0, "weno7": 4757.0, "musta": 1257.0}
 BYTES_PER_CELL_STEP = {"f64": 320.0, "f32": 160.0}
 # bytes one stage kernel moves per cell, averaged over the three stages of a step: 320/3 (fp64)
-# DRAM bytes of one stage (tile kernel + z sweep), dram__bytes_read.sum + dram__bytes_write.sum of one
-# `ncu --set full` capture each at 512^3: profiles/r01_tiled_ncu.txt, profiles/r01_zsweep_ncu.txt
-TRAFFIC_BYTES_PER_STAGE = {("weno5", "f64", 512): 10.942e9 + 5.393e9 + 14.678e9 + 10.783e9}
+# DRAM bytes of one stage (x/z kernel + y sweep), dram__bytes_read.sum + dram__bytes_write.sum of one
+# `ncu --set full` capture each at 512^3: profiles/r01_xz_ncu.txt, profiles/r01_ysweep_ncu.txt
+TRAFFIC_BYTES_PER_STAGE = {("weno5", "f64", 512): 10.728e9 + 5.398e9 + 14.689e9 + 10.793e9}
 METRIC = "3D cell-updates/s per RK3 step"
 UNIT = "cell-updates/s"
 CFL = 0.2
@@ -223,8 +223,8 @@ def roofline(scheme, precision, ncell, stage_ms, stage_n, alu_peak_tf, peaks):
             "traffic": TRAFFIC_BYTES_PER_STAGE.get((scheme, precision, round(ncell ** (1.0 / 3.0)))),
             "traffic_note": "DRAM bytes of one stage from profiles/r01_*_ncu.txt; algorithmic bytes of one stage: %.3g"
                             % (BYTES_PER_CELL_STEP[precision] / 3.0 * ncell),
-            "kernel": "one RK stage = stage_tiled_kernel (x/y fluxes + combine) + z_sweep_kernel (z fluxes, con2prim "
-                      "epilogue), timed together with one CUDA-event pair on the stream",
+            "kernel": "one RK stage = xz_sweep_kernel (x and z fluxes + combine) + z_sweep_kernel<DIR=y> (y fluxes, "
+                      "con2prim epilogue), timed together with one CUDA-event pair on the stream",
             "launch_ms": per_launch_s * 1e3,
             "hbm_gbs_achieved": byts / per_launch_s / 1e9, "hbm_frac": byts / per_launch_s / 1e9 / peaks["hbm_gbs"]}
 
