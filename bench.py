@@ -161,14 +161,26 @@ def run_reference(args):
 SPLIT_Z = None  # --split-z: override the library's default stage decomposition (experiments)
 
 
-def timed_run(B, torch, w, precision, steps, warmup, dist=None, profile=True):
-    """Warm up, then time `steps` RK3 steps with CUDA events on the stream.  Returns a dict."""
+def timed_run(B, torch, w, precision, steps, warmup, dist=None, profile=True, slab=None):
+    """Warm up, then time `steps` RK3 steps with CUDA events on the stream.  Returns a dict.
+    slab = (rank, world): this rank owns one z-slab of the global grid and exchanges halo planes with its
+    neighbours every stage (paper_1604_03360_b200/slab.py); otherwise the rank advances the whole grid."""
     prec = B.F32 if precision == "f32" else B.F64
-    h = B.from_workload(w, precision=prec)
+    if slab is None:
+        h = B.from_workload(w, precision=prec)
+        advance = lambda k: h.step_cfl(CFL, k)
+    else:
+        from paper_1604_03360_b200 import slab as S
+        rank, world = slab
+        k0, k1 = S.split_planes(w.n[2], world)[rank]
+        h = S.make_slab(B, w, k0, k1, precision=prec)
+        comm = S.DistComm(dist, w.bc[2]) if dist is not None else S.LocalComm(1, w.bc[2])
+        group = S.SlabGroup([h], comm, w.dx)
+        advance = lambda k: group.step_cfl(CFL, k)
     if SPLIT_Z is not None:
         h.set_option("split_z", SPLIT_Z)
     stream = torch.cuda.current_stream()
-    h.step_cfl(CFL, warmup)
+    advance(warmup)
     torch.cuda.synchronize()
     if profile:
         h.set_option("profile", 1)
@@ -180,7 +192,7 @@ def timed_run(B, torch, w, precision, steps, warmup, dist=None, profile=True):
     t0 = time.perf_counter()
     e0.record(stream)
     for _ in range(steps):
-        h.step_cfl(CFL, 1)
+        advance(1)
     e1.record(stream)
     torch.cuda.synchronize()
     t1 = time.perf_counter()
@@ -193,7 +205,7 @@ def timed_run(B, torch, w, precision, steps, warmup, dist=None, profile=True):
     status = h.status()
     tnow = h.time
     return dict(h=h, ms=ms, launches=launches, stage_ms=stage_ms, stage_n=stage_n, status=status, t=tnow,
-                wall=(t0, t1))
+                wall=(t0, t1), advance=advance)
 
 
 def max_over_ranks(value, dist=None, device="cpu"):
@@ -249,7 +261,10 @@ def run_ours(args):
 
     n = args.n
     ncell = n ** 3
-    w = make_workload(n, args.scheme, rank)
+    slab_mode = args.decomp == "slab"
+    # events: every rank its own event (seeded by rank); slab: ONE global event, this rank owns a z-slab of it
+    w = make_workload(n, args.scheme, 0 if slab_mode else rank)
+    slab = (rank, world) if slab_mode else None
 
     # ALU roofline denominator: 148 SMs x 64 fp64 (128 fp32) FMA lanes x 2 flop x
     # the SM clock.  Nominal uses clocks.max.sm; the sustained figure is measured by the library's probe.
@@ -260,11 +275,12 @@ def run_ours(args):
 
     sampler = ClockSampler(local)
     sampler.start()
-    r = timed_run(B, torch, w, args.precision, args.steps, args.warmup, dist)
+    r = timed_run(B, torch, w, args.precision, args.steps, args.warmup, dist, slab=slab)
     clocks = sampler.stop(*r["wall"])
     ms = max_over_ranks(r["ms"], dist, "cuda")
-    value = aggregate_value(ncell, args.steps, world, ms)
-    roof = roofline(args.scheme, args.precision, ncell, r["stage_ms"], r["stage_n"], nominal_tf, peaks)
+    value = aggregate_value(ncell, args.steps, 1 if slab_mode else world, ms)
+    ncell_local = ncell // world if slab_mode else ncell
+    roof = roofline(args.scheme, args.precision, ncell_local, r["stage_ms"], r["stage_n"], nominal_tf, peaks)
     if roof is not None:
         roof["peak_source"] = ("nominal: %d SMs x %d lanes x 2 x %.0f MHz (DESIGN.md section 8); "
                                "hbm peak %s" % (sms, lanes, peaks.get("sm_max_mhz", 1965.0), peaks_src))
@@ -280,26 +296,32 @@ def run_ours(args):
     h = r.pop("h")
     esz = 8 if args.precision == "f64" else 4
     tdt = torch.float64 if args.precision == "f64" else torch.float32
-    host_in = torch.from_numpy(w.cons).to(tdt).pin_memory()
+    advance = r.pop("advance")
+    if slab_mode:
+        from paper_1604_03360_b200 import slab as S
+        k0, k1 = S.split_planes(n, world)[rank]
+        host_in = torch.from_numpy(np.ascontiguousarray(w.cons[:, k0:k1])).to(tdt).pin_memory()
+    else:
+        host_in = torch.from_numpy(w.cons).to(tdt).pin_memory()
     host_out = torch.empty_like(host_in).pin_memory()
     h.set_state_host(host_in)          # warm the copy path
-    h.step_cfl(CFL, 1)
+    advance(1)
     h.get_state_host(host_out)
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     h.set_state_host(host_in)
-    h.step_cfl(CFL, args.steps)
+    advance(args.steps)
     h.get_state_host(host_out)
     torch.cuda.synchronize()
     e2e_s = max_over_ranks(time.perf_counter() - t0, dist, "cuda")
-    state_bytes = 5 * ncell * esz
-    e2e = {"value": ncell * args.steps * world / e2e_s, "unit": UNIT,
+    state_bytes = 5 * ncell_local * esz
+    e2e = {"value": aggregate_value(ncell, args.steps, 1 if slab_mode else world, e2e_s * 1e3), "unit": UNIT,
            "h2d_bytes_per_step": state_bytes / max(args.steps, 1),
            "d2h_bytes_per_step": state_bytes / max(args.steps, 1),
-           "job": "hydro_set_state_host (pinned) + hydro_step_cfl(%d) + hydro_get_state_host; "
-                  "state %d bytes each way per job" % (args.steps, state_bytes),
+           "job": "hydro_set_state_host (pinned) + %d steps + hydro_get_state_host; "
+                  "state %d bytes each way per job and rank" % (args.steps, state_bytes),
            "finite": bool(torch.isfinite(host_out).all().item())}
     launches_per_step = r["launches"] / max(args.steps, 1)
     h.close()
@@ -308,7 +330,7 @@ def run_ours(args):
 
     # ---- the other headline variants of config 5 (same grid, fewer steps each)
     variants = {}
-    if not args.no_variants and rank == 0 and world == 1:
+    if not args.no_variants and rank == 0 and world == 1 and not slab_mode:
         for sch, prec in (("weno5", "f64"), ("weno7", "f64"), ("musta", "f64"), ("weno5", "f32"), ("weno7", "f32")):
             if (sch, prec) == (args.scheme, args.precision):
                 continue
@@ -339,15 +361,19 @@ def run_ours(args):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / max(args.steps, 1), "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
+            "scaling": "strong" if slab_mode else "weak", "vs_baseline": None, "dtype": args.precision,
+            "data": "synthetic",
             "config": {"workload": "BASELINE.json configs[4]: %d^3 periodic lumpy state, 200 hotspots, blended "
-                                   "velocities, %s %s, CFL %.1f (one independent event per GPU)" %
-                                   (n, args.scheme, args.precision, CFL),
-                       "grid": [n, n, n], "scheme": args.scheme, "cfl": CFL,
+                                   "velocities, %s %s, CFL %.1f (%s)" %
+                                   (n, args.scheme, args.precision, CFL,
+                                    "one event, z-slab per GPU, halo exchange per stage" if slab_mode
+                                    else "one independent event per GPU"),
+                       "grid": [n, n, n], "scheme": args.scheme, "cfl": CFL, "decomp": args.decomp,
                        "l2": "no flush needed: the state (%.2f GB per copy) is far larger than the 126 MB L2" %
                              (state_bytes / 1e9)},
             "roofline": roof,
             "step_roofline": {"value": value / world, "roof": step_roof, "frac": value / world / step_roof,
+                              "per": "GPU",
                               "flop_roof": flop_roof, "byte_roof": byte_roof, "unit": UNIT,
                               "note": "min(hbm peak / 320 B, nominal ALU peak / algorithmic flops) per cell-update"},
             "cpu_baseline": cpu,
@@ -378,6 +404,9 @@ def main():
     ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--split-z", type=int, default=None, choices=[0, 1])
+    ap.add_argument("--decomp", default="events", choices=["events", "slab"],
+                    help="N > 1: 'events' = one independent event per GPU (weak scaling, no data-path collective); "
+                         "'slab' = one event decomposed along z, halo exchange per stage (strong scaling)")
     args = ap.parse_args()
     global SPLIT_Z
     SPLIT_Z = args.split_z

@@ -43,7 +43,8 @@ extern "C" {
 typedef struct hydro_ctx hydro_ctx; /* opaque, owned by the library */
 
 enum { HYDRO_WENO5 = 0, HYDRO_WENO7 = 1, HYDRO_MUSTA_FORCE = 2 };          /* scheme            */
-enum { HYDRO_BC_OUTFLOW = 0, HYDRO_BC_PERIODIC = 1, HYDRO_BC_HUBBLE = 2 }; /* per axis          */
+enum { HYDRO_BC_OUTFLOW = 0, HYDRO_BC_PERIODIC = 1, HYDRO_BC_HUBBLE = 2,
+       HYDRO_BC_EXTERNAL = 3 /* z only: the caller provides the ghost planes (hydro_put_zhalo) */ }; /* per axis */
 enum { HYDRO_F64 = 0, HYDRO_F32 = 1 };                                     /* "precision"       */
 enum { HYDRO_KERNEL_AUTO = 0, HYDRO_KERNEL_GENERIC = 1, HYDRO_KERNEL_FUSED = 2 }; /* "kernel"   */
 enum {
@@ -130,6 +131,19 @@ int hydro_status(hydro_ctx *ctx);
 
 /* Number of kernels the context has launched since creation (bench.py "gpu_launches"). */
 long long hydro_launch_count(const hydro_ctx *ctx);
+
+/* Slab decomposition along z: with "bc_z" = HYDRO_BC_EXTERNAL the z-ghost planes of a
+ * stage input are the caller's business.  `buffer` is the state buffer that is the input of stage 0, 1, 2 of a
+ * step (0 = u^n).  hydro_get_zhalo packs the g outermost INTERIOR planes of `side` (0 low z, 1 high z) into a
+ * DEVICE buffer [5][g][ny][nx] (hydro_zhalo_elems elements of the context's precision); hydro_put_zhalo writes
+ * such a buffer into the g GHOST planes of `side`.  hydro_step_stage runs ONE stage (0, 1, 2, in this order)
+ * of a step of size dt: x/y ghost fill, the stage kernels; stage 2 also advances the time.  A driver advances
+ * a slab as: for s in 0..2 { get both halos of buffer s, exchange with the neighbours, put, step_stage(dt, s) }.
+ * All asynchronous on the stream. */
+size_t hydro_zhalo_elems(const hydro_ctx *ctx);
+int hydro_get_zhalo(hydro_ctx *ctx, int buffer, int side, void *packed_device_out);
+int hydro_put_zhalo(hydro_ctx *ctx, int buffer, int side, const void *packed_device_in);
+int hydro_step_stage(hydro_ctx *ctx, double dt, int stage);
 
 /* With the "profile" option on: total device time in milliseconds of the stage kernels (the L(u) +
  * Runge-Kutta kernel, the dominant one) launched since the last call, and their number, written to HOST

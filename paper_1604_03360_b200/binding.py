@@ -12,7 +12,7 @@ import os
 import torch
 
 WENO5, WENO7, MUSTA_FORCE = 0, 1, 2
-BC_OUTFLOW, BC_PERIODIC, BC_HUBBLE = 0, 1, 2
+BC_OUTFLOW, BC_PERIODIC, BC_HUBBLE, BC_EXTERNAL = 0, 1, 2, 3
 F64, F32 = 0, 1
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_FUSED = 0, 1, 2
 OK, EINVAL, ENOMEM, ECUDA, EUNPHYSICAL = 0, -1, -2, -3, -4
@@ -24,7 +24,8 @@ SYMBOLS = [
     "hydro_create", "hydro_set_option", "hydro_set_stream", "hydro_workspace_bytes", "hydro_bind_workspace",
     "hydro_set_state", "hydro_get_state", "hydro_set_state_host", "hydro_get_state_host", "hydro_step",
     "hydro_step_cfl", "hydro_max_signal_speed", "hydro_eval_L", "hydro_get_time", "hydro_status",
-    "hydro_launch_count", "hydro_stage_kernel_time", "hydro_last_error", "hydro_destroy", "hydro_probe_fma_peak",
+    "hydro_launch_count", "hydro_stage_kernel_time", "hydro_last_error",
+    "hydro_zhalo_elems", "hydro_get_zhalo", "hydro_put_zhalo", "hydro_step_stage", "hydro_destroy", "hydro_probe_fma_peak",
 ]
 
 
@@ -60,6 +61,11 @@ def _load():
     L.hydro_launch_count.argtypes = [vp]
     L.hydro_launch_count.restype = ctypes.c_longlong
     L.hydro_stage_kernel_time.argtypes = [vp, pd, ctypes.POINTER(ctypes.c_longlong)]
+    L.hydro_zhalo_elems.argtypes = [vp]
+    L.hydro_zhalo_elems.restype = sz
+    L.hydro_get_zhalo.argtypes = [vp, i32, i32, vp]
+    L.hydro_put_zhalo.argtypes = [vp, i32, i32, vp]
+    L.hydro_step_stage.argtypes = [vp, dbl, i32]
     L.hydro_last_error.argtypes = [vp]
     L.hydro_last_error.restype = ctypes.c_char_p
     L.hydro_destroy.argtypes = [vp]
@@ -173,6 +179,23 @@ class Hydro:
     @property
     def launch_count(self):
         return lib.hydro_launch_count(self._h)
+
+    def zhalo_elems(self):
+        return lib.hydro_zhalo_elems(self._h)
+
+    def get_zhalo(self, buffer, side, out=None):
+        if out is None:
+            out = torch.empty(self.zhalo_elems(), dtype=self.dtype, device=self.device)
+        assert out.is_cuda and out.is_contiguous() and out.dtype == self.dtype and out.numel() == self.zhalo_elems()
+        self._check(lib.hydro_get_zhalo(self._h, int(buffer), int(side), out.data_ptr()))
+        return out
+
+    def put_zhalo(self, buffer, side, packed):
+        assert packed.is_cuda and packed.is_contiguous() and packed.dtype == self.dtype and packed.numel() == self.zhalo_elems()
+        self._check(lib.hydro_put_zhalo(self._h, int(buffer), int(side), packed.data_ptr()))
+
+    def step_stage(self, dt, stage):
+        self._check(lib.hydro_step_stage(self._h, float(dt), int(stage)))
 
     def stage_kernel_time(self):
         """(total ms, launches) of the stage kernels since the last call ("profile" option)."""

@@ -222,7 +222,7 @@ int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double 
 // other W buffer (and stage 3 the max signal speed), so con2prim runs as a separate pass only for the first
 // step after hydro_set_state / hydro_eval_L; the ghost cells' primitives come from the halo kernel.
 template <class T>
-int do_step(hydro_ctx* c, double dt_fixed, double cfl) {
+int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl) {
     T* U[3] = {(T*)c->U[0], (T*)c->U[1], (T*)c->U[2]};
     const bool weno = c->scheme != HYDRO_MUSTA_FORCE;
     const bool cflmode = !(dt_fixed > 0.0);
@@ -232,27 +232,55 @@ int do_step(hydro_ctx* c, double dt_fixed, double cfl) {
     T* const in[3] = {U[0], U[1], U[2]};
     T* const out[3] = {U[1], U[2], U[0]};   // stage 3 writes u^n in place: each cell reads only its own u^n
     int rc;
-    bool have_w = c->w_ready;
-    for (int s = 0; s < 3; ++s) {
-        if ((rc = do_halo<T>(c, in[s], tfrac[s], false, 0.0, (weno && have_w) ? (T*)c->Wb[c->wcur] : nullptr))) return rc;
-        if (weno && !have_w) {
-            if ((rc = do_prim<T>(c, in[s], (s == 0 && cflmode) ? 1 : 0))) return rc;
-        } else if (!weno && s == 0 && cflmode) {
-            if ((rc = do_max_speed<T>(c, in[s]))) return rc;
-        }
-        if (s == 0) {
-            begin_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl, dt_fixed, cfl, c->dx);
-            LAUNCHED(c, "begin_step_kernel");
-        }
-        T* Wnext = epi ? (T*)c->Wb[c->wcur ^ 1] : nullptr;
-        if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, Wnext, s == 2 ? 1 : 0))) return rc;
-        if (epi) c->wcur ^= 1;
-        have_w = epi;
+    const bool have_w = c->w_ready;   // interior primitives of in[s] already in Wb[wcur] (previous stage's epilogue)
+    if ((rc = do_halo<T>(c, in[s], tfrac[s], false, 0.0, (weno && have_w) ? (T*)c->Wb[c->wcur] : nullptr))) return rc;
+    if (weno && !have_w) {
+        if ((rc = do_prim<T>(c, in[s], (s == 0 && cflmode) ? 1 : 0))) return rc;
+    } else if (!weno && s == 0 && cflmode) {
+        if ((rc = do_max_speed<T>(c, in[s]))) return rc;
     }
-    c->w_ready = have_w;
-    end_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
-    LAUNCHED(c, "end_step_kernel");
+    if (s == 0) {
+        begin_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl, dt_fixed, cfl, c->dx);
+        LAUNCHED(c, "begin_step_kernel");
+    }
+    T* Wnext = epi ? (T*)c->Wb[c->wcur ^ 1] : nullptr;
+    if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, Wnext, s == 2 ? 1 : 0))) return rc;
+    if (epi) c->wcur ^= 1;
+    c->w_ready = epi;
+    if (s == 2) {
+        end_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
+        LAUNCHED(c, "end_step_kernel");
+    }
     return HYDRO_OK;
+}
+
+template <class T>
+int do_step(hydro_ctx* c, double dt_fixed, double cfl) {
+    for (int s = 0; s < 3; ++s) {
+        const int rc = do_step_stage<T>(c, s, dt_fixed, cfl);
+        if (rc) return rc;
+    }
+    return HYDRO_OK;
+}
+
+// z-halo planes of one state buffer <-> a packed device buffer [5][g][ny][nx] (slab decomposition, DESIGN 9).
+// get: the g outermost INTERIOR planes of the side; put: the g GHOST planes of the side.
+template <class T>
+__global__ void zhalo_kernel(Geom G, T* pad, T* packed, int side, int put) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int l = blockIdx.z;   // 0 .. g-1, in increasing z
+    if (i >= G.n[0] || j >= G.n[1]) return;
+    const int g = G.g[2];
+    const int k = put ? (side == 0 ? l - g : G.n[2] + l) : (side == 0 ? l : G.n[2] - g + l);
+    const long long p = G.pidx(i, j, k);
+    const long long plane = (long long)G.n[0] * G.n[1];
+    const long long q = ((long long)l * G.n[1] + j) * G.n[0] + i;
+#pragma unroll
+    for (int c = 0; c < NF; ++c) {
+        if (put) pad[c * G.fs + p] = packed[c * g * plane + q];
+        else packed[c * g * plane + q] = pad[c * G.fs + p];
+    }
 }
 
 template <class T>
@@ -336,7 +364,7 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
         c->profile = v != 0.0;
     } else if (k == "bc_x" || k == "bc_y" || k == "bc_z") {
         const int b = (int)v;
-        if (b < 0 || b > 2) return fail(c, HYDRO_EINVAL, "unknown boundary rule %d", b);
+        if (b < 0 || b > 3 || (b == 3 && k[3] != 'z')) return fail(c, HYDRO_EINVAL, "unknown boundary rule %d", b);
         c->bc[k[3] - 'x'] = b;
     } else if (k == "musta_stages") {
         if (v < 1) return fail(c, HYDRO_EINVAL, "musta_stages < 1");
@@ -476,6 +504,15 @@ int hydro_max_signal_speed(hydro_ctx* c, double* out_host) {
     int rc = need_ws(c);
     if (rc) return rc;
     if (!out_host) return HYDRO_EINVAL;
+    if (c->w_ready) {   // the stage-3 epilogue of the last step left the max speed of u^n in the control block
+        Ctl h0;
+        CUDA_OK(c, cudaMemcpyAsync(&h0, c->ctl, sizeof h0, cudaMemcpyDeviceToHost, c->stream));
+        CUDA_OK(c, cudaStreamSynchronize(c->stream));
+        if (h0.maxspeed_bits != 0ull) {
+            memcpy(out_host, &h0.maxspeed_bits, sizeof(double));
+            return HYDRO_OK;
+        }
+    }
     reset_max_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
     LAUNCHED(c, "reset_max_kernel");
     rc = c->precision == HYDRO_F64 ? do_max_speed<double>(c, (const double*)c->U[0])
@@ -495,6 +532,35 @@ int hydro_eval_L(hydro_ctx* c, const void* cons, double t_stage, void* L_out) {
     if (!cons || !L_out) return HYDRO_EINVAL;
     return c->precision == HYDRO_F64 ? eval_L_impl<double>(c, cons, t_stage, L_out)
                                      : eval_L_impl<float>(c, cons, t_stage, L_out);
+}
+
+size_t hydro_zhalo_elems(const hydro_ctx* c) {
+    if (!c) return 0;
+    return (size_t)NF * c->G.g[2] * c->G.n[1] * c->G.n[0];
+}
+
+static int zhalo_impl(hydro_ctx* c, int buffer, int side, void* packed, int put) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    if (!packed || buffer < 0 || buffer > 2 || (side != 0 && side != 1)) return fail(c, HYDRO_EINVAL, "zhalo: bad argument");
+    if (c->G.g[2] == 0) return fail(c, HYDRO_EINVAL, "zhalo: the z axis is inactive");
+    const dim3 b = blk2d(64, 4);
+    const dim3 g((c->G.n[0] + b.x - 1) / b.x, (c->G.n[1] + b.y - 1) / b.y, c->G.g[2]);
+    if (c->precision == HYDRO_F64) zhalo_kernel<double><<<g, b, 0, c->stream>>>(c->G, (double*)c->U[buffer], (double*)packed, side, put);
+    else zhalo_kernel<float><<<g, b, 0, c->stream>>>(c->G, (float*)c->U[buffer], (float*)packed, side, put);
+    LAUNCHED(c, "zhalo_kernel");
+    return HYDRO_OK;
+}
+int hydro_get_zhalo(hydro_ctx* c, int buffer, int side, void* packed_out) { return zhalo_impl(c, buffer, side, packed_out, 0); }
+int hydro_put_zhalo(hydro_ctx* c, int buffer, int side, const void* packed_in) {
+    return zhalo_impl(c, buffer, side, const_cast<void*>(packed_in), 1);
+}
+
+int hydro_step_stage(hydro_ctx* c, double dt, int stage) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    if (!(dt > 0) || stage < 0 || stage > 2) return fail(c, HYDRO_EINVAL, "hydro_step_stage: dt <= 0 or stage not in 0..2");
+    return c->precision == HYDRO_F64 ? do_step_stage<double>(c, stage, dt, 0.0) : do_step_stage<float>(c, stage, dt, 0.0);
 }
 
 int hydro_stage_kernel_time(hydro_ctx* c, double* ms_total_host, long long* launches_host) {

@@ -134,7 +134,14 @@ __global__ void halo_fill_kernel(Geom G, HaloArgs A, Ctl* ctl, double tfrac, dou
     ix[a2] = src[a2] = q2;
     ix[a] = side == 0 ? -l : G.n[a] - 1 + l;
     T val[NF];
-    if (A.bc[a] == 2) {
+    if (A.bc[a] == 3) {
+        // external ghosts (slab decomposition): the caller put them there (hydro_put_zhalo); only their
+        // primitives may have to be made below
+        if (Wghost == nullptr) return;
+        const long long pg = G.pidx(ix[0], ix[1], ix[2]);
+#pragma unroll
+        for (int c = 0; c < NF; ++c) val[c] = pad[c * G.fs + pg];
+    } else if (A.bc[a] == 2) {
         const double tt = use_abs ? t_abs : ctl->t + tfrac * ctl->dt;
         hubble_cons<T>(A.H, A.bc, ix[0], ix[1], ix[2], tt, val);
     } else {
@@ -145,8 +152,10 @@ __global__ void halo_fill_kernel(Geom G, HaloArgs A, Ctl* ctl, double tfrac, dou
         for (int c = 0; c < NF; ++c) val[c] = pad[c * G.fs + ps];
     }
     const long long p = G.pidx(ix[0], ix[1], ix[2]);
+    if (A.bc[a] != 3) {
 #pragma unroll
-    for (int c = 0; c < NF; ++c) pad[c * G.fs + p] = val[c];
+        for (int c = 0; c < NF; ++c) pad[c * G.fs + p] = val[c];
+    }
     // when the interior primitives came from the previous stage's z-sweep epilogue, the ghost cells' are made here
     if (Wghost != nullptr) {
         T w[NW];

@@ -1,0 +1,103 @@
+"""Slab decomposition along z.  CPU: the partition and neighbour logic, and the
+neighbour exchange / max-reduction over a 2-rank gloo group (the same code that runs over NCCL).  GPU (-m gpu):
+several slabs advanced in lockstep in one process must reproduce the undecomposed run BIT FOR BIT."""
+import os
+import sys
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1604_03360_b200 import slab as S            # noqa: E402  (pure torch; loads no CUDA library)
+from paper_1604_03360_b200 import workloads as W       # noqa: E402
+
+
+def test_split_and_neighbours():
+    assert S.split_planes(10, 3) == [(0, 4), (4, 7), (7, 10)]
+    assert S.split_planes(512, 8)[-1] == (448, 512)
+    assert S.neighbours(0, 4, S.BC_PERIODIC) == (3, 1) and S.neighbours(3, 4, S.BC_PERIODIC) == (2, 0)
+    assert S.neighbours(0, 4, S.BC_OUTFLOW) == (None, 1) and S.neighbours(3, 4, S.BC_OUTFLOW) == (2, None)
+    assert S.neighbours(0, 1, S.BC_PERIODIC) == (0, 0)
+
+
+def test_outflow_ghost_repeats_the_boundary_plane():
+    g, ny, nx = 3, 2, 4
+    planes = torch.arange(5 * g * ny * nx, dtype=torch.float64)
+    lo = S.outflow_ghost(planes, g, 0).view(5, g, ny * nx)
+    hi = S.outflow_ghost(planes, g, 1).view(5, g, ny * nx)
+    src = planes.view(5, g, ny * nx)
+    for l in range(g):
+        assert torch.equal(lo[:, l], src[:, 0]) and torch.equal(hi[:, l], src[:, g - 1])
+
+
+def test_local_comm_wiring():
+    for bc in (S.BC_PERIODIC, S.BC_OUTFLOW):
+        c = S.LocalComm(3, bc)
+        pairs = [("lo%d" % r, "hi%d" % r) for r in range(3)]
+        got = c.exchange(pairs)
+        assert got[1] == ("hi0", "lo2")
+        assert got[0] == (("hi2" if bc == S.BC_PERIODIC else None), "lo1")
+        assert got[2] == ("hi1", ("lo0" if bc == S.BC_PERIODIC else None))
+        assert c.max([0.2, 0.7, 0.5]) == 0.7
+
+
+def _worker(rank, world, port, bc, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    comm = S.DistComm(dist, bc)
+    lo = torch.full((6,), 10.0 * rank + 1.0, dtype=torch.float64)     # "my lowest planes"
+    hi = torch.full((6,), 10.0 * rank + 2.0, dtype=torch.float64)     # "my highest planes"
+    (below, above), = comm.exchange([(lo, hi)])
+    m = comm.max([0.3 + 0.1 * rank])
+    out[rank] = (None if below is None else float(below[0]), None if above is None else float(above[0]), m)
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("bc", [S.BC_PERIODIC, S.BC_OUTFLOW])
+def test_dist_comm_over_gloo_two_ranks(bc):
+    world, port = 2, 31500 + os.getpid() % 2000 + bc
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_worker, args=(world, port, bc, out), nprocs=world, join=True)
+        res = dict(out)
+    # rank 0's ghosts above are rank 1's lowest planes (11), rank 1's ghosts below are rank 0's highest (2)
+    assert res[0][1] == 11.0 and res[1][0] == 2.0
+    if bc == S.BC_PERIODIC:
+        assert res[0][0] == 12.0 and res[1][1] == 1.0       # the ring closes
+    else:
+        assert res[0][0] is None and res[1][1] is None      # physical ends
+    assert res[0][2] == res[1][2] == pytest.approx(0.4)
+
+
+# ------------------------------------------------------------------ GPU: bit-identity with the undecomposed run
+@pytest.mark.gpu
+@pytest.mark.parametrize("scheme", [W.WENO5, W.WENO7, W.MUSTA_FORCE])
+@pytest.mark.parametrize("bc_z,parts", [(W.BC_PERIODIC, 2), (W.BC_OUTFLOW, 3), (W.BC_PERIODIC, 1)])
+def test_slabs_reproduce_the_single_domain_run_bit_for_bit(scheme, bc_z, parts):
+    from paper_1604_03360_b200 import binding as B
+    n = (40, 33, 70)
+    big = W.lumpy(n=max(n), hotspots=12, with_velocity=True, scheme=scheme, box=max(n) / 16.0, sigma_unit=0.12)
+    cons = np.ascontiguousarray(big.cons[:, :n[2], :n[1], :n[0]])
+    w = W.Workload("slab", n, big.dx, (0.0, 0.0, 0.0), scheme, (W.BC_PERIODIC, W.BC_OUTFLOW, bc_z), cons, 0.0, cfl=0.2)
+    ref = B.from_workload(w)
+    ref.step_cfl(0.2, 3)
+    want = ref.get_state().cpu()
+    t_ref = ref.time
+    ref.close()
+    ranges = S.split_planes(n[2], parts)
+    hs = [S.make_slab(B, w, k0, k1) for k0, k1 in ranges]
+    group = S.SlabGroup(hs, S.LocalComm(parts, bc_z), w.dx)
+    group.step_cfl(0.2, 3)
+    got = torch.cat([h.get_state().cpu() for h in hs], dim=1)
+    assert all(h.status() == 0 for h in hs)
+    assert abs(hs[0].time - t_ref) == 0.0
+    assert torch.equal(got, want)
+    for h in hs:
+        h.close()
