@@ -1,5 +1,11 @@
-// kernel_fused.cuh -- the tiled stage kernels: L(u) of Eq. (2) fused with the SSP-RK3
-// combination (a9), every interface flux computed once.
+// kernel_fused.cuh -- stage kernels: L(u) of Eq. (2) fused with the SSP-RK3 combination
+// (a9), every interface flux computed once.  This header holds
+//   * z_sweep_kernel<T, SCHEME, EPI, DIR>: the marching sweep along y (DIR = 1, default layout) or z (DIR = 2):
+//     thread per (x, other axis) column, 2r-cell stencil in a register window, cp.async pipeline, optional
+//     con2prim epilogue.  With kernel_xz.cuh's x/z marching kernel it forms the DEFAULT stage ("layout" 1);
+//   * stage_tiled_kernel<T, SCHEME, WITH_Z>: the TMA-staged x/y tile kernel of the alternative layout
+//     ("layout" 0: tile kernel, then the z sweep) and, with WITH_Z, the single-kernel variant ("split_z" 0);
+//   * the plan (tensor maps, shared-memory attributes) and the launchers.
 //
 // stage_tiled_kernel<T, SCHEME, WITH_Z>
 //   A block is 32 x TY threads over an (x, y) tile and marches along z through a chunk of planes.  Thread
@@ -14,9 +20,6 @@
 //   WITH_Z: z: f(k+1/2) by owning threads from a register window of the column (cells k-R+1 .. k+R,
 //     shifted and refilled by one prefetched plane per step) -> lower face is last plane's flux.
 //   Redundant work: one column of x-fluxes per 31, one row of y-fluxes per TY-1, one z-flux per chunk.
-// z_sweep_kernel<T, SCHEME>   (used when the stage is split: tiled kernel without z, then this)
-//   thread per (i, j) column marching along z with the same register window, adds the z-flux difference
-//   to the output of the x/y kernel.  No shared memory, no barrier, no redundancy except one flux per chunk.
 #pragma once
 #include <cuda.h>
 

@@ -218,6 +218,26 @@ def test_step_cfl_follows_the_oracle_dt_sequence(B, oracle):
         h.close()
 
 
+def test_max_signal_speed_after_steps_uses_the_epilogue_value(B, oracle):
+    """After a step the max signal speed comes from the stage-3 epilogue (no extra pass over the grid): it
+    must equal the oracle's for the new state, and agree with a context that recomputes it."""
+    w = small_workload(W.WENO5, (40, 33, 70))
+    o = oracle.from_workload(w)
+    w.nsteps = 3
+    dts = oracle.run(o, w)
+    h = B.from_workload(w)
+    for dt in dts:
+        h.step(dt, 1)
+    cached = h.max_signal_speed()
+    ref = o.max_signal_speed()
+    assert abs(cached - ref) <= 1e-13 * ref
+    h2 = B.from_workload(w)
+    h2.set_state(h.get_state())            # same state, no epilogue history: recomputed by max_speed_kernel
+    assert abs(h2.max_signal_speed() - cached) <= 4e-16 * cached
+    h.close()
+    h2.close()
+
+
 # ------------------------------------------------------------------ config 1: Sod tube, full size
 @pytest.mark.parametrize("scheme", SCHEMES)
 def test_config1_sod_full_run(B, oracle, scheme):
