@@ -422,3 +422,47 @@ def test_full_size_step_on_sampled_cells(B, oracle, scheme, prec, n):
     for a, b in zip(tot0, tot1):
         assert abs(a - b) <= (1e-13 if prec == 0 else 2e-6) * tot0[0], (tot0, tot1)
     h.close()
+
+
+# ------------------------------------------------------------------ configs 3 and 4 at their full size
+def test_config3_ellipsoidal_full_size_against_closed_form(B):
+    """Config 3 itself (256^3, WENO7, outflow, CFL 0.2, 100 steps; reading Q14) against the closed form along
+    the three axes on |x_i| <= 4.5, where the zero-gradient boundary cannot have been felt (no oracle involved)."""
+    w = W.ellipsoidal()
+    h = B.from_workload(w)
+    h.step_cfl(w.cfl, w.nsteps)
+    t = h.time
+    assert 12.5 < t < 13.5 and h.status() == 0
+    ug = h.get_state().cpu().numpy()
+    n, c = 256, W.cell_centres(256, w.dx, -6.0)
+    mid = n // 2          # the cells just above the centre plane: coordinate +dx/2
+    sel = np.abs(c) <= 4.5
+    worst_e = worst_n = 0.0
+    for axis in range(3):
+        coords = [np.full(n, c[mid]), np.full(n, c[mid]), np.full(n, c[mid])]
+        coords[axis] = c
+        e, nn, vx, vy, vz = W.hubble_fields(coords[0], coords[1], coords[2], t, 12.0, 1.0, 1.0, b=W.ELLIPSOID_B)
+        exact = W.prim_to_cons(e, nn, vx, vy, vz)
+        line = [ug[:, mid, mid, :], ug[:, mid, :, mid], ug[:, :, mid, mid]][axis]
+        worst_e = max(worst_e, np.max(np.abs(line[0][sel] - exact[0][sel]) / exact[0][sel]))
+        worst_n = max(worst_n, np.max(np.abs(line[4][sel] - exact[4][sel])) / np.max(exact[4][sel]))
+    assert worst_e < 1e-6 and worst_n < 1e-4, (worst_e, worst_n)
+    h.close()
+
+
+def test_config4_lumpy_musta_full_size_conservation(B):
+    """Config 4 itself: 256^3 periodic, 40 hotspots at rest, MUSTA-FORCE K=2, CFL 0.2, 50 steps: the totals of
+    E, M and R are conserved (sum M starts at exactly 0 and must stay at rounding level)."""
+    w = W.lumpy()
+    assert w.n == (256, 256, 256) and w.scheme == W.MUSTA_FORCE
+    h = B.from_workload(w)
+    tot0 = [math.fsum(w.cons[c].ravel()) for c in range(5)]
+    assert tot0[1] == 0.0 and tot0[2] == 0.0 and tot0[3] == 0.0
+    h.step_cfl(w.cfl, w.nsteps)
+    u = h.get_state().cpu().numpy()
+    assert h.status() == 0 and np.all(np.isfinite(u))
+    tot1 = [math.fsum(u[c].ravel()) for c in range(5)]
+    assert np.max(np.abs(u[1:4])) > 1e-3                      # the hotspots are expanding
+    for a, b in zip(tot0, tot1):
+        assert abs(a - b) <= 1e-13 * tot0[0], (tot0, tot1)
+    h.close()
