@@ -466,3 +466,34 @@ def test_config4_lumpy_musta_full_size_conservation(B):
     for a, b in zip(tot0, tot1):
         assert abs(a - b) <= 1e-13 * tot0[0], (tot0, tot1)
     h.close()
+
+
+# ------------------------------------------------------------------ several events at once: one context per stream
+def test_two_contexts_on_two_streams_do_not_interfere(B):
+    """Event-by-event use: independent contexts on their own CUDA streams, launches interleaved from
+    the host, must give exactly what each gives alone."""
+    import torch
+    ws = [small_workload(W.WENO5, (45, 23, 70), seed=W.SEED), small_workload(W.MUSTA_FORCE, (45, 23, 70), seed=W.SEED + 1)]
+    alone = []
+    for w in ws:
+        h = B.from_workload(w)
+        h.step_cfl(0.2, 4)
+        alone.append(h.get_state().cpu())
+        h.close()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    hs = []
+    for w, st in zip(ws, streams):
+        with torch.cuda.stream(st):
+            hs.append(B.from_workload(w))       # bind() takes torch's current stream
+    for _ in range(4):
+        for h in hs:
+            h.step_cfl(0.2, 1)                  # asynchronous: the two streams overlap on the device
+    outs = []
+    for h, st in zip(hs, streams):
+        with torch.cuda.stream(st):
+            outs.append(h.get_state())
+    torch.cuda.synchronize()
+    for o, a, h in zip(outs, alone, hs):
+        assert torch.equal(o.cpu(), a)
+        assert h.status() == 0
+        h.close()
