@@ -300,10 +300,15 @@ def run_ours(args):
     if slab_mode:
         from paper_1604_03360_b200 import slab as S
         k0, k1 = S.split_planes(n, world)[rank]
-        host_in = torch.from_numpy(np.ascontiguousarray(w.cons[:, k0:k1])).to(tdt).pin_memory()
+        host_in = torch.from_numpy(np.ascontiguousarray(w.cons[:, k0:k1])).to(tdt)
     else:
-        host_in = torch.from_numpy(w.cons).to(tdt).pin_memory()
-    host_out = torch.empty_like(host_in).pin_memory()
+        host_in = torch.from_numpy(w.cons).to(tdt)
+    host_out = torch.empty_like(host_in)
+    pinned = True
+    try:
+        host_in, host_out = host_in.pin_memory(), host_out.pin_memory()
+    except RuntimeError:
+        pinned = False                 # many ranks on one host can exhaust lockable memory: pageable copies then
     h.set_state_host(host_in)          # warm the copy path
     advance(1)
     h.get_state_host(host_out)
@@ -320,7 +325,8 @@ def run_ours(args):
     e2e = {"value": aggregate_value(ncell, args.steps, 1 if slab_mode else world, e2e_s * 1e3), "unit": UNIT,
            "h2d_bytes_per_step": state_bytes / max(args.steps, 1),
            "d2h_bytes_per_step": state_bytes / max(args.steps, 1),
-           "job": "hydro_set_state_host (pinned) + %d steps + hydro_get_state_host; "
+           "pinned_host_memory": pinned,
+           "job": "hydro_set_state_host + %d steps + hydro_get_state_host; "
                   "state %d bytes each way per job and rank" % (args.steps, state_bytes),
            "finite": bool(torch.isfinite(host_out).all().item())}
     launches_per_step = r["launches"] / max(args.steps, 1)
