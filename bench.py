@@ -3,7 +3,7 @@
 BASELINE.json configs[4]: the 512^3 periodic lumpy state with 200 hotspots and blended velocities.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--scheme weno5|weno7|musta] [--precision f64|f32]
-                    [--n 512] [--no-variants] [--no-cpu-baseline] [--impl reference]
+                    [--grid 512] [--no-variants] [--no-cpu-baseline] [--impl reference]
 
 One "step" is one SSP-RK3 step of the whole grid with dt = CFL dx / max signal speed taken on the device
 (hydro_step_cfl, reading Q10): per stage the ghost fill, the x/z marching kernel and the y sweep, whose epilogue
@@ -406,7 +406,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scheme", default="weno5", choices=sorted(SCHEMES))
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
-    ap.add_argument("--n", type=int, default=512)
+    ap.add_argument("--grid", "--n", dest="n", type=int, default=512,
+                    help="cells per axis (use --grid under torchrun: its parser finds --n ambiguous)")
     ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--split-z", type=int, default=None, choices=[0, 1])
