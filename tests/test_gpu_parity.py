@@ -497,3 +497,27 @@ def test_two_contexts_on_two_streams_do_not_interfere(B):
         assert torch.equal(o.cpu(), a)
         assert h.status() == 0
         h.close()
+
+
+# ------------------------------------------------------------------ argument checking of the compute calls
+def test_compute_calls_reject_bad_arguments(B):
+    import ctypes
+    w = small_workload(W.WENO5, (20, 12, 9))
+    h = B.from_workload(w)
+    lib = B.lib
+    assert lib.hydro_step(h._h, -1.0, 1) == B.EINVAL and b"dt" in lib.hydro_last_error(h._h)
+    assert lib.hydro_step_cfl(h._h, 0.0, 1) == B.EINVAL
+    assert lib.hydro_step_stage(h._h, 0.01, 3) == B.EINVAL
+    assert lib.hydro_get_zhalo(h._h, 5, 0, ctypes.c_void_p(16)) == B.EINVAL
+    assert lib.hydro_set_state(h._h, None) == B.EINVAL
+    assert lib.hydro_set_option(h._h, b"bc_x", 3.0) == B.EINVAL        # external ghosts exist for z only
+    assert lib.hydro_set_option(h._h, b"precision", 1.0) == B.EINVAL   # after the workspace is bound
+    # nothing of the above touched the state
+    assert np.array_equal(h.get_state().cpu().numpy(), w.cons)
+    h.close()
+    # the z-halo calls need an active z axis
+    w2 = W.Workload("2d", (24, 30, 1), 0.05, (0, 0, 0), W.WENO5, (W.BC_OUTFLOW,) * 3, W.random_state((1, 30, 24), seed=2, vmax=0.3))
+    h2 = B.from_workload(w2)
+    assert h2.zhalo_elems() == 0
+    assert lib.hydro_get_zhalo(h2._h, 0, 0, ctypes.c_void_p(16)) == B.EINVAL
+    h2.close()
