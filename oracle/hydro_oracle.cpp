@@ -186,14 +186,34 @@ T minmod(T a, T b) {
     return (a > 0 ? (T)1 : (T)-1) * std::fmin(std::fabs(a), std::fabs(b));
 }
 
+// O6'. The other slope limiters ("a variety of slope limiting methods"), as limited
+// slopes of the backward difference a = u_i - u_{i-1} and the forward difference b = u_{i+1} - u_i.  All vanish
+// unless a and b have the same sign (ab > 0), are symmetric in (a, b), homogeneous of degree one, equal a when
+// a = b, and stay inside Sweby's second-order TVD region |slope| <= 2 min(|a|, |b|):
+//   0 minmod     sign(a) min(|a|, |b|)
+//   1 van Leer   2ab / (a + b)                                  (harmonic mean)
+//   2 MC         sign(a) min(2|a|, 2|b|, |a + b| / 2)           (monotonised central)
+//   3 superbee   sign(a) max(min(2|a|, |b|), min(|a|, 2|b|))
+enum { LIM_MINMOD = 0, LIM_VANLEER = 1, LIM_MC = 2, LIM_SUPERBEE = 3 };
+template <class T>
+T limited_slope(int lim, T a, T b) {
+    if (lim == LIM_MINMOD) return minmod(a, b);
+    if (a * b <= (T)0) return (T)0;
+    const T sg = a > 0 ? (T)1 : (T)-1;
+    const T aa = std::fabs(a), ab = std::fabs(b);
+    if (lim == LIM_VANLEER) return (T)2 * a * b / (a + b);
+    if (lim == LIM_MC) return sg * std::fmin(std::fmin((T)2 * aa, (T)2 * ab), std::fabs(a + b) / (T)2);
+    return sg * std::fmax(std::fmin((T)2 * aa, ab), std::fmin(aa, (T)2 * ab));
+}
+
 // O7. MUSTA-FORCE flux, K stages.
 //   cells[0..3] = u_{i-1}, u_i, u_{i+1}, u_{i+2}.  tau = C/S, S = max(a_d(Q_L), a_d(Q_R)) per stage.
 template <class T>
-void musta_force_flux(const T cells[4][NF], int d, int K, T C, T fstar[NF], int* flag) {
+void musta_force_flux(const T cells[4][NF], int d, int K, T C, T fstar[NF], int* flag, int lim = LIM_MINMOD) {
     T QL[NF], QR[NF];
     for (int c = 0; c < NF; ++c) {
-        const T di = minmod(cells[1][c] - cells[0][c], cells[2][c] - cells[1][c]);
-        const T dip = minmod(cells[2][c] - cells[1][c], cells[3][c] - cells[2][c]);
+        const T di = limited_slope(lim, cells[1][c] - cells[0][c], cells[2][c] - cells[1][c]);
+        const T dip = limited_slope(lim, cells[2][c] - cells[1][c], cells[3][c] - cells[2][c]);
         QL[c] = cells[1][c] + di / (T)2;
         QR[c] = cells[2][c] - dip / (T)2;
     }
@@ -229,6 +249,7 @@ struct Solver {
     int bc[3] = {BC_OUTFLOW, BC_OUTFLOW, BC_OUTFLOW};
     double eps = 1e-6, musta_cfl = 0.9, t = 0.0;
     int musta_stages = 2;
+    int limiter = LIM_MINMOD;
     double origin[3] = {0, 0, 0};
     double hub_t0 = 1, hub_e0 = 1, hub_n0 = 1, hub_b[3] = {0, 0, 0};
     int flag = 0;
@@ -324,7 +345,7 @@ struct Solver {
                 jx[a] += m - 1;
                 load(pad, jx[0], jx[1], jx[2], cells[m]);
             }
-            musta_force_flux<T>(cells, a, musta_stages, (T)musta_cfl, fh, &flag);
+            musta_force_flux<T>(cells, a, musta_stages, (T)musta_cfl, fh, &flag, limiter);
         } else {
             T cells[8][NF], F[8][NF], sp[8];
             for (int m = 0; m < 2 * r; ++m) {
@@ -506,14 +527,14 @@ int oracle_set_option(oracle_ctx* c, const char* key, double v) {
             auto* S = new Solver<float>(c->nx, c->ny, c->nz, c->dx, c->scheme);
             auto* D = c->d;
             for (int a = 0; a < 3; ++a) { S->bc[a] = D->bc[a]; S->origin[a] = D->origin[a]; S->hub_b[a] = D->hub_b[a]; }
-            S->eps = D->eps; S->musta_cfl = D->musta_cfl; S->musta_stages = D->musta_stages; S->t = D->t;
+            S->eps = D->eps; S->musta_cfl = D->musta_cfl; S->musta_stages = D->musta_stages; S->t = D->t; S->limiter = D->limiter;
             S->hub_t0 = D->hub_t0; S->hub_e0 = D->hub_e0; S->hub_n0 = D->hub_n0;
             delete c->d; c->d = nullptr; c->f = S;
         } else {
             auto* S = new Solver<double>(c->nx, c->ny, c->nz, c->dx, c->scheme);
             auto* D = c->f;
             for (int a = 0; a < 3; ++a) { S->bc[a] = D->bc[a]; S->origin[a] = D->origin[a]; S->hub_b[a] = D->hub_b[a]; }
-            S->eps = D->eps; S->musta_cfl = D->musta_cfl; S->musta_stages = D->musta_stages; S->t = D->t;
+            S->eps = D->eps; S->musta_cfl = D->musta_cfl; S->musta_stages = D->musta_stages; S->t = D->t; S->limiter = D->limiter;
             S->hub_t0 = D->hub_t0; S->hub_e0 = D->hub_e0; S->hub_n0 = D->hub_n0;
             delete c->f; c->f = nullptr; c->d = S;
         }
@@ -527,6 +548,7 @@ int oracle_set_option(oracle_ctx* c, const char* key, double v) {
             if (b < 0 || b > 2) rc = EINVAL_; else S->bc[k[3] - 'x'] = b;
         } else if (k == "musta_stages") { if (v < 1) rc = EINVAL_; else S->musta_stages = (int)v; }
         else if (k == "musta_cfl") { if (!(v > 0)) rc = EINVAL_; else S->musta_cfl = v; }
+        else if (k == "limiter") { if (v < 0 || v > 3) rc = EINVAL_; else S->limiter = (int)v; }
         else if (k == "weno_eps") { if (!(v > 0)) rc = EINVAL_; else S->eps = v; }
         else if (k == "t") S->t = v;
         else if (k == "x0") S->origin[0] = v;
@@ -605,6 +627,14 @@ void oracle_phys_flux(const double u[5], int d, double F[5]) {
 double oracle_weno5(const double f[5], double eps) { return weno5<double>(f, eps); }
 double oracle_weno7(const double f[7], double eps) { return weno7<double>(f, eps); }
 double oracle_minmod(double a, double b) { return minmod<double>(a, b); }
+double oracle_limited_slope(int lim, double a, double b) { return limited_slope<double>(lim, a, b); }
+int oracle_musta_force_flux_lim(const double* cells, int d, int K, double C, int lim, double fstar[5]) {
+    double cc[4][NF];
+    std::memcpy(cc, cells, sizeof(cc));
+    int flag = 0;
+    musta_force_flux<double>(cc, d, K, C, fstar, &flag, lim);
+    return flag;
+}
 // cells: [2r][5] row-major, u_{i-r+1}..u_{i+r}; r = 3 (WENO5) or 4 (WENO7)
 int oracle_llf_weno_flux(int r, const double* cells, int d, double eps, double fhat[5]) {
     if (r != 3 && r != 4) return EINVAL_;

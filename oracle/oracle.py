@@ -58,6 +58,9 @@ def lib():
         L.oracle_weno7.restype = dbl
         L.oracle_minmod.argtypes = [dbl, dbl]
         L.oracle_minmod.restype = dbl
+        L.oracle_limited_slope.argtypes = [i32, dbl, dbl]
+        L.oracle_limited_slope.restype = dbl
+        L.oracle_musta_force_flux_lim.argtypes = [pd, i32, i32, dbl, i32, pd]
         L.oracle_llf_weno_flux.argtypes = [i32, pd, i32, dbl, pd]
         L.oracle_musta_force_flux.argtypes = [pd, i32, i32, dbl, pd]
         _lib = L
@@ -117,10 +120,17 @@ def llf_weno_flux(r, cells, d, eps=1e-6):
     return out
 
 
-def musta_force_flux(cells, d, K=2, C=0.9):
+def limited_slope(lim, a, b):
+    return lib().oracle_limited_slope(int(lim), a, b)
+
+
+def musta_force_flux(cells, d, K=2, C=0.9, limiter=0):
     cells = _arr(cells, 20)
     out = np.empty(5)
-    lib().oracle_musta_force_flux(_pd(cells), d, K, C, _pd(out))
+    if limiter:
+        lib().oracle_musta_force_flux_lim(_pd(cells), d, K, C, int(limiter), _pd(out))
+    else:
+        lib().oracle_musta_force_flux(_pd(cells), d, K, C, _pd(out))
     return out
 
 
