@@ -67,6 +67,8 @@ int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme)
  *   "weno_eps"      epsilon of the WENO weights (default 1e-6, reading Q5)
  *   "musta_stages"  K of MUSTA-FORCE (default 2, reading Q8);  "musta_cfl" its local Courant number
  *                   (default 0.9, reading Q7)
+ *   "limiter"       MUSCL slope limiter of MUSTA-FORCE: 0 minmod (default, reading Q6), 1 van Leer, 2 MC,
+ *                   3 superbee ("a variety of slope limiting methods")
  *   "t"             current time (used by the analytic Hubble ghost fill)
  *   "x0|y0|z0"      coordinate of the low face of the domain on each axis
  *   "hubble_t0|hubble_e0|hubble_n0|hubble_bx|hubble_by|hubble_bz"  parameters of the closed-form

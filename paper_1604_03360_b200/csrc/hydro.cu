@@ -28,6 +28,7 @@ struct hydro_ctx {
     int bc[3] = {HYDRO_BC_OUTFLOW, HYDRO_BC_OUTFLOW, HYDRO_BC_OUTFLOW};
     double eps = 1e-6, musta_cfl = 0.9;
     int musta_stages = 2;
+    int limiter = 0;
     double t_host = 0.0;  // value to push into the control block at bind / set_option("t")
     HubbleParams H;
     cudaStream_t stream = nullptr;
@@ -161,6 +162,7 @@ StageArgs stage_args(const hydro_ctx* c, double ca, double cb, int mode) {
     A.eps = c->eps;
     A.musta_K = c->musta_stages;
     A.musta_C = c->musta_cfl;
+    A.limiter = c->limiter;
     A.epi_max = 0;
     return A;
 }
@@ -369,6 +371,9 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
     } else if (k == "musta_stages") {
         if (v < 1) return fail(c, HYDRO_EINVAL, "musta_stages < 1");
         c->musta_stages = (int)v;
+    } else if (k == "limiter") {
+        if (v < 0 || v > 3) return fail(c, HYDRO_EINVAL, "limiter must be 0..3");
+        c->limiter = (int)v;
     } else if (k == "musta_cfl") {
         if (!(v > 0)) return fail(c, HYDRO_EINVAL, "musta_cfl <= 0");
         c->musta_cfl = v;

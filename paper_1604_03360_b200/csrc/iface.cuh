@@ -107,6 +107,21 @@ __device__ __forceinline__ double minmod<double>(double a, double b) {
 }
 #endif
 
+// The other limiters ("a variety of slope limiting methods", a7'): limited slope
+// of the backward difference a and the forward difference b.  1 van Leer 2ab/(a+b); 2 MC
+// sign(a) min(2|a|, 2|b|, |a+b|/2); 3 superbee sign(a) max(min(2|a|,|b|), min(|a|,2|b|)); all 0 unless ab > 0.
+template <class T>
+HD T limited_slope(int lim, T a, T b) {
+    if (lim == 0) return minmod(a, b);
+    if (a * b <= (T)0) return (T)0;
+    const T aa = tabs(a), ab = tabs(b);
+    if (lim == 1) return (T)2 * a * b * fast_rcp(aa + ab) * (a > (T)0 ? (T)1 : (T)-1);
+    T m;
+    if (lim == 2) m = tmin(tmin((T)2 * aa, (T)2 * ab), (T)0.5 * (aa + ab));
+    else m = tmax(tmin((T)2 * aa, ab), tmin(aa, (T)2 * ab));
+    return a > (T)0 ? m : -m;
+}
+
 // physical flux of a conserved state along DIR plus its signal speed (every evaluation needs its own
 // con2prim, O7).  Q is modified only if the Q16 clamp fires.
 template <class T, int DIR>
@@ -134,15 +149,17 @@ HD void flux_only(const T Q[NF], T F[NF], int& flag) {
 // acc.u(c, k), k = 0..3 for cells i-1 .. i+2.  K stages, local Courant number C (tau = C/S).
 // KS > 0: the number of stages is the compile-time constant KS (fully unrolled, the default K = 2 takes this
 // path); KS = 0: run-time K.
-template <class T, int DIR, int KS, class Acc>
-HD void musta_force_stages(const Acc& acc, int K, T C, T fh[NF], int& flag) {
+// LIMS >= 0: the limiter is the compile-time constant LIMS (the default minmod takes this path at full speed: a
+// run-time limiter inside the interface code cost 17 % of the MUSTA step); LIMS < 0: run-time `lim`.
+template <class T, int DIR, int KS, int LIMS, class Acc>
+HD void musta_force_stages(const Acc& acc, int K, T C, int lim, T fh[NF], int& flag) {
     T QL[NF], QR[NF];
 #pragma unroll
     for (int c = 0; c < NF; ++c) {
         const T u0 = acc.u(c, 0), u1 = acc.u(c, 1), u2 = acc.u(c, 2), u3 = acc.u(c, 3);
         const T dm = u1 - u0, d0 = u2 - u1, dp = u3 - u2;
-        QL[c] = tfma((T)0.5, minmod(dm, d0), u1);
-        QR[c] = tfma((T)-0.5, minmod(d0, dp), u2);
+        QL[c] = tfma((T)0.5, LIMS == 0 ? minmod(dm, d0) : limited_slope(lim, dm, d0), u1);
+        QR[c] = tfma((T)-0.5, LIMS == 0 ? minmod(d0, dp) : limited_slope(lim, d0, dp), u2);
     }
     const T invC = (T)1 / C;
     const int nst = KS > 0 ? KS : K;
@@ -170,9 +187,9 @@ HD void musta_force_stages(const Acc& acc, int K, T C, T fh[NF], int& flag) {
 }
 
 template <class T, int DIR, class Acc>
-HD void musta_force_iface(const Acc& acc, int K, T C, T fh[NF], int& flag) {
-    if (K == 2) musta_force_stages<T, DIR, 2>(acc, K, C, fh, flag);
-    else musta_force_stages<T, DIR, 0>(acc, K, C, fh, flag);
+HD void musta_force_iface(const Acc& acc, int K, T C, int lim, T fh[NF], int& flag) {
+    if (K == 2 && lim == 0) musta_force_stages<T, DIR, 2, 0>(acc, K, C, lim, fh, flag);
+    else musta_force_stages<T, DIR, 0, -1>(acc, K, C, lim, fh, flag);
 }
 
 }  // namespace hydro

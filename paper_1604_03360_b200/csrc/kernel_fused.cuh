@@ -99,7 +99,7 @@ struct ZWindow {
 template <class T, int SCHEME, int DIR, class Acc>
 __device__ __forceinline__ void iface_from(const Acc& acc, const StageArgs& A, T fh[NF], int& flag) {
     constexpr int R = SCHEME == 0 ? 3 : (SCHEME == 1 ? 4 : 2);
-    if constexpr (SCHEME == 2) musta_force_iface<T, DIR>(acc, A.musta_K, (T)A.musta_C, fh, flag);
+    if constexpr (SCHEME == 2) musta_force_iface<T, DIR>(acc, A.musta_K, (T)A.musta_C, A.limiter, fh, flag);
     else llf_weno_iface<T, R, DIR>(acc, (T)A.eps, fh);
 }
 

@@ -521,3 +521,26 @@ def test_compute_calls_reject_bad_arguments(B):
     assert h2.zhalo_elems() == 0
     assert lib.hydro_get_zhalo(h2._h, 0, 0, ctypes.c_void_p(16)) == B.EINVAL
     h2.close()
+
+
+# ------------------------------------------------------------------ the other slope limiters
+@pytest.mark.parametrize("limiter", [1, 2, 3])
+def test_musta_with_other_limiters_matches_oracle(B, oracle, limiter):
+    w = small_workload(W.MUSTA_FORCE, (45, 23, 70))
+    w.options = {"limiter": limiter}
+    o = oracle.from_workload(w)
+    h = B.from_workload(w)
+    Lo = o.eval_L(w.cons)
+    Lg = h.eval_L(to_dev(B, w.cons)).cpu().numpy()
+    assert reldiff(Lg, Lo, scale=np.max(np.abs(w.cons[0])) / w.dx) <= TOL_STAGE
+    # and it is not minmod's operator
+    w0 = small_workload(W.MUSTA_FORCE, (45, 23, 70))
+    L0 = oracle.from_workload(w0).eval_L(w0.cons)
+    assert np.max(np.abs(L0 - Lo)) > 1e-3 * np.max(np.abs(Lo))
+    w.nsteps = 20
+    dts = oracle.run(o, w)
+    for dt in dts:
+        h.step(dt, 1)
+    assert reldiff(h.get_state().cpu().numpy(), o.get_state()) <= 1e-10
+    assert h.status() == 0
+    h.close()
