@@ -46,8 +46,48 @@ struct Prim {
     T e, p, n, v[3];
 };
 
+// Equation of state.  kind 0: p = e/3 (reading Q2, the default everywhere).  kind 1: p = p0, a
+// constant: the closure for which the anisotropic free-streaming flow of the paper's ref. [8]
+// is an exact solution.
+struct Eos {
+    int kind;
+    double p0;
+    Eos() : kind(0), p0(0.0) {}
+};
+
+// O1'. p = p0 constant: from E + p0 = (e + p0) gamma^2 and M = (e + p0) gamma^2 v:
+//   v_i = M_i / (E + p0),  e = E - M^2 / (E + p0),  p = p0,  n = R sqrt(1 - v^2).
+// Clamps in the spirit of Q16: E + p0 >= 1e-300 and |M| <= (1 - 1e-12)(E + p0), raising the flag.
 template <class T>
-Prim<T> con2prim(const T u[NF], int* flag) {
+Prim<T> con2prim_pconst(const T u[NF], int* flag, T p0) {
+    T H = u[0] + p0, M[3] = {u[1], u[2], u[3]}, R = u[4];
+    if (!(H >= (T)1e-300)) {
+        H = (T)1e-300;
+        if (flag) *flag = 1;
+    }
+    T Mabs = std::sqrt(M[0] * M[0] + M[1] * M[1] + M[2] * M[2]);
+    const T lim = ((T)1 - (T)1e-12) * H;
+    if (Mabs > lim) {
+        const T sc = lim / Mabs;
+        for (int i = 0; i < 3; ++i) M[i] *= sc;
+        Mabs = lim;
+        if (flag) *flag = 1;
+    }
+    Prim<T> w;
+    T v2 = 0;
+    for (int i = 0; i < 3; ++i) {
+        w.v[i] = M[i] / H;
+        v2 += w.v[i] * w.v[i];
+    }
+    w.e = (H - p0) - Mabs * Mabs / H;
+    w.p = p0;
+    w.n = R * std::sqrt((T)1 - v2);
+    return w;
+}
+
+template <class T>
+Prim<T> con2prim(const T u[NF], int* flag, const Eos& eos = Eos()) {
+    if (eos.kind == 1) return con2prim_pconst<T>(u, flag, (T)eos.p0);
     T E = u[0], M[3] = {u[1], u[2], u[3]}, R = u[4];
     if (!(E >= (T)1e-300)) {
         E = (T)1e-300;
@@ -77,8 +117,10 @@ Prim<T> con2prim(const T u[NF], int* flag) {
 // ------------------------------------------------------------------------------------------
 // O2. directional characteristic speed, c_s^2 = 1/3:
 //   a_d = ( |v_d|(1-cs2) + cs sqrt((1-v^2)(1 - v_d^2 - (v^2 - v_d^2) cs2)) ) / (1 - v^2 cs2)
+// p = p0 constant: c_s = 0, all five characteristic speeds of direction d equal v_d, so a_d = |v_d|.
 template <class T>
-T signal_speed(const T v[3], int d) {
+T signal_speed(const T v[3], int d, const Eos& eos = Eos()) {
+    if (eos.kind == 1) return std::fabs(v[d]);
     const T cs2 = (T)1 / (T)3;
     const T cs = std::sqrt(cs2);
     const T v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
@@ -168,12 +210,12 @@ void llf_weno_split(int r, const T cells[][NF], const T F[][NF], const T a[], T 
 
 // the same, starting from the conserved cells only (a2, a3, a5 done per cell first)
 template <class T>
-void llf_weno_flux(int r, const T cells[][NF], int d, T eps, T fhat[NF], int* flag) {
+void llf_weno_flux(int r, const T cells[][NF], int d, T eps, T fhat[NF], int* flag, const Eos& eos = Eos()) {
     T F[8][NF], a[8];
     for (int k = 0; k < 2 * r; ++k) {
-        const Prim<T> w = con2prim(cells[k], flag);
+        const Prim<T> w = con2prim(cells[k], flag, eos);
         phys_flux(cells[k], w, d, F[k]);
-        a[k] = signal_speed(w.v, d);
+        a[k] = signal_speed(w.v, d, eos);
     }
     llf_weno_split(r, cells, F, a, eps, fhat);
 }
@@ -209,7 +251,8 @@ T limited_slope(int lim, T a, T b) {
 // O7. MUSTA-FORCE flux, K stages.
 //   cells[0..3] = u_{i-1}, u_i, u_{i+1}, u_{i+2}.  tau = C/S, S = max(a_d(Q_L), a_d(Q_R)) per stage.
 template <class T>
-void musta_force_flux(const T cells[4][NF], int d, int K, T C, T fstar[NF], int* flag, int lim = LIM_MINMOD) {
+void musta_force_flux(const T cells[4][NF], int d, int K, T C, T fstar[NF], int* flag, int lim = LIM_MINMOD,
+                      const Eos& eos = Eos()) {
     T QL[NF], QR[NF];
     for (int c = 0; c < NF; ++c) {
         const T di = limited_slope(lim, cells[1][c] - cells[0][c], cells[2][c] - cells[1][c]);
@@ -218,14 +261,14 @@ void musta_force_flux(const T cells[4][NF], int d, int K, T C, T fstar[NF], int*
         QR[c] = cells[2][c] - dip / (T)2;
     }
     for (int stage = 1;; ++stage) {
-        const Prim<T> wl = con2prim(QL, flag), wr = con2prim(QR, flag);
+        const Prim<T> wl = con2prim(QL, flag, eos), wr = con2prim(QR, flag, eos);
         T FL[NF], FR[NF], QM[NF], FM[NF];
         phys_flux(QL, wl, d, FL);
         phys_flux(QR, wr, d, FR);
-        const T S = std::fmax(signal_speed(wl.v, d), signal_speed(wr.v, d));
+        const T S = std::fmax(signal_speed(wl.v, d, eos), signal_speed(wr.v, d, eos));
         const T tau = C / S;
         for (int c = 0; c < NF; ++c) QM[c] = (QL[c] + QR[c]) / (T)2 - tau * (FR[c] - FL[c]) / (T)2;
-        const Prim<T> wm = con2prim(QM, flag);
+        const Prim<T> wm = con2prim(QM, flag, eos);
         phys_flux(QM, wm, d, FM);
         for (int c = 0; c < NF; ++c)
             fstar[c] = (FL[c] + (T)2 * FM[c] + FR[c] - (QR[c] - QL[c]) / tau) / (T)4;
@@ -250,6 +293,7 @@ struct Solver {
     double eps = 1e-6, musta_cfl = 0.9, t = 0.0;
     int musta_stages = 2;
     int limiter = LIM_MINMOD;
+    Eos eos;
     double origin[3] = {0, 0, 0};
     double hub_t0 = 1, hub_e0 = 1, hub_n0 = 1, hub_b[3] = {0, 0, 0};
     int flag = 0;
@@ -345,7 +389,7 @@ struct Solver {
                 jx[a] += m - 1;
                 load(pad, jx[0], jx[1], jx[2], cells[m]);
             }
-            musta_force_flux<T>(cells, a, musta_stages, (T)musta_cfl, fh, &flag, limiter);
+            musta_force_flux<T>(cells, a, musta_stages, (T)musta_cfl, fh, &flag, limiter, eos);
         } else {
             T cells[8][NF], F[8][NF], sp[8];
             for (int m = 0; m < 2 * r; ++m) {
@@ -354,7 +398,7 @@ struct Solver {
                 load(pad, jx[0], jx[1], jx[2], cells[m]);
                 const Prim<T>& w = prim[pidx(jx[0], jx[1], jx[2])];
                 phys_flux(cells[m], w, a, F[m]);
-                sp[m] = signal_speed(w.v, a);
+                sp[m] = signal_speed(w.v, a, eos);
             }
             llf_weno_split<T>(r, cells, F, sp, (T)eps, fh);
         }
@@ -378,7 +422,7 @@ struct Solver {
                         if (out > 1) continue;
                         T c[NF];
                         load(pad, i, j, k, c);
-                        prim[pidx(i, j, k)] = con2prim(c, &flag);
+                        prim[pidx(i, j, k)] = con2prim(c, &flag, eos);
                     }
         }
         for (int a = 0; a < 3; ++a) {
@@ -471,9 +515,9 @@ struct Solver {
                 for (int i = 0; i < n[0]; ++i) {
                     T c[NF];
                     load(u, i, j, k, c);
-                    const Prim<T> w = con2prim(c, &flag);
+                    const Prim<T> w = con2prim(c, &flag, eos);
                     for (int a = 0; a < 3; ++a)
-                        if (g[a] > 0) m = std::fmax(m, (double)signal_speed(w.v, a));
+                        if (g[a] > 0) m = std::fmax(m, (double)signal_speed(w.v, a, eos));
                 }
         return m;
     }
@@ -527,14 +571,14 @@ int oracle_set_option(oracle_ctx* c, const char* key, double v) {
             auto* S = new Solver<float>(c->nx, c->ny, c->nz, c->dx, c->scheme);
             auto* D = c->d;
             for (int a = 0; a < 3; ++a) { S->bc[a] = D->bc[a]; S->origin[a] = D->origin[a]; S->hub_b[a] = D->hub_b[a]; }
-            S->eps = D->eps; S->musta_cfl = D->musta_cfl; S->musta_stages = D->musta_stages; S->t = D->t; S->limiter = D->limiter;
+            S->eps = D->eps; S->musta_cfl = D->musta_cfl; S->musta_stages = D->musta_stages; S->t = D->t; S->limiter = D->limiter; S->eos = D->eos;
             S->hub_t0 = D->hub_t0; S->hub_e0 = D->hub_e0; S->hub_n0 = D->hub_n0;
             delete c->d; c->d = nullptr; c->f = S;
         } else {
             auto* S = new Solver<double>(c->nx, c->ny, c->nz, c->dx, c->scheme);
             auto* D = c->f;
             for (int a = 0; a < 3; ++a) { S->bc[a] = D->bc[a]; S->origin[a] = D->origin[a]; S->hub_b[a] = D->hub_b[a]; }
-            S->eps = D->eps; S->musta_cfl = D->musta_cfl; S->musta_stages = D->musta_stages; S->t = D->t; S->limiter = D->limiter;
+            S->eps = D->eps; S->musta_cfl = D->musta_cfl; S->musta_stages = D->musta_stages; S->t = D->t; S->limiter = D->limiter; S->eos = D->eos;
             S->hub_t0 = D->hub_t0; S->hub_e0 = D->hub_e0; S->hub_n0 = D->hub_n0;
             delete c->f; c->f = nullptr; c->d = S;
         }
@@ -548,6 +592,8 @@ int oracle_set_option(oracle_ctx* c, const char* key, double v) {
             if (b < 0 || b > 2) rc = EINVAL_; else S->bc[k[3] - 'x'] = b;
         } else if (k == "musta_stages") { if (v < 1) rc = EINVAL_; else S->musta_stages = (int)v; }
         else if (k == "musta_cfl") { if (!(v > 0)) rc = EINVAL_; else S->musta_cfl = v; }
+        else if (k == "eos") { if (v != 0 && v != 1) rc = EINVAL_; else S->eos.kind = (int)v; }
+        else if (k == "eos_p0") { if (!(v >= 0)) rc = EINVAL_; else S->eos.p0 = v; }
         else if (k == "limiter") { if (v < 0 || v > 3) rc = EINVAL_; else S->limiter = (int)v; }
         else if (k == "weno_eps") { if (!(v > 0)) rc = EINVAL_; else S->eps = v; }
         else if (k == "t") S->t = v;
@@ -627,6 +673,19 @@ void oracle_phys_flux(const double u[5], int d, double F[5]) {
 double oracle_weno5(const double f[5], double eps) { return weno5<double>(f, eps); }
 double oracle_weno7(const double f[7], double eps) { return weno7<double>(f, eps); }
 double oracle_minmod(double a, double b) { return minmod<double>(a, b); }
+// the pointwise pieces with an equation of state (eos 0: p = e/3, 1: p = p0)
+int oracle_con2prim_eos(const double u[5], int eos, double p0, double prim_out[6]) {
+    Eos q; q.kind = eos; q.p0 = p0;
+    int flag = 0;
+    const Prim<double> w = con2prim<double>(u, &flag, q);
+    prim_out[0] = w.e; prim_out[1] = w.p; prim_out[2] = w.n;
+    prim_out[3] = w.v[0]; prim_out[4] = w.v[1]; prim_out[5] = w.v[2];
+    return flag;
+}
+double oracle_signal_speed_eos(const double v[3], int d, int eos, double p0) {
+    Eos q; q.kind = eos; q.p0 = p0;
+    return signal_speed<double>(v, d, q);
+}
 double oracle_limited_slope(int lim, double a, double b) { return limited_slope<double>(lim, a, b); }
 int oracle_musta_force_flux_lim(const double* cells, int d, int K, double C, int lim, double fstar[5]) {
     double cc[4][NF];

@@ -58,6 +58,9 @@ def lib():
         L.oracle_weno7.restype = dbl
         L.oracle_minmod.argtypes = [dbl, dbl]
         L.oracle_minmod.restype = dbl
+        L.oracle_con2prim_eos.argtypes = [pd, i32, dbl, pd]
+        L.oracle_signal_speed_eos.argtypes = [pd, i32, i32, dbl]
+        L.oracle_signal_speed_eos.restype = dbl
         L.oracle_limited_slope.argtypes = [i32, dbl, dbl]
         L.oracle_limited_slope.restype = dbl
         L.oracle_musta_force_flux_lim.argtypes = [pd, i32, i32, dbl, i32, pd]
@@ -87,9 +90,19 @@ def con2prim(u):
     return out, flag
 
 
-def signal_speed(v, d):
+def signal_speed(v, d, eos=0, p0=0.0):
     v = _arr(v, 3)
+    if eos:
+        return lib().oracle_signal_speed_eos(_pd(v), d, int(eos), float(p0))
     return lib().oracle_signal_speed(_pd(v), d)
+
+
+def con2prim_eos(u, eos, p0):
+    """u -> (e, p, n, vx, vy, vz), flag for the equation of state `eos` (0: p = e/3, 1: p = p0)."""
+    u = _arr(u, 5)
+    out = np.empty(6)
+    flag = lib().oracle_con2prim_eos(_pd(u), int(eos), float(p0), _pd(out))
+    return out, flag
 
 
 def phys_flux(u, d):

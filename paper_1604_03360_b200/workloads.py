@@ -54,6 +54,21 @@ def prim_to_cons(e, n, vx, vy, vz):
     return out
 
 
+def prim_to_cons_p0(e, n, vx, vy, vz, p0):
+    """The same definition with the constant-pressure closure p = p0."""
+    e = np.asarray(e, dtype=np.float64)
+    v2 = vx * vx + vy * vy + vz * vz
+    g2 = 1.0 / (1.0 - v2)
+    w = (e + p0) * g2
+    out = np.empty((5,) + e.shape, dtype=np.float64)
+    out[0] = w - p0
+    out[1] = w * vx
+    out[2] = w * vy
+    out[3] = w * vz
+    out[4] = n * np.sqrt(g2)
+    return out
+
+
 def cell_centres(n, dx, origin):
     return origin + (np.arange(n, dtype=np.float64) + 0.5) * dx
 
@@ -129,6 +144,46 @@ def ellipsoidal(n=256, half_width=6.0, t0=12.0, scheme=WENO7, nsteps=100, cfl=0.
             "hubble_bx": ELLIPSOID_B[0], "hubble_by": ELLIPSOID_B[1], "hubble_bz": ELLIPSOID_B[2]}
     return Workload("ellipsoidal", (n, n, n), dx, (-half_width,) * 3, scheme,
                     (bc,) * 3, cons, t0, cfl=cfl, nsteps=nsteps, options=opts)
+
+
+# ---------------------------------------------------------------- p = const: anisotropic free streaming (ref. [8])
+FREE_T = (2.0, 2.6, 3.4)
+
+
+def free_streaming_cons(x, y, z, t, p0=1.0, Q0=6.0, R0=1.0, T=FREE_T, axes=(True, True, True)):
+    """Exact solution for the closure p = p0 (the anisotropic flow of the paper's ref. [8],
+    v_i = x_i / (t + T_i), is exact for constant pressure).  Every fluid element moves with constant velocity
+    xi_i = x_i / (t + T_i), so Q = E + p0 = (e + p0) gamma^2 and R = n gamma obey the continuity equation, whose
+    solution along those straight lines is  Q = G(xi) / J(t),  R = H(xi) / J(t),  J = prod_i (t + T_i) / T_i  over
+    the flagged axes; G = Q0 exp(-|xi|^2 / 2), H = R0 exp(-|xi|^2).  Returns the conserved variables
+    E = Q - p0, M_i = Q xi_i, R (broadcast arrays)."""
+    coords = (x, y, z)
+    zero = 0.0 * (x + y + z)
+    xi, J, xi2 = [], 1.0, zero
+    for c, Ti, a in zip(coords, T, axes):
+        if a:
+            xi.append(c / (t + Ti) + zero)
+            J = J * (t + Ti) / Ti
+            xi2 = xi2 + (c / (t + Ti)) ** 2
+        else:
+            xi.append(zero)
+    Q = Q0 * np.exp(-0.5 * xi2) / J
+    R = R0 * np.exp(-xi2) / J
+    out = np.empty((5,) + np.shape(zero), dtype=np.float64)
+    out[0] = Q - p0
+    out[1], out[2], out[3] = Q * xi[0], Q * xi[1], Q * xi[2]
+    out[4] = R
+    return out
+
+
+def free_streaming(n=48, half_width=1.0, scheme=WENO5, nsteps=40, cfl=0.2, p0=1.0):
+    """3-D free-streaming workload for the p = p0 closure on [-L, L]^3 from t = 0, zero-gradient outflow (every
+    characteristic speed is v_d, pointing outward at all six faces)."""
+    dx = 2.0 * half_width / n
+    c = cell_centres(n, dx, -half_width)
+    cons = free_streaming_cons(c[None, None, :], c[None, :, None], c[:, None, None], 0.0, p0=p0)
+    return Workload("free_streaming", (n, n, n), dx, (-half_width,) * 3, scheme, (BC_OUTFLOW,) * 3, cons, 0.0,
+                    cfl=cfl, nsteps=nsteps, options={"eos": 1, "eos_p0": p0})
 
 
 # ---------------------------------------------------------------- configs 4, 5
