@@ -67,6 +67,9 @@ int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme)
  *   "weno_eps"      epsilon of the WENO weights (default 1e-6, reading Q5)
  *   "musta_stages"  K of MUSTA-FORCE (default 2, reading Q8);  "musta_cfl" its local Courant number
  *                   (default 0.9, reading Q7)
+ *   "eos", "eos_p0" equation of state: 0 (default) p = e/3 (reading Q2); 1 p = eos_p0, a constant (the closure for
+ *                   which the free-streaming flow of the paper's ref. [8] is exact, reading Q14); the
+ *                   characteristic speeds are then all v_d
  *   "limiter"       MUSCL slope limiter of MUSTA-FORCE: 0 minmod (default, reading Q6), 1 van Leer, 2 MC,
  *                   3 superbee ("a variety of slope limiting methods")
  *   "t"             current time (used by the analytic Hubble ghost fill)

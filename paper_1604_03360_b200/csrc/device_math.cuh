@@ -119,6 +119,32 @@ HD void con2prim(T E, T M0, T M1, T M2, T& winv, T& p, T& v2, int& flag) {
     winv = w * sc;
 }
 
+// The constant-pressure closure p = p0 (reading Q14): v_i = M_i/(E + p0), p = p0; same outputs
+// and clamp policy (E + p0 >= 1e-300, |M| <= (1 - 1e-12)(E + p0)) as con2prim.
+template <class T>
+HD void con2prim_p0(T E, T M0, T M1, T M2, T p0, T& winv, T& p, T& v2, int& flag) {
+    T H = E + p0;
+    if (!(H >= (T)1e-300)) {
+        H = (T)1e-300;
+        flag = 1;
+    }
+    T m2 = tfma(M0, M0, tfma(M1, M1, M2 * M2));
+    const T lim = ((T)1 - (T)1e-12) * H;
+    T sc = (T)1;
+    if (m2 > lim * lim) {
+        const T mabs = tsqrt(m2);
+        if (mabs > lim) {
+            sc = lim / mabs;
+            m2 = lim * lim;
+            flag = 1;
+        }
+    }
+    const T w = fast_rcp(H);
+    p = p0;
+    v2 = m2 * w * w;
+    winv = w * sc;
+}
+
 // a3. directional characteristic speeds, c_s^2 = 1/3 (a3):
 //   a_d = ( |v_d| (1-cs2) + cs sqrt((1-v^2)(1 - v_d^2 - (v^2 - v_d^2) cs2)) ) / (1 - v^2 cs2)
 template <class T>

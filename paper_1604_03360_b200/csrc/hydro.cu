@@ -29,6 +29,7 @@ struct hydro_ctx {
     double eps = 1e-6, musta_cfl = 0.9;
     int musta_stages = 2;
     int limiter = 0;
+    EosArgs eos = {0, 0.0};
     double t_host = 0.0;  // value to push into the control block at bind / set_option("t")
     HubbleParams H;
     cudaStream_t stream = nullptr;
@@ -128,6 +129,7 @@ int do_halo(hydro_ctx* c, T* pad, double tfrac, bool use_abs, double t_abs, T* W
     }
     A.H = c->H;
     A.H.dx = c->dx;
+    A.eos = c->eos;
     if (total == 0) return HYDRO_OK;
     const int tb = 256;
     halo_fill_kernel<T><<<(unsigned)((total + tb - 1) / tb), tb, 0, c->stream>>>(c->G, A, c->ctl, tfrac, t_abs,
@@ -140,7 +142,7 @@ template <class T>
 int do_prim(hydro_ctx* c, const T* pad, int do_max) {
     const dim3 b = blk2d(64, 4);
     prim_kernel<T><<<grd(c->G.np[0], c->G.np[1], c->G.np[2], b), b, 0, c->stream>>>(c->G, pad, (T*)c->Wb[c->wcur], c->ctl,
-                                                                                      do_max);
+                                                                                      do_max, c->eos);
     LAUNCHED(c, "prim_kernel");
     return HYDRO_OK;
 }
@@ -148,7 +150,7 @@ int do_prim(hydro_ctx* c, const T* pad, int do_max) {
 template <class T>
 int do_max_speed(hydro_ctx* c, const T* pad) {
     const dim3 b = blk2d(64, 4);
-    max_speed_kernel<T><<<grd(c->G.n[0], c->G.n[1], c->G.n[2], b), b, 0, c->stream>>>(c->G, pad, c->ctl);
+    max_speed_kernel<T><<<grd(c->G.n[0], c->G.n[1], c->G.n[2], b), b, 0, c->stream>>>(c->G, pad, c->ctl, c->eos);
     LAUNCHED(c, "max_speed_kernel");
     return HYDRO_OK;
 }
@@ -163,6 +165,7 @@ StageArgs stage_args(const hydro_ctx* c, double ca, double cb, int mode) {
     A.musta_K = c->musta_stages;
     A.musta_C = c->musta_cfl;
     A.limiter = c->limiter;
+    A.eos = c->eos;
     A.epi_max = 0;
     return A;
 }
@@ -371,6 +374,14 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
     } else if (k == "musta_stages") {
         if (v < 1) return fail(c, HYDRO_EINVAL, "musta_stages < 1");
         c->musta_stages = (int)v;
+    } else if (k == "eos") {
+        if (v != 0.0 && v != 1.0) return fail(c, HYDRO_EINVAL, "eos must be 0 (p = e/3) or 1 (p = p0)");
+        c->eos.kind = (int)v;
+        c->w_ready = false;
+    } else if (k == "eos_p0") {
+        if (!(v >= 0)) return fail(c, HYDRO_EINVAL, "eos_p0 < 0");
+        c->eos.p0 = v;
+        c->w_ready = false;
     } else if (k == "limiter") {
         if (v < 0 || v > 3) return fail(c, HYDRO_EINVAL, "limiter must be 0..3");
         c->limiter = (int)v;

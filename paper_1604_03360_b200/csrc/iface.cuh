@@ -123,22 +123,26 @@ HD T limited_slope(int lim, T a, T b) {
 }
 
 // physical flux of a conserved state along DIR plus its signal speed (every evaluation needs its own
-// con2prim, O7).  Q is modified only if the Q16 clamp fires.
-template <class T, int DIR>
-HD void flux_and_speed(const T Q[NF], T F[NF], T& a, int& flag) {
+// con2prim, O7).  Q is modified only if the Q16 clamp fires.  EOSRT: the equation of state is the run-time
+// (eos, p0); otherwise the default p = e/3 at compile time.
+template <class T, int DIR, bool EOSRT>
+HD void flux_and_speed(const T Q[NF], T F[NF], T& a, int& flag, int eos, T p0) {
     T winv, p, v2;
-    con2prim(Q[0], Q[1], Q[2], Q[3], winv, p, v2, flag);
+    if (EOSRT && eos == 1) con2prim_p0(Q[0], Q[1], Q[2], Q[3], p0, winv, p, v2, flag);
+    else con2prim(Q[0], Q[1], Q[2], Q[3], winv, p, v2, flag);
     const T vd = Q[1 + DIR] * winv;
     F[0] = Q[1 + DIR];
 #pragma unroll
     for (int j = 0; j < 3; ++j) F[1 + j] = (j == DIR) ? tfma(Q[1 + j], vd, p) : Q[1 + j] * vd;
     F[4] = Q[4] * vd;
-    a = signal_speed(vd, v2, speed_inv_den(v2));
+    if (EOSRT && eos == 1) a = tabs(vd);
+    else a = signal_speed(vd, v2, speed_inv_den(v2));
 }
-template <class T, int DIR>
-HD void flux_only(const T Q[NF], T F[NF], int& flag) {
+template <class T, int DIR, bool EOSRT>
+HD void flux_only(const T Q[NF], T F[NF], int& flag, int eos, T p0) {
     T winv, p, v2;
-    con2prim(Q[0], Q[1], Q[2], Q[3], winv, p, v2, flag);
+    if (EOSRT && eos == 1) con2prim_p0(Q[0], Q[1], Q[2], Q[3], p0, winv, p, v2, flag);
+    else con2prim(Q[0], Q[1], Q[2], Q[3], winv, p, v2, flag);
     const T vd = Q[1 + DIR] * winv;
     F[0] = Q[1 + DIR];
 #pragma unroll
@@ -152,7 +156,8 @@ HD void flux_only(const T Q[NF], T F[NF], int& flag) {
 // LIMS >= 0: the limiter is the compile-time constant LIMS (the default minmod takes this path at full speed: a
 // run-time limiter inside the interface code cost 17 % of the MUSTA step); LIMS < 0: run-time `lim`.
 template <class T, int DIR, int KS, int LIMS, class Acc>
-HD void musta_force_stages(const Acc& acc, int K, T C, int lim, T fh[NF], int& flag) {
+HD void musta_force_stages(const Acc& acc, int K, T C, int lim, int eos, T p0, T fh[NF], int& flag) {
+    constexpr bool EOSRT = LIMS < 0;   // the fast path (compile-time K, minmod) is also the default closure's
     T QL[NF], QR[NF];
 #pragma unroll
     for (int c = 0; c < NF; ++c) {
@@ -166,13 +171,16 @@ HD void musta_force_stages(const Acc& acc, int K, T C, int lim, T fh[NF], int& f
 #pragma unroll
     for (int stage = 1; stage <= nst; ++stage) {
         T FL[NF], FR[NF], QM[NF], FM[NF], aL, aR;
-        flux_and_speed<T, DIR>(QL, FL, aL, flag);
-        flux_and_speed<T, DIR>(QR, FR, aR, flag);
+        flux_and_speed<T, DIR, EOSRT>(QL, FL, aL, flag, eos, p0);
+        flux_and_speed<T, DIR, EOSRT>(QR, FR, aR, flag, eos, p0);
         const T S = tmax(aL, aR);
+        // p = p0: S = max |v_d| vanishes where the fluid is at rest and tau = C/S is then infinite, in the oracle
+        // as here (reading Q7 has no finite local step without a sound speed): MUSTA-FORCE with that closure is
+        // for moving fluid only
         const T tau = C * fast_rcp(S), itau = S * invC;
 #pragma unroll
         for (int c = 0; c < NF; ++c) QM[c] = (T)0.5 * ((QL[c] + QR[c]) - tau * (FR[c] - FL[c]));
-        flux_only<T, DIR>(QM, FM, flag);
+        flux_only<T, DIR, EOSRT>(QM, FM, flag, eos, p0);
 #pragma unroll
         for (int c = 0; c < NF; ++c)
             fh[c] = (T)0.25 * (FL[c] + (T)2 * FM[c] + FR[c] - (QR[c] - QL[c]) * itau);
@@ -187,9 +195,9 @@ HD void musta_force_stages(const Acc& acc, int K, T C, int lim, T fh[NF], int& f
 }
 
 template <class T, int DIR, class Acc>
-HD void musta_force_iface(const Acc& acc, int K, T C, int lim, T fh[NF], int& flag) {
-    if (K == 2 && lim == 0) musta_force_stages<T, DIR, 2, 0>(acc, K, C, lim, fh, flag);
-    else musta_force_stages<T, DIR, 0, -1>(acc, K, C, lim, fh, flag);
+HD void musta_force_iface(const Acc& acc, int K, T C, int lim, int eos, T p0, T fh[NF], int& flag) {
+    if (K == 2 && lim == 0 && eos == 0) musta_force_stages<T, DIR, 2, 0>(acc, K, C, lim, eos, p0, fh, flag);
+    else musta_force_stages<T, DIR, 0, -1>(acc, K, C, lim, eos, p0, fh, flag);
 }
 
 }  // namespace hydro

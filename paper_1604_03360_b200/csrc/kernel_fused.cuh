@@ -99,7 +99,7 @@ struct ZWindow {
 template <class T, int SCHEME, int DIR, class Acc>
 __device__ __forceinline__ void iface_from(const Acc& acc, const StageArgs& A, T fh[NF], int& flag) {
     constexpr int R = SCHEME == 0 ? 3 : (SCHEME == 1 ? 4 : 2);
-    if constexpr (SCHEME == 2) musta_force_iface<T, DIR>(acc, A.musta_K, (T)A.musta_C, A.limiter, fh, flag);
+    if constexpr (SCHEME == 2) musta_force_iface<T, DIR>(acc, A.musta_K, (T)A.musta_C, A.limiter, A.eos.kind, (T)A.eos.p0, fh, flag);
     else llf_weno_iface<T, R, DIR>(acc, (T)A.eps, fh);
 }
 
@@ -402,7 +402,7 @@ z_sweep_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restric
         issue(k + D);             // refill the slot just consumed
         if (EPI) {
             T w[NW];
-            prim_of_cell(o, w, flag);
+            prim_of_cell(o, w, flag, A.eos);
 #pragma unroll
             for (int a = 0; a < NW; ++a) Wnext[a * G.fs + q] = w[a];
             if (A.epi_max) amax = fmax(amax, fmax((double)w[W_AX], fmax((double)w[W_AX + 1], (double)w[W_AX + 2])));

@@ -31,15 +31,32 @@ __global__ void end_step_kernel(Ctl* ctl) {
 }
 __global__ void reset_max_kernel(Ctl* ctl) { ctl->maxspeed_bits = 0ull; }
 
-// W = (winv, p, a_x, a_y, a_z) of one cell from its conserved values (a2-a3); returns the three speeds too
-template <class T>
-__device__ __forceinline__ void prim_of_cell(const T u[NF], T w[NW], int& flag) {
+// W = (winv, p, a_x, a_y, a_z) of one cell from its conserved values (a2-a3).  EOS 0: p = e/3; EOS 1: p = p0,
+// whose characteristic speeds are all v_d, so a_d = |v_d|.
+template <class T, int EOS>
+__device__ __forceinline__ void prim_of_cell_t(const T u[NF], T w[NW], int& flag, T p0) {
     T v2;
-    con2prim(u[0], u[1], u[2], u[3], w[W_INV], w[W_P], v2, flag);
-    const T id = speed_inv_den(v2);
-    w[W_AX + 0] = signal_speed(u[1] * w[W_INV], v2, id);
-    w[W_AX + 1] = signal_speed(u[2] * w[W_INV], v2, id);
-    w[W_AX + 2] = signal_speed(u[3] * w[W_INV], v2, id);
+    if (EOS == 1) {
+        con2prim_p0(u[0], u[1], u[2], u[3], p0, w[W_INV], w[W_P], v2, flag);
+        w[W_AX + 0] = tabs(u[1] * w[W_INV]);
+        w[W_AX + 1] = tabs(u[2] * w[W_INV]);
+        w[W_AX + 2] = tabs(u[3] * w[W_INV]);
+    } else {
+        con2prim(u[0], u[1], u[2], u[3], w[W_INV], w[W_P], v2, flag);
+        const T id = speed_inv_den(v2);
+        w[W_AX + 0] = signal_speed(u[1] * w[W_INV], v2, id);
+        w[W_AX + 1] = signal_speed(u[2] * w[W_INV], v2, id);
+        w[W_AX + 2] = signal_speed(u[3] * w[W_INV], v2, id);
+    }
+}
+struct EosArgs {
+    int kind;     // 0: p = e/3, 1: p = p0
+    double p0;
+};
+template <class T>
+__device__ __forceinline__ void prim_of_cell(const T u[NF], T w[NW], int& flag, const EosArgs& eos) {
+    if (eos.kind == 1) prim_of_cell_t<T, 1>(u, w, flag, (T)eos.p0);
+    else prim_of_cell_t<T, 0>(u, w, flag, (T)0);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -100,6 +117,7 @@ __device__ void hubble_cons(const HubbleParams& H, const int bc[3], int i, int j
 }
 
 struct HaloArgs {
+    EosArgs eos;
     int bc[3];
     long long count[3];  // ghost cells per axis
     HubbleParams H;
@@ -160,7 +178,7 @@ __global__ void halo_fill_kernel(Geom G, HaloArgs A, Ctl* ctl, double tfrac, dou
     if (Wghost != nullptr) {
         T w[NW];
         int flag = 0;
-        prim_of_cell(val, w, flag);
+        prim_of_cell(val, w, flag, A.eos);
 #pragma unroll
         for (int a = 0; a < NW; ++a) Wghost[a * G.fs + p] = w[a];
         if (flag) ctl->flag = 1;
@@ -190,7 +208,7 @@ __device__ __forceinline__ void block_max_to_ctl(double m, Ctl* ctl) {
 // Writes W = (winv, p, a_x, a_y, a_z).
 template <class T>
 __global__ void __launch_bounds__(256) prim_kernel(Geom G, const T* __restrict__ U, T* __restrict__ W,
-                                                   Ctl* ctl, int do_max) {
+                                                   Ctl* ctl, int do_max, EosArgs eos) {
     const int pi = blockIdx.x * blockDim.x + threadIdx.x;
     const int pj = blockIdx.y * blockDim.y + threadIdx.y;
     const int pk = blockIdx.z;
@@ -201,18 +219,12 @@ __global__ void __launch_bounds__(256) prim_kernel(Geom G, const T* __restrict__
         const int out = (i < 0 || i >= G.n[0]) + (j < 0 || j >= G.n[1]) + (k < 0 || k >= G.n[2]);
         if (out <= 1) {
             const long long p = (long long)pk * G.sxy + (long long)pj * G.sx + pi;
-            const T E = U[p], M0 = U[G.fs + p], M1 = U[2 * G.fs + p], M2 = U[3 * G.fs + p];
-            T winv, pr, v2;
-            con2prim(E, M0, M1, M2, winv, pr, v2, flag);
-            const T id = speed_inv_den(v2);
-            const T ax = signal_speed(M0 * winv, v2, id);
-            const T ay = signal_speed(M1 * winv, v2, id);
-            const T az = signal_speed(M2 * winv, v2, id);
-            W[p] = winv;
-            W[G.fs + p] = pr;
-            W[2 * G.fs + p] = ax;
-            W[3 * G.fs + p] = ay;
-            W[4 * G.fs + p] = az;
+            const T u[NF] = {U[p], U[G.fs + p], U[2 * G.fs + p], U[3 * G.fs + p], (T)0};
+            T w[NW];
+            prim_of_cell(u, w, flag, eos);
+            const T ax = w[W_AX], ay = w[W_AX + 1], az = w[W_AX + 2];
+#pragma unroll
+            for (int a = 0; a < NW; ++a) W[a * G.fs + p] = w[a];
             if (do_max && out == 0) {
                 if (G.g[0]) m = fmax(m, (double)ax);
                 if (G.g[1]) m = fmax(m, (double)ay);
@@ -226,7 +238,7 @@ __global__ void __launch_bounds__(256) prim_kernel(Geom G, const T* __restrict__
 
 // a4 alone: interior cells only, nothing stored.
 template <class T>
-__global__ void __launch_bounds__(256) max_speed_kernel(Geom G, const T* __restrict__ U, Ctl* ctl) {
+__global__ void __launch_bounds__(256) max_speed_kernel(Geom G, const T* __restrict__ U, Ctl* ctl, EosArgs eos) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     const int k = blockIdx.z;
@@ -234,13 +246,12 @@ __global__ void __launch_bounds__(256) max_speed_kernel(Geom G, const T* __restr
     int flag = 0;
     if (i < G.n[0] && j < G.n[1]) {
         const long long p = G.pidx(i, j, k);
-        const T E = U[p], M0 = U[G.fs + p], M1 = U[2 * G.fs + p], M2 = U[3 * G.fs + p];
-        T winv, pr, v2;
-        con2prim(E, M0, M1, M2, winv, pr, v2, flag);
-        const T id = speed_inv_den(v2);
-        if (G.g[0]) m = fmax(m, (double)signal_speed(M0 * winv, v2, id));
-        if (G.g[1]) m = fmax(m, (double)signal_speed(M1 * winv, v2, id));
-        if (G.g[2]) m = fmax(m, (double)signal_speed(M2 * winv, v2, id));
+        const T u[NF] = {U[p], U[G.fs + p], U[2 * G.fs + p], U[3 * G.fs + p], (T)0};
+        T w[NW];
+        prim_of_cell(u, w, flag, eos);
+        if (G.g[0]) m = fmax(m, (double)w[W_AX]);
+        if (G.g[1]) m = fmax(m, (double)w[W_AX + 1]);
+        if (G.g[2]) m = fmax(m, (double)w[W_AX + 2]);
     }
     if (flag) ctl->flag = 1;
     block_max_to_ctl(m, ctl);
