@@ -48,7 +48,9 @@ HD double fast_rcp(double x) {
 }
 HD float fast_rcp(float x) {
 #ifdef __CUDA_ARCH__
-    return __frcp_rn(x);
+    float y;   // MUFU.RCP alone: 1 ulp-level, against the correctly rounded __frcp_rn's fix-up sequence
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
 #else
     return 1.0f / x;
 #endif
@@ -71,7 +73,15 @@ HD double fast_sqrt(double x) {
     return sqrt(x);
 #endif
 }
-HD float fast_sqrt(float x) { return sqrtf(x); }
+HD float fast_sqrt(float x) {
+#ifdef __CUDA_ARCH__
+    float y;   // MUFU.SQRT alone
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+#else
+    return sqrtf(x);
+#endif
+}
 
 // ------------------------------------------------------------------------------------------------
 // a2. conserved -> primitive, closed form for p = e/3 (a2; reading Q16).
