@@ -27,6 +27,15 @@ template <class T> HD T tabs(T x) { return x < (T)0 ? -x : x; }
 template <class T> HD T tmax(T a, T b);
 template <> HD double tmax<double>(double a, double b) { return fmax(a, b); }
 template <> HD float tmax<float>(float a, float b) { return fmaxf(a, b); }
+// max of two NON-NEGATIVE numbers.  fp64 on the device: non-negative doubles order like their bit patterns, so
+// the compare runs in the integer pipe instead of occupying the fp64 pipe (DSETP + selects)
+template <class T> HD T max_nonneg(T a, T b) { return tmax(a, b); }
+#ifdef __CUDA_ARCH__
+template <>
+__device__ __forceinline__ double max_nonneg<double>(double a, double b) {
+    return __longlong_as_double(max(__double_as_longlong(a), __double_as_longlong(b)));
+}
+#endif
 template <class T> HD T tmin(T a, T b);
 template <> HD double tmin<double>(double a, double b) { return fmin(a, b); }
 template <> HD float tmin<float>(float a, float b) { return fminf(a, b); }
@@ -164,7 +173,7 @@ HD T signal_speed(T vd, T v2, T inv_den) {
     const T vd2 = vd * vd;
     // disc >= 0 analytically; the floor keeps the reciprocal-square-root seed finite when a clamped state
     // (reading Q16) drives it to zero
-    const T disc = tmax(((T)1 - v2) * ((T)1 - vd2 - (v2 - vd2) * cs2), (T)1e-30);
+    const T disc = max_nonneg(((T)1 - v2) * ((T)1 - vd2 - (v2 - vd2) * cs2), (T)1e-30);   // (a negative value loses too)
     return (tabs(vd) * ((T)1 - cs2) + cs * fast_sqrt(disc)) * inv_den;
 }
 template <class T>

@@ -39,7 +39,7 @@ HD void llf_weno_iface(const Acc& acc, T eps, T fh[NF]) {
     T md[M], vp[M], vm[M];
     T al = acc.w(W_AX + DIR, 0);
 #pragma unroll
-    for (int k = 1; k < M; ++k) al = tmax(al, acc.w(W_AX + DIR, k));
+    for (int k = 1; k < M; ++k) al = max_nonneg(al, acc.w(W_AX + DIR, k));
 #pragma unroll
     for (int k = 0; k < M; ++k) {
         md[k] = acc.u(1 + DIR, k);
@@ -173,7 +173,7 @@ HD void musta_force_stages(const Acc& acc, int K, T C, int lim, int eos, T p0, T
         T FL[NF], FR[NF], QM[NF], FM[NF], aL, aR;
         flux_and_speed<T, DIR, EOSRT>(QL, FL, aL, flag, eos, p0);
         flux_and_speed<T, DIR, EOSRT>(QR, FR, aR, flag, eos, p0);
-        const T S = tmax(aL, aR);
+        const T S = max_nonneg(aL, aR);
         // p = p0: S = max |v_d| vanishes where the fluid is at rest and tau = C/S is then infinite, in the oracle
         // as here (reading Q7 has no finite local step without a sound speed): MUSTA-FORCE with that closure is
         // for moving fluid only
