@@ -41,7 +41,7 @@ BYTES_PER_CELL_STEP = {"f64": 320.0, "f32": 160.0}
 # bytes one stage kernel moves per cell, averaged over the three stages of a step: 320/3 (fp64)
 # DRAM bytes of one stage (x/z kernel + y sweep), dram__bytes_read.sum + dram__bytes_write.sum of one
 # `ncu --set full` capture each at 512^3: profiles/r01_xz_ncu.txt, profiles/r01_ysweep_ncu.txt
-TRAFFIC_BYTES_PER_STAGE = {("weno5", "f64", 512): 10.728e9 + 5.398e9 + 14.689e9 + 10.793e9}
+TRAFFIC_BYTES_PER_STAGE = {("weno5", "f64", 512): 10.707e9 + 5.395e9 + 14.690e9 + 10.788e9}
 METRIC = "3D cell-updates/s per RK3 step"
 UNIT = "cell-updates/s"
 CFL = 0.2
