@@ -158,8 +158,6 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------------------------
-SPLIT_Z = None  # --split-z: override the library's default stage decomposition (experiments)
-
 
 def timed_run(B, torch, w, precision, steps, warmup, dist=None, profile=True, slab=None):
     """Warm up, then time `steps` RK3 steps with CUDA events on the stream.  Returns a dict.
@@ -177,8 +175,6 @@ def timed_run(B, torch, w, precision, steps, warmup, dist=None, profile=True, sl
         comm = S.DistComm(dist, w.bc[2]) if dist is not None else S.LocalComm(1, w.bc[2])
         group = S.SlabGroup([h], comm, w.dx)
         advance = lambda k: group.step_cfl(CFL, k)
-    if SPLIT_Z is not None:
-        h.set_option("split_z", SPLIT_Z)
     stream = torch.cuda.current_stream()
     advance(warmup)
     torch.cuda.synchronize()
@@ -410,13 +406,10 @@ def main():
                     help="cells per axis (use --grid under torchrun: its parser finds --n ambiguous)")
     ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--split-z", type=int, default=None, choices=[0, 1])
     ap.add_argument("--decomp", default="events", choices=["events", "slab"],
                     help="N > 1: 'events' = one independent event per GPU (weak scaling, no data-path collective); "
                          "'slab' = one event decomposed along z, halo exchange per stage (strong scaling)")
     args = ap.parse_args()
-    global SPLIT_Z
-    SPLIT_Z = args.split_z
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

@@ -52,7 +52,8 @@ enum {
     HYDRO_EINVAL = -1,      /* bad argument, unknown option, call out of order                   */
     HYDRO_ENOMEM = -2,      /* workspace missing or too small                                    */
     HYDRO_ECUDA = -3,       /* a CUDA runtime call or kernel launch failed (text in last_error)  */
-    HYDRO_EUNPHYSICAL = -4  /* con2prim had to clamp a cell (E < 1e-300 or |M| > (1-1e-12) E)    */
+    HYDRO_EUNPHYSICAL = -4  /* con2prim had to clamp a cell (E < 1e-300, |M| > (1-1e-12) E) or met a
+                               non-finite value (NaN / Inf energy or momentum)                  */
 };
 
 /* Create a context for an nx x ny x nz grid of spacing dx (same on all axes, the |e_i| of Eq. (2),
@@ -64,7 +65,9 @@ int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme)
 /* Set an option.  Must precede hydro_bind_workspace for "precision" (it changes the workspace size).
  *   "precision"     HYDRO_F64 (default) | HYDRO_F32: arithmetic and storage type of the whole path
  *   "bc_x|bc_y|bc_z" boundary rule per axis (default outflow = copy the nearest interior cell)
- *   "weno_eps"      epsilon of the WENO weights (default 1e-6, reading Q5)
+ *   "weno_eps"      epsilon of the WENO weights (default 1e-6, reading Q5; EINVAL below 1e-40: the weights are
+ *                   evaluated cross-multiplied, which takes epsilon to the 6th power.  For the same reason fp64
+ *                   data must stay below about 1e25 in magnitude; the fp32 path rescales and has no such limit)
  *   "musta_stages"  K of MUSTA-FORCE (default 2, reading Q8);  "musta_cfl" its local Courant number
  *                   (default 0.9, reading Q7)
  *   "eos", "eos_p0" equation of state: 0 (default) p = e/3 (reading Q2); 1 p = eos_p0, a constant (the closure for
@@ -76,16 +79,14 @@ int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme)
  *   "x0|y0|z0"      coordinate of the low face of the domain on each axis
  *   "hubble_t0|hubble_e0|hubble_n0|hubble_bx|hubble_by|hubble_bz"  parameters of the closed-form
  *                   Hubble flow used by HYDRO_BC_HUBBLE (readings Q13, Q14)
- *   "split_z"       1 (default): a stage is the x/y tiled kernel followed by the z sweep kernel;
- *                   0: one kernel with the z register window inside
- *   "layout"        with split_z = 1: 1 (default) = x/z marching kernel + y sweep, 0 = x/y tile kernel + z sweep
- *   "tile_zc", "sweep_zc"  planes a block of the tile kernel / of the z sweep marches through (defaults 64 / 128;
- *                   tuning knobs: a longer march amortises the one redundant z-flux and the pipeline fill)
+ *   "tile_zc", "sweep_zc"  cells a block of the x/z kernel marches through along z / of the y sweep along y
+ *                   (defaults 128 / 128 for the WENO kernels, 64 / 128 for MUSTA-FORCE; tuning knobs: a longer
+ *                   march amortises the one redundant flux and the pipeline fill of a chunk)
  *   "profile"       0 (default) | 1: record a CUDA event pair on the stream around every stage-kernel
  *                   launch, read back with hydro_stage_kernel_time
- *   "kernel"        HYDRO_KERNEL_AUTO (default: fused stage kernel where the grid allows, else the
- *                   generic one) | HYDRO_KERNEL_GENERIC | HYDRO_KERNEL_FUSED (EINVAL at step time if
- *                   the grid does not allow it)
+ *   "kernel"        HYDRO_KERNEL_AUTO (default: the marching stage kernels where all three axes are active,
+ *                   else the generic one-thread-per-cell kernel) | HYDRO_KERNEL_GENERIC | HYDRO_KERNEL_FUSED
+ *                   (= marching; EINVAL at step time if the grid does not allow it)
  * EINVAL for an unknown key or a value out of range. */
 int hydro_set_option(hydro_ctx *ctx, const char *key, double value);
 
@@ -94,21 +95,25 @@ int hydro_set_option(hydro_ctx *ctx, const char *key, double value);
 int hydro_set_stream(hydro_ctx *ctx, void *cuda_stream);
 
 /* Bytes of device memory the context needs for its padded state copies (three: u^n and two RK stage
- * buffers), two copies of the per-cell primitive arrays and a small control block. */
+ * buffers, five arrays each), two copies of the seven per-cell primitive arrays (v_x, v_y, v_z, p, a_x, a_y, a_z)
+ * and a 256-byte control block. */
 size_t hydro_workspace_bytes(const hydro_ctx *ctx);
 
 /* Hand the context its device memory (256-byte aligned, at least hydro_workspace_bytes()).  The caller
- * keeps ownership.  ENOMEM if too small, EINVAL if misaligned.  Zero-fills it on the stream. */
+ * keeps ownership.  ENOMEM if too small, EINVAL if misaligned or not CUDA device memory.  Zero-fills it on the
+ * stream.  The context remembers the device the memory lives on: every later call runs there whatever device is
+ * current in the calling thread (and restores the caller's current device before returning). */
 int hydro_bind_workspace(hydro_ctx *ctx, void *device_ptr, size_t bytes);
 
 /* Copy the interior conserved state in from / out to a DEVICE pointer ([5][nz][ny][nx], element type
- * per "precision").  Asynchronous on the stream.  set_state also clears the unphysical flag. */
+ * per "precision").  Asynchronous on the stream.  set_state also clears the unphysical flag and the cached max
+ * signal speed; the current time is NOT touched (it only changes through the "t" option and by stepping). */
 int hydro_set_state(hydro_ctx *ctx, const void *cons_device);
 int hydro_get_state(hydro_ctx *ctx, void *cons_device_out);
 
-/* The same through HOST pointers: the library stages through the first RK buffer with
+/* The same through HOST pointers: the library stages through its third state buffer (idle between steps) with
  * cudaMemcpyAsync and synchronises the stream before returning.  These are the end-to-end entry points
- * (bench.py "e2e"). */
+ * (bench.py "e2e").  EINVAL between hydro_step_stage(., 0) and hydro_step_stage(., 2), where that buffer is live. */
 int hydro_set_state_host(hydro_ctx *ctx, const void *cons_host);
 int hydro_get_state_host(hydro_ctx *ctx, void *cons_host_out);
 

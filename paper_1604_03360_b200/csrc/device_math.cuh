@@ -14,8 +14,9 @@
 namespace hydro {
 
 enum { NF = 5 };                       // E, Mx, My, Mz, R
-enum { W_INV = 0, W_P = 1, W_AX = 2 }; // primitive arrays: 1/(E+p) scaled (see con2prim), p, a_x, a_y, a_z
-enum { NW = 5 };
+// primitive arrays kept beside a state: v_x, v_y, v_z, p, a_x, a_y, a_z (a2-a3 of every cell, made once per stage)
+enum { W_V = 0, W_P = 3, W_AX = 4 };
+enum { NW = 7 };
 
 template <class T> HD T tfma(T a, T b, T c);
 template <> HD double tfma<double>(double a, double b, double c) { return fma(a, b, c); }
@@ -99,13 +100,17 @@ HD float fast_sqrt(float x) {
 // |M| <= (1-1e-12) E raises flag; the caller's E and M are left alone (the physical flux keeps using
 // them), the rescaling of M goes into winv.
 template <class T>
-HD bool below_floor(T E) { return !(E >= (T)1e-300); }
+HD bool below_floor(T E) {   // true for NaN and +Inf too: a non-finite energy must raise the flag (reading Q16)
+    return !(E >= (T)1e-300) || E > (T)(sizeof(T) == 8 ? 1.7976931348623157e308 : 3.4028234e38);
+}
 #ifdef __CUDA_ARCH__
 // fp64: positive doubles order like their bit patterns, so the floor test is an integer compare on the high
 // word (negative E fails it through the sign bit); keeps one compare off the fp64 pipe
 template <>
 __device__ __forceinline__ bool below_floor<double>(double E) {
-    return __double2hiint(E) < 0x01a56e1f;   // high word of 1e-300 = 0x01a56e1fc2f8f359
+    // high word of 1e-300 = 0x01a56e1fc2f8f359; 0x7ff00000 and above is +Inf / +NaN: one unsigned compare of
+    // (hi - floor) against the width of the admissible band rejects negative, tiny, infinite and NaN energies
+    return (unsigned)(__double2hiint(E) - 0x01a56e1f) >= (unsigned)(0x7ff00000 - 0x01a56e1f);
 }
 #endif
 
@@ -119,10 +124,10 @@ HD void con2prim(T E, T M0, T M1, T M2, T& winv, T& p, T& v2, int& flag) {
     T t = E * E;
     T sc = (T)1;
     const T c2 = ((T)1 - (T)1e-12) * ((T)1 - (T)1e-12);
-    if (m2 > c2 * t) {   // |M| > (1 - 1e-12) E up to rounding: settle it with the square root (rare path)
+    if (!(m2 <= c2 * t)) {   // |M| > (1 - 1e-12) E up to rounding, or NaN: settle it with the square root (rare path)
         const T lim = ((T)1 - (T)1e-12) * E;
         const T mabs = tsqrt(m2);
-        if (mabs > lim) {
+        if (!(mabs <= lim)) {   // a NaN momentum lands here as well: flagged
             sc = lim / mabs;
             m2 = lim * lim;
             flag = 1;
@@ -150,9 +155,9 @@ HD void con2prim_p0(T E, T M0, T M1, T M2, T p0, T& winv, T& p, T& v2, int& flag
     T m2 = tfma(M0, M0, tfma(M1, M1, M2 * M2));
     const T lim = ((T)1 - (T)1e-12) * H;
     T sc = (T)1;
-    if (m2 > lim * lim) {
+    if (!(m2 <= lim * lim)) {
         const T mabs = tsqrt(m2);
-        if (mabs > lim) {
+        if (!(mabs <= lim)) {
             sc = lim / mabs;
             m2 = lim * lim;
             flag = 1;
@@ -187,19 +192,48 @@ HD T speed_inv_den(T v2) { return fast_rcp(tfma(v2, (T)(-1.0 / 3.0), (T)1)); }
 // the classic weights alpha_k = d_k/(eps+beta_k)^2 multiplied through by prod_j (eps+beta_j)^2
 // (DESIGN.md section 6).  beta' and eps' carry a common scale factor, which cancels in N/D.
 
-// WENO5 (Jiang-Shu, O3).  Here beta' = 4 beta and eps4 = 4 eps.
+// Cross-multiplied weights need the products prod_{j != k} B_j^2 (B^4 for WENO5, B^6 for WENO7) to stay inside the
+// normal range.  fp64: they do for |data| < 1e25 (documented in include/hydro.h).  fp32: flux jumps of order 1e3
+// overflow B^6 and a tiny epsilon on flat data underflows it, so the B_k are first multiplied by the power of two
+// that brings the smallest of them to [1, 2) (exact, and it cancels in N/D) and clamped at 2^18: a sub-stencil
+// whose indicator is 2^18 times the smallest carries a weight below 2^-36 of the dominant one either way, far
+// under fp32 resolution; the products then stay below 2^108, which leaves room for the factors g_k of N.
+template <class T, int NB>
+HD void normalise_indicators(T (&B)[NB]) {}
+#ifdef __CUDA_ARCH__
+template <>
+__device__ __forceinline__ void normalise_indicators<float, 3>(float (&B)[3]) {
+    const float m = fminf(B[0], fminf(B[1], B[2]));
+    const float s = __int_as_float(0x7f000000 - (__float_as_int(m) & 0x7f800000));   // 2^(127 - exponent(m)) / 2^0
+    const float cap = 262144.0f;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) B[k] = fminf(B[k] * s, cap);
+}
+template <>
+__device__ __forceinline__ void normalise_indicators<float, 4>(float (&B)[4]) {
+    const float m = fminf(fminf(B[0], B[1]), fminf(B[2], B[3]));
+    const float s = __int_as_float(0x7f000000 - (__float_as_int(m) & 0x7f800000));
+    const float cap = 262144.0f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) B[k] = fminf(B[k] * s, cap);
+}
+#endif
+
+// WENO5 (Jiang-Shu, O3) from the four first differences D_j = f_{j+1} - f_j of the stencil
+// (a, b, c, d, e).  Here beta' = 4 beta and eps4 = 4 eps.
 template <class T>
-HD void weno5_nd(T a, T b, T c, T d, T e, T eps4, T& N, T& D) {
-    const T D1 = b - a, D2 = c - b, D3 = d - c, D4 = e - d;
+HD void weno5_nd_d(T D1, T D2, T D3, T D4, T eps4, T& N, T& D) {
     const T t0 = D2 - D1, t1 = D3 - D2, t2 = D4 - D3;      // second differences
     const T u0 = tfma((T)3, D2, -D1);                      // a - 4b + 3c
     const T u1 = D2 + D3;                                  // d - b
     const T u2 = tfma((T)-3, D3, D4);                      // 3c - 4d + e, sign irrelevant (squared)
     const T k = (T)(13.0 / 3.0);
-    const T B0 = tfma(k * t0, t0, tfma(u0, u0, eps4));
-    const T B1 = tfma(k * t1, t1, tfma(u1, u1, eps4));
-    const T B2 = tfma(k * t2, t2, tfma(u2, u2, eps4));
-    const T s0 = B0 * B0, s1 = B1 * B1, s2 = B2 * B2;
+    T B[3];
+    B[0] = tfma(k * t0, t0, tfma(u0, u0, eps4));
+    B[1] = tfma(k * t1, t1, tfma(u1, u1, eps4));
+    B[2] = tfma(k * t2, t2, tfma(u2, u2, eps4));
+    normalise_indicators<T, 3>(B);
+    const T s0 = B[0] * B[0], s1 = B[1] * B[1], s2 = B[2] * B[2];
     const T P0 = s1 * s2, P1 = s0 * s2, P2 = s0 * s1;
     // 10 d_k = (1, 6, 3);  q_k - c = (5 D2 - 2 D1)/6, (D2 + 2 D3)/6, (4 D3 - D4)/6
     const T g0 = tfma((T)(5.0 / 6.0), D2, (T)(-1.0 / 3.0) * D1);
@@ -208,6 +242,10 @@ HD void weno5_nd(T a, T b, T c, T d, T e, T eps4, T& N, T& D) {
     N = tfma(P0, g0, tfma(P1, g1, P2 * g2));
     D = tfma((T)6, P1, tfma((T)3, P2, P0));
 }
+template <class T>
+HD void weno5_nd(T a, T b, T c, T d, T e, T eps4, T& N, T& D) {
+    weno5_nd_d(b - a, c - b, d - c, e - d, eps4, N, D);
+}
 
 // WENO7 (Balsara-Shu, O4).  For the cubic through four cell averages written as
 // c0 + c1 x + c2 x^2 + c3 x^3 about the centre of cell i (dx = 1) the smoothness indicator is
@@ -215,10 +253,9 @@ HD void weno5_nd(T a, T b, T c, T d, T e, T eps4, T& N, T& D) {
 // (the integrals of the squared first, second and third derivatives over the cell, summed); in terms
 // of undivided differences c3 = D3/6, c2 = (second difference at i)/2 and c1 follows from matching
 // the averages.  This equals the integer-coefficient quadratic forms of O4 divided by 240.
+// Input: the six first differences E_j = f_{j+1} - f_j of the stencil (a..g), centre cell d.
 template <class T>
-HD void weno7_nd(T a, T b, T c, T d, T e, T f, T g, T eps, T& N, T& D) {
-    // first differences around the centre cell d
-    const T E1 = b - a, E2 = c - b, E3 = d - c, E4 = e - d, E5 = f - e, E6 = g - f;
+HD void weno7_nd_d(T E1, T E2, T E3, T E4, T E5, T E6, T eps, T& N, T& D) {
     const T S1 = E2 - E1, S2 = E3 - E2, S3 = E4 - E3, S4 = E5 - E4, S5 = E6 - E5;  // second
     const T T1 = S2 - S1, T2 = S3 - S2, T3 = S4 - S3, T4 = S5 - S4;                // third
     // Stencil k holds cells (k..k+3) of (a..g); the centre cell d sits at position 3-k inside it.
@@ -234,11 +271,13 @@ HD void weno7_nd(T a, T b, T c, T d, T e, T f, T g, T eps, T& N, T& D) {
     const T c3_1 = T2 * sixth, c2_1 = (T)0.5 * S3, m_1 = tfma((T)(-1.0 / 6.0), T2, (T)0.5 * (E3 + E4));
     const T c3_2 = T3 * sixth, c2_2 = (T)0.5 * S3, m_2 = tfma((T)(-1.0 / 6.0), T3, (T)0.5 * (E3 + E4));
     const T c3_3 = T4 * sixth, c2_3 = (T)0.5 * (S4 - T4), m_3 = E4 + tfma((T)-0.5, S4, (T)(1.0 / 3.0) * T4);
-    const T B0 = tfma(m_0, m_0, tfma(k13 * c2_0, c2_0, tfma(k781 * c3_0, c3_0, eps)));
-    const T B1 = tfma(m_1, m_1, tfma(k13 * c2_1, c2_1, tfma(k781 * c3_1, c3_1, eps)));
-    const T B2 = tfma(m_2, m_2, tfma(k13 * c2_2, c2_2, tfma(k781 * c3_2, c3_2, eps)));
-    const T B3 = tfma(m_3, m_3, tfma(k13 * c2_3, c2_3, tfma(k781 * c3_3, c3_3, eps)));
-    const T s0 = B0 * B0, s1 = B1 * B1, s2 = B2 * B2, s3 = B3 * B3;
+    T B[4];
+    B[0] = tfma(m_0, m_0, tfma(k13 * c2_0, c2_0, tfma(k781 * c3_0, c3_0, eps)));
+    B[1] = tfma(m_1, m_1, tfma(k13 * c2_1, c2_1, tfma(k781 * c3_1, c3_1, eps)));
+    B[2] = tfma(m_2, m_2, tfma(k13 * c2_2, c2_2, tfma(k781 * c3_2, c3_2, eps)));
+    B[3] = tfma(m_3, m_3, tfma(k13 * c2_3, c2_3, tfma(k781 * c3_3, c3_3, eps)));
+    normalise_indicators<T, 4>(B);
+    const T s0 = B[0] * B[0], s1 = B[1] * B[1], s2 = B[2] * B[2], s3 = B[3] * B[3];
     const T s01 = s0 * s1, s23 = s2 * s3;
     const T P0 = s1 * s23, P1 = s0 * s23, P2 = s01 * s3, P3 = s01 * s2;
     // q_k - d (centre value) from the candidate polynomials of O4:
@@ -253,6 +292,10 @@ HD void weno7_nd(T a, T b, T c, T d, T e, T f, T g, T eps, T& N, T& D) {
     const T g3 = tfma((T)3, E4, tfma((T)(-4.0 / 3.0), E5, (T)(1.0 / 3.0) * E6)); // x 4/12
     N = tfma(P0, g0, tfma(P1, g1, tfma(P2, g2, P3 * g3)));
     D = tfma((T)12, P1, tfma((T)18, P2, tfma((T)4, P3, P0)));
+}
+template <class T>
+HD void weno7_nd(T a, T b, T c, T d, T e, T f, T g, T eps, T& N, T& D) {
+    weno7_nd_d(b - a, c - b, d - c, e - d, f - e, g - f, eps, N, D);
 }
 
 }  // namespace hydro

@@ -1,6 +1,7 @@
 // hydro.cu -- C ABI of libhydro_b200 (include/hydro.h): context, options, workspace carving and the
 // launch sequence of one SSP-RK3 step:
-//   per stage:  halo fill (a1) -> con2prim + speeds [+ max] (a2-a4) -> stage kernel (a5-a9)
+//   per stage:  halo fill (a1) -> [con2prim + speeds + max (a2-a4), first step only] -> stage kernels (a5-a9, and
+//   a2-a4 of the cells they finish)
 // No CPU arithmetic of the method happens here: the host only orders kernels on the caller's stream.
 #include <cuda_runtime.h>
 
@@ -12,9 +13,9 @@
 
 #include "../../include/hydro.h"
 #include "grid.cuh"
-#include "kernel_fused.cuh"
-#include "kernel_xz.cuh"
+#include "kernel_fp.cuh"
 #include "kernel_generic.cuh"
+#include "kernel_musta.cuh"
 #include "kernels_aux.cuh"
 
 using namespace hydro;
@@ -43,8 +44,12 @@ struct hydro_ctx {
                                                 // writes the next stage's while this stage's are still read
     int wcur = 0;                               // buffer holding the primitives of the stage input
     bool w_ready = false;                       // interior of Wb[wcur] already holds the primitives of u^n
-    FusedPlan fused;                            // tensor maps etc. for the fused kernel
-    bool fused_ready = false;
+    bool max_ready = false;                     // ctl->maxspeed_bits holds the max signal speed of u^n (stage-3 epilogue)
+    int stage_open = 0;                         // stages of a hydro_step_stage sequence done so far (0 = between steps)
+    int device = -1;                            // CUDA device of the workspace (captured at bind)
+    int zc = 0, yc = 0;                         // chunk lengths of the z / y march ("tile_zc", "sweep_zc"; 0 = default)
+    bool fused_ready = false;                   // the marching kernels' shared-memory attributes are set
+    char plan_err[256] = {0};
     long long launches = 0;
     // "profile" option: CUDA events around every stage-kernel launch (bench.py roofline)
     int profile = 0;
@@ -84,6 +89,21 @@ void make_geom(hydro_ctx* c) {
 }
 
 size_t state_bytes(const hydro_ctx* c) { return (size_t)NF * (size_t)c->G.fs * esize(c); }
+size_t prim_bytes(const hydro_ctx* c) { return (size_t)NW * (size_t)c->G.fs * esize(c); }
+
+// Every entry point that touches the device runs on the device of the workspace, whatever device is current in the
+// calling thread; the caller's current device is restored on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const hydro_ctx* c) {
+        if (c && c->device >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != c->device)
+            switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+};
 
 #define CUDA_OK(c, call)                                                                      \
     do {                                                                                      \
@@ -101,8 +121,8 @@ size_t state_bytes(const hydro_ctx* c) { return (size_t)NF * (size_t)c->G.fs * e
 dim3 blk2d(int bx, int by) { return dim3(bx, by, 1); }
 dim3 grd(int nx, int ny, int nz, dim3 b) { return dim3((nx + b.x - 1) / b.x, (ny + b.y - 1) / b.y, nz); }
 
-__global__ void set_ctl_kernel(Ctl* ctl, double t, int reset_flag) {
-    ctl->t = t;
+__global__ void set_ctl_kernel(Ctl* ctl, double t, int set_t, int reset_flag) {
+    if (set_t) ctl->t = t;
     if (reset_flag) {
         ctl->flag = 0;
         ctl->maxspeed_bits = 0ull;
@@ -170,10 +190,22 @@ StageArgs stage_args(const hydro_ctx* c, double ca, double cb, int mode) {
     return A;
 }
 
+// the marching kernels need all three axes active (the 400 x 1 x 1 shock tube takes the generic kernel)
+bool fused_supported(const Geom& G) { return G.g[0] > 0 && G.g[1] > 0 && G.g[2] > 0; }
+
 bool want_fused(const hydro_ctx* c) {
     if (c->kernel == HYDRO_KERNEL_GENERIC) return false;
     if (c->kernel == HYDRO_KERNEL_AUTO && !c->fused_ready) return false;
-    return fused_supported(c->G, c->scheme, c->precision);
+    return fused_supported(c->G);
+}
+
+template <class T>
+int configure_marching(hydro_ctx* c) {
+    switch (c->scheme) {
+        case HYDRO_WENO5: return configure_fp<T, 3>(c->plan_err, sizeof c->plan_err);
+        case HYDRO_WENO7: return configure_fp<T, 4>(c->plan_err, sizeof c->plan_err);
+        default: return configure_musta<T>(c->plan_err, sizeof c->plan_err);
+    }
 }
 
 // records an event pair around the stage kernel when the "profile" option is on
@@ -192,23 +224,33 @@ struct StageTimer {
     }
 };
 
+// One stage: Uout = ca u^n + cb (Us + dt L(Us)), or L(Us) itself (mode 1).  Pbuf: scratch state buffer for the
+// partial result of the field-parallel pair (may be Uout unless Uout is u^n).
 template <class T>
-int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double cb, int mode, T* Wnext = nullptr,
-             int epi_max = 0) {
+int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, T* Pbuf, double ca, double cb, int mode,
+             T* Wnext = nullptr, int epi_max = 0) {
     StageArgs A = stage_args(c, ca, cb, mode);
     A.epi_max = epi_max;
     StageTimer timer(c);
     if (want_fused(c)) {
-        if (!c->fused_ready) return fail(c, HYDRO_ECUDA, "fused plan not built: %s", c->fused.err);
-        int nl = 0;
-        const int rc = launch_fused<T>(c->fused, c->G, c->scheme, A, Us, (const T*)c->Wb[c->wcur], Un, Uout, Wnext,
-                                       c->ctl, c->stream, &nl);
-        if (rc != 0) return fail(c, HYDRO_ECUDA, "fused launch: %s", c->fused.err);
+        if (!c->fused_ready) return fail(c, HYDRO_ECUDA, "marching kernels not configured: %s", c->plan_err);
+        int nl = 0, rc;
+        const T* W = (const T*)c->Wb[c->wcur];
+        if (c->scheme == HYDRO_MUSTA_FORCE)
+            rc = launch_musta<T>(c->G, A, Us, Un, Uout, c->ctl, c->zc > 0 ? c->zc : 64, c->yc > 0 ? c->yc : 128,
+                                 c->stream, &nl, c->plan_err, sizeof c->plan_err);
+        else if (c->scheme == HYDRO_WENO5)
+            rc = launch_fp<T, 3>(c->G, A, Us, W, Un, Uout, Pbuf, Wnext, c->ctl, c->zc > 0 ? c->zc : FP_ZC,
+                                 c->yc > 0 ? c->yc : FP_YC, c->stream, &nl, c->plan_err, sizeof c->plan_err);
+        else
+            rc = launch_fp<T, 4>(c->G, A, Us, W, Un, Uout, Pbuf, Wnext, c->ctl, c->zc > 0 ? c->zc : FP_ZC,
+                                 c->yc > 0 ? c->yc : FP_YC, c->stream, &nl, c->plan_err, sizeof c->plan_err);
+        if (rc != 0) return fail(c, HYDRO_ECUDA, "stage launch: %s", c->plan_err);
         c->launches += nl;
         return HYDRO_OK;
     }
     if (c->kernel == HYDRO_KERNEL_FUSED)
-        return fail(c, HYDRO_EINVAL, "kernel=fused requested but the grid/scheme does not allow it");
+        return fail(c, HYDRO_EINVAL, "kernel=fused requested but the grid does not allow it (an axis is inactive)");
     const dim3 b = blk2d(32, 4);
     const dim3 g = grd(c->G.n[0], c->G.n[1], c->G.n[2], b);
     const T* W = (const T*)c->Wb[c->wcur];
@@ -223,39 +265,51 @@ int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double 
 
 // One SSP-RK3 step (a9, O8):  u1 = u + dt L(u);  u2 = 3/4 u + 1/4 (u1 + dt L(u1));
 // u' = 1/3 u + 2/3 (u2 + dt L(u2)), ghosts at t, t+dt, t+dt/2.  dt_fixed > 0, or CFL mode.
-// WENO with the split tiled kernels: the z sweep of every stage leaves the primitives of its output in the
-// other W buffer (and stage 3 the max signal speed), so con2prim runs as a separate pass only for the first
-// step after hydro_set_state / hydro_eval_L; the ghost cells' primitives come from the halo kernel.
+// With the marching kernels every stage leaves what the next one needs: the WENO x/z kernel's epilogue writes the
+// primitives of its output into the other W buffer, and stage 3 of either scheme reduces the max signal speed of
+// the new state.  con2prim (WENO) or the max-speed pass (MUSTA-FORCE, CFL mode) therefore run as separate kernels
+// only for the first step after hydro_set_state / hydro_eval_L; the ghost cells' primitives come from the halo kernel.
 template <class T>
 int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl) {
     T* U[3] = {(T*)c->U[0], (T*)c->U[1], (T*)c->U[2]};
     const bool weno = c->scheme != HYDRO_MUSTA_FORCE;
     const bool cflmode = !(dt_fixed > 0.0);
-    const bool epi = weno && want_fused(c) && c->fused.split_z;
+    const bool marching = want_fused(c);
+    const bool epi = weno && marching;
     const double tfrac[3] = {0.0, 1.0, 0.5};
     const double ca[3] = {0.0, 0.75, 1.0 / 3.0}, cb[3] = {1.0, 0.25, 2.0 / 3.0};
     T* const in[3] = {U[0], U[1], U[2]};
     T* const out[3] = {U[1], U[2], U[0]};   // stage 3 writes u^n in place: each cell reads only its own u^n
+    T* const scratch[3] = {U[1], U[2], U[1]};   // partial result of the field-parallel pair; U[1] is free in stage 3
     int rc;
     const bool have_w = c->w_ready;   // interior primitives of in[s] already in Wb[wcur] (previous stage's epilogue)
     if ((rc = do_halo<T>(c, in[s], tfrac[s], false, 0.0, (weno && have_w) ? (T*)c->Wb[c->wcur] : nullptr))) return rc;
+    const bool need_max = s == 0 && cflmode && !c->max_ready;
+    if (need_max) {   // the reduction accumulates with atomicMax: start from zero
+        reset_max_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
+        LAUNCHED(c, "reset_max_kernel");
+    }
     if (weno && !have_w) {
-        if ((rc = do_prim<T>(c, in[s], (s == 0 && cflmode) ? 1 : 0))) return rc;
-    } else if (!weno && s == 0 && cflmode) {
+        if ((rc = do_prim<T>(c, in[s], need_max ? 1 : 0))) return rc;
+    } else if (need_max) {
         if ((rc = do_max_speed<T>(c, in[s]))) return rc;
     }
     if (s == 0) {
         begin_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl, dt_fixed, cfl, c->dx);
         LAUNCHED(c, "begin_step_kernel");
+        c->max_ready = false;
     }
     T* Wnext = epi ? (T*)c->Wb[c->wcur ^ 1] : nullptr;
-    if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, Wnext, s == 2 ? 1 : 0))) return rc;
+    if ((rc = do_stage<T>(c, in[s], U[0], out[s], scratch[s], ca[s], cb[s], 0, Wnext, (marching && s == 2) ? 1 : 0)))
+        return rc;
     if (epi) c->wcur ^= 1;
     c->w_ready = epi;
     if (s == 2) {
         end_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
         LAUNCHED(c, "end_step_kernel");
+        c->max_ready = marching;
     }
+    c->stage_open = s == 2 ? 0 : s + 1;
     return HYDRO_OK;
 }
 
@@ -300,7 +354,7 @@ int eval_L_impl(hydro_ctx* c, const void* cons, double t_stage, void* L_out) {
     LAUNCHED(c, "pack_kernel");
     if ((rc = do_halo<T>(c, U1, 0.0, true, t_stage))) return rc;
     if (c->scheme != HYDRO_MUSTA_FORCE && (rc = do_prim<T>(c, U1, 0))) return rc;
-    if ((rc = do_stage<T>(c, U1, U1, U2, 0.0, 1.0, 1))) return rc;
+    if ((rc = do_stage<T>(c, U1, U1, U2, U2, 0.0, 1.0, 1))) return rc;
     unpack_kernel<T><<<g, b, 0, c->stream>>>(c->G, U2, (T*)L_out);
     LAUNCHED(c, "unpack_kernel");
     return HYDRO_OK;
@@ -357,14 +411,9 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
         const int p = (int)v;
         if (p < 0 || p > 2) return fail(c, HYDRO_EINVAL, "kernel must be 0, 1 or 2");
         c->kernel = p;
-    } else if (k == "layout") {
-        if (v != 0.0 && v != 1.0) return fail(c, HYDRO_EINVAL, "layout must be 0 or 1");
-        c->fused.layout = (int)v;
-    } else if (k == "split_z") {
-        c->fused.split_z = v != 0.0;
     } else if (k == "tile_zc" || k == "sweep_zc") {
         if (v < 1) return fail(c, HYDRO_EINVAL, "%s < 1", key);
-        (k == "tile_zc" ? c->fused.tile_zc : c->fused.sweep_zc) = (int)v;
+        (k == "tile_zc" ? c->zc : c->yc) = (int)v;
     } else if (k == "profile") {
         c->profile = v != 0.0;
     } else if (k == "bc_x" || k == "bc_y" || k == "bc_z") {
@@ -377,11 +426,11 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
     } else if (k == "eos") {
         if (v != 0.0 && v != 1.0) return fail(c, HYDRO_EINVAL, "eos must be 0 (p = e/3) or 1 (p = p0)");
         c->eos.kind = (int)v;
-        c->w_ready = false;
+        c->w_ready = c->max_ready = false;   // cached primitives and max signal speed belong to the old closure
     } else if (k == "eos_p0") {
         if (!(v >= 0)) return fail(c, HYDRO_EINVAL, "eos_p0 < 0");
         c->eos.p0 = v;
-        c->w_ready = false;
+        c->w_ready = c->max_ready = false;
     } else if (k == "limiter") {
         if (v < 0 || v > 3) return fail(c, HYDRO_EINVAL, "limiter must be 0..3");
         c->limiter = (int)v;
@@ -389,12 +438,14 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
         if (!(v > 0)) return fail(c, HYDRO_EINVAL, "musta_cfl <= 0");
         c->musta_cfl = v;
     } else if (k == "weno_eps") {
-        if (!(v > 0)) return fail(c, HYDRO_EINVAL, "weno_eps <= 0");
+        // the cross-multiplied weights take epsilon to the 4th (WENO5) or 6th (WENO7) power
+        if (!(v >= 1e-40)) return fail(c, HYDRO_EINVAL, "weno_eps < 1e-40");
         c->eps = v;
     } else if (k == "t") {
         c->t_host = v;
         if (c->ws) {
-            set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, v, 0);
+            DeviceGuard dg(c);
+            set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, v, 1, 0);
             LAUNCHED(c, "set_ctl_kernel");
         }
     } else if (k == "x0") c->H.origin[0] = v;
@@ -412,7 +463,7 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
 
 size_t hydro_workspace_bytes(const hydro_ctx* c) {
     if (!c) return 0;
-    return 256 + 5 * state_bytes(c);  // control block, U0, U1, U2, W (two buffers)
+    return 256 + 3 * state_bytes(c) + 2 * prim_bytes(c);  // control block, U0, U1, U2, W (two buffers)
 }
 
 int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
@@ -420,6 +471,13 @@ int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
     if (((size_t)p & 255) != 0) return fail(c, HYDRO_EINVAL, "workspace must be 256-byte aligned");
     if (bytes < hydro_workspace_bytes(c))
         return fail(c, HYDRO_ENOMEM, "workspace too small: %zu < %zu", bytes, hydro_workspace_bytes(c));
+    cudaPointerAttributes attr;
+    if (cudaPointerGetAttributes(&attr, p) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+        cudaGetLastError();
+        return fail(c, HYDRO_EINVAL, "workspace is not CUDA device memory");
+    }
+    c->device = attr.device;
+    DeviceGuard dg(c);
     c->ws = p;
     c->ws_bytes = bytes;
     char* base = (char*)p;
@@ -427,19 +485,18 @@ int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
     const size_t sb = state_bytes(c);
     for (int i = 0; i < 3; ++i) c->U[i] = base + 256 + i * sb;
     c->Wb[0] = base + 256 + 3 * sb;
-    c->Wb[1] = base + 256 + 4 * sb;
+    c->Wb[1] = c->Wb[0] + prim_bytes(c);
     c->wcur = 0;
-    c->w_ready = false;
+    c->w_ready = c->max_ready = false;
+    c->stage_open = 0;
     CUDA_OK(c, cudaMemsetAsync(p, 0, hydro_workspace_bytes(c), c->stream));
-    set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, c->t_host, 1);
+    set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, c->t_host, 1, 1);
     LAUNCHED(c, "set_ctl_kernel");
     c->fused_ready = false;
-    if (fused_supported(c->G, c->scheme, c->precision) && c->kernel != HYDRO_KERNEL_GENERIC) {
-        void* Ubuf[3] = {c->U[0], c->U[1], c->U[2]};
-        void* Wbuf[2] = {c->Wb[0], c->Wb[1]};
-        c->fused_ready = build_fused_plan(c->fused, c->G, c->scheme, c->precision, Ubuf, Wbuf) == 0;
+    if (fused_supported(c->G) && c->kernel != HYDRO_KERNEL_GENERIC) {
+        c->fused_ready = (c->precision == HYDRO_F64 ? configure_marching<double>(c) : configure_marching<float>(c)) == 0;
         if (!c->fused_ready && c->kernel == HYDRO_KERNEL_FUSED)
-            return fail(c, HYDRO_ECUDA, "fused plan: %s", c->fused.err);
+            return fail(c, HYDRO_ECUDA, "marching kernels: %s", c->plan_err);
     }
     return HYDRO_OK;
 }
@@ -447,14 +504,16 @@ int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
 int hydro_set_state(hydro_ctx* c, const void* cons) {
     int rc = need_ws(c);
     if (rc) return rc;
+    DeviceGuard dg(c);
     if (!cons) return HYDRO_EINVAL;
     const dim3 b = blk2d(64, 4);
     const dim3 g = grd(c->G.n[0], c->G.n[1], c->G.n[2], b);
     if (c->precision == HYDRO_F64) pack_kernel<double><<<g, b, 0, c->stream>>>(c->G, (const double*)cons, (double*)c->U[0]);
     else pack_kernel<float><<<g, b, 0, c->stream>>>(c->G, (const float*)cons, (float*)c->U[0]);
     LAUNCHED(c, "pack_kernel");
-    c->w_ready = false;
-    set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, c->t_host, 1);
+    c->w_ready = c->max_ready = false;
+    c->stage_open = 0;
+    set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, 0.0, 0, 1);   // the time is the caller's ("t" option): kept
     LAUNCHED(c, "set_ctl_kernel");
     return HYDRO_OK;
 }
@@ -462,6 +521,7 @@ int hydro_set_state(hydro_ctx* c, const void* cons) {
 int hydro_get_state(hydro_ctx* c, void* out) {
     int rc = need_ws(c);
     if (rc) return rc;
+    DeviceGuard dg(c);
     if (!out) return HYDRO_EINVAL;
     const dim3 b = blk2d(64, 4);
     const dim3 g = grd(c->G.n[0], c->G.n[1], c->G.n[2], b);
@@ -471,11 +531,14 @@ int hydro_get_state(hydro_ctx* c, void* out) {
     return HYDRO_OK;
 }
 
-// Host entry points: stage through the (idle between steps) second RK buffer.
+// Host entry points: stage through the third state buffer, which is idle BETWEEN steps (inside a
+// hydro_step_stage sequence it is a live stage input, so the calls are refused there).
 int hydro_set_state_host(hydro_ctx* c, const void* cons_host) {
     int rc = need_ws(c);
     if (rc) return rc;
+    DeviceGuard dg(c);
     if (!cons_host) return HYDRO_EINVAL;
+    if (c->stage_open) return fail(c, HYDRO_EINVAL, "hydro_set_state_host inside a hydro_step_stage sequence");
     const size_t bytes = (size_t)NF * c->n[0] * c->n[1] * c->n[2] * esize(c);
     CUDA_OK(c, cudaMemcpyAsync(c->U[2], cons_host, bytes, cudaMemcpyHostToDevice, c->stream));
     if ((rc = hydro_set_state(c, c->U[2]))) return rc;
@@ -486,7 +549,9 @@ int hydro_set_state_host(hydro_ctx* c, const void* cons_host) {
 int hydro_get_state_host(hydro_ctx* c, void* out_host) {
     int rc = need_ws(c);
     if (rc) return rc;
+    DeviceGuard dg(c);
     if (!out_host) return HYDRO_EINVAL;
+    if (c->stage_open) return fail(c, HYDRO_EINVAL, "hydro_get_state_host inside a hydro_step_stage sequence");
     const size_t bytes = (size_t)NF * c->n[0] * c->n[1] * c->n[2] * esize(c);
     if ((rc = hydro_get_state(c, c->U[2]))) return rc;
     CUDA_OK(c, cudaMemcpyAsync(out_host, c->U[2], bytes, cudaMemcpyDeviceToHost, c->stream));
@@ -497,7 +562,9 @@ int hydro_get_state_host(hydro_ctx* c, void* out_host) {
 int hydro_step(hydro_ctx* c, double dt, int nsteps) {
     int rc = need_ws(c);
     if (rc) return rc;
+    DeviceGuard dg(c);
     if (!(dt > 0) || nsteps < 0) return fail(c, HYDRO_EINVAL, "hydro_step: dt <= 0 or nsteps < 0");
+    if (c->stage_open) return fail(c, HYDRO_EINVAL, "hydro_step inside a hydro_step_stage sequence");
     for (int s = 0; s < nsteps; ++s) {
         rc = c->precision == HYDRO_F64 ? do_step<double>(c, dt, 0.0) : do_step<float>(c, dt, 0.0);
         if (rc) return rc;
@@ -508,7 +575,9 @@ int hydro_step(hydro_ctx* c, double dt, int nsteps) {
 int hydro_step_cfl(hydro_ctx* c, double cfl, int nsteps) {
     int rc = need_ws(c);
     if (rc) return rc;
+    DeviceGuard dg(c);
     if (!(cfl > 0) || nsteps < 0) return fail(c, HYDRO_EINVAL, "hydro_step_cfl: cfl <= 0 or nsteps < 0");
+    if (c->stage_open) return fail(c, HYDRO_EINVAL, "hydro_step_cfl inside a hydro_step_stage sequence");
     for (int s = 0; s < nsteps; ++s) {
         rc = c->precision == HYDRO_F64 ? do_step<double>(c, -1.0, cfl) : do_step<float>(c, -1.0, cfl);
         if (rc) return rc;
@@ -519,8 +588,9 @@ int hydro_step_cfl(hydro_ctx* c, double cfl, int nsteps) {
 int hydro_max_signal_speed(hydro_ctx* c, double* out_host) {
     int rc = need_ws(c);
     if (rc) return rc;
+    DeviceGuard dg(c);
     if (!out_host) return HYDRO_EINVAL;
-    if (c->w_ready) {   // the stage-3 epilogue of the last step left the max speed of u^n in the control block
+    if (c->max_ready) {   // the stage-3 epilogue of the last step left the max speed of u^n in the control block
         Ctl h0;
         CUDA_OK(c, cudaMemcpyAsync(&h0, c->ctl, sizeof h0, cudaMemcpyDeviceToHost, c->stream));
         CUDA_OK(c, cudaStreamSynchronize(c->stream));
@@ -539,13 +609,16 @@ int hydro_max_signal_speed(hydro_ctx* c, double* out_host) {
     CUDA_OK(c, cudaStreamSynchronize(c->stream));
     memcpy(out_host, &h.maxspeed_bits, sizeof(double));
     // the value stays in the control block: it is the max speed of u^n, which is what the next CFL step needs
+    c->max_ready = true;
     return HYDRO_OK;
 }
 
 int hydro_eval_L(hydro_ctx* c, const void* cons, double t_stage, void* L_out) {
     int rc = need_ws(c);
     if (rc) return rc;
+    DeviceGuard dg(c);
     if (!cons || !L_out) return HYDRO_EINVAL;
+    if (c->stage_open) return fail(c, HYDRO_EINVAL, "hydro_eval_L inside a hydro_step_stage sequence");
     return c->precision == HYDRO_F64 ? eval_L_impl<double>(c, cons, t_stage, L_out)
                                      : eval_L_impl<float>(c, cons, t_stage, L_out);
 }
@@ -558,6 +631,7 @@ size_t hydro_zhalo_elems(const hydro_ctx* c) {
 static int zhalo_impl(hydro_ctx* c, int buffer, int side, void* packed, int put) {
     int rc = need_ws(c);
     if (rc) return rc;
+    DeviceGuard dg(c);
     if (!packed || buffer < 0 || buffer > 2 || (side != 0 && side != 1)) return fail(c, HYDRO_EINVAL, "zhalo: bad argument");
     if (c->G.g[2] == 0) return fail(c, HYDRO_EINVAL, "zhalo: the z axis is inactive");
     const dim3 b = blk2d(64, 4);
@@ -575,7 +649,9 @@ int hydro_put_zhalo(hydro_ctx* c, int buffer, int side, const void* packed_in) {
 int hydro_step_stage(hydro_ctx* c, double dt, int stage) {
     int rc = need_ws(c);
     if (rc) return rc;
+    DeviceGuard dg(c);
     if (!(dt > 0) || stage < 0 || stage > 2) return fail(c, HYDRO_EINVAL, "hydro_step_stage: dt <= 0 or stage not in 0..2");
+    if (stage != c->stage_open) return fail(c, HYDRO_EINVAL, "hydro_step_stage: stage %d out of order (expected %d)", stage, c->stage_open);
     return c->precision == HYDRO_F64 ? do_step_stage<double>(c, stage, dt, 0.0) : do_step_stage<float>(c, stage, dt, 0.0);
 }
 
@@ -598,6 +674,7 @@ int hydro_stage_kernel_time(hydro_ctx* c, double* ms_total_host, long long* laun
 int hydro_get_time(hydro_ctx* c, double* t_host) {
     int rc = need_ws(c);
     if (rc) return rc;
+    DeviceGuard dg(c);
     if (!t_host) return HYDRO_EINVAL;
     Ctl h;
     CUDA_OK(c, cudaMemcpyAsync(&h, c->ctl, sizeof h, cudaMemcpyDeviceToHost, c->stream));
@@ -609,6 +686,7 @@ int hydro_get_time(hydro_ctx* c, double* t_host) {
 int hydro_status(hydro_ctx* c) {
     int rc = need_ws(c);
     if (rc) return rc;
+    DeviceGuard dg(c);
     Ctl h;
     CUDA_OK(c, cudaMemcpyAsync(&h, c->ctl, sizeof h, cudaMemcpyDeviceToHost, c->stream));
     CUDA_OK(c, cudaStreamSynchronize(c->stream));

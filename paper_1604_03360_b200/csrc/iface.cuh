@@ -2,7 +2,7 @@
 //
 // The accessor hides where the stencil lives (global memory in the generic kernel, the shared-memory
 // ring / plane in the fused kernel): acc.u(c, k) is conserved field c of stencil cell k and
-// acc.w(a, k) primitive array a (W_INV, W_P, W_AX + axis), k = 0 .. 2r-1 for cells i-r+1 .. i+r.
+// acc.w(a, k) primitive array a (W_V + axis, W_P, W_AX + axis), k = 0 .. 2r-1 for cells i-r+1 .. i+r.
 #pragma once
 #include "device_math.cuh"
 
@@ -43,7 +43,7 @@ HD void llf_weno_iface(const Acc& acc, T eps, T fh[NF]) {
 #pragma unroll
     for (int k = 0; k < M; ++k) {
         md[k] = acc.u(1 + DIR, k);
-        const T vd = md[k] * acc.w(W_INV, k);
+        const T vd = acc.w(W_V + DIR, k);
         vp[k] = vd + al;
         vm[k] = vd - al;
     }
@@ -81,6 +81,33 @@ HD void llf_weno_iface(const Acc& acc, T eps, T fh[NF]) {
         }
         fh[c] = (T)0.5 * combine_pair(fp[R - 1] + fm[R - 1], Np, Dp, Nm, Dm);
     }
+}
+
+// The same flux for ONE field from first differences (the field-parallel kernels, kernel_fp.cuh).  With F the
+// physical flux of the field and u the field itself, the split fluxes are f+- = F +- alpha u (the factor 1/2 again
+// outside), so their first differences are one fused multiply-add each from the differences of F and of u, which
+// do not depend on the interface and are carried along the marched axis:
+//   f+_{k+1} - f+_k = dF_k + alpha du_k  (cells 0..2r-2),   mirrored f-: f-_{(k)} - f-_{(k+1)} = -dF_k + alpha du_k,
+//   centre values f+_{r-1} + f-_{r} = (F_{r-1} + F_r) - alpha du_{r-1}.
+// dF[k] = F_{k+1} - F_k, du[k] = u_{k+1} - u_k for the 2r-1 pairs of the 2r stencil cells; Fsum = F_{r-1} + F_r.
+// Returns TWICE the interface flux (the caller folds the 1/2 into 1/dx: exact in binary floating point).
+template <class T, int R>
+HD T llf_weno_field2(const T (&dF)[2 * R - 1], const T (&du)[2 * R - 1], T Fsum, T al, T eps) {
+    const T epsx = (R == 3 ? (T)16 : (T)4) * eps;
+    T Np, Dp, Nm, Dm;
+    if (R == 3) {
+        weno5_nd_d(tfma(al, du[0], dF[0]), tfma(al, du[1], dF[1]), tfma(al, du[2], dF[2]), tfma(al, du[3], dF[3]),
+                   epsx, Np, Dp);
+        weno5_nd_d(tfma(al, du[4], -dF[4]), tfma(al, du[3], -dF[3]), tfma(al, du[2], -dF[2]), tfma(al, du[1], -dF[1]),
+                   epsx, Nm, Dm);
+    } else {
+        constexpr int J5 = (R == 4) ? 5 : 0, J6 = (R == 4) ? 6 : 0;   // only read when R == 4
+        weno7_nd_d(tfma(al, du[0], dF[0]), tfma(al, du[1], dF[1]), tfma(al, du[2], dF[2]), tfma(al, du[3], dF[3]),
+                   tfma(al, du[4], dF[4]), tfma(al, du[J5], dF[J5]), epsx, Np, Dp);
+        weno7_nd_d(tfma(al, du[J6], -dF[J6]), tfma(al, du[J5], -dF[J5]), tfma(al, du[4], -dF[4]),
+                   tfma(al, du[3], -dF[3]), tfma(al, du[2], -dF[2]), tfma(al, du[1], -dF[1]), epsx, Nm, Dm);
+    }
+    return combine_pair(tfma(-al, du[R - 1], Fsum), Np, Dp, Nm, Dm);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -2,7 +2,7 @@
 //   (d) halo_fill_kernel    a1: outflow / periodic / analytic Hubble ghost fill, face ghosts only
 //   (a) prim_kernel         a2-a4: con2prim + three signal speeds per padded cell, fused with the
 //                           warp-shuffle / block / atomic max reduction for the CFL time step
-//       max_speed_kernel    a4 alone (interior cells, no stores): hydro_max_signal_speed, MUSTA CFL mode
+//       max_speed_kernel    a4 alone (interior cells, no stores): hydro_max_signal_speed
 //       pack / unpack       interior <-> padded copies for hydro_set_state / hydro_get_state
 //       begin_step / end_step  device-resident dt and t
 #pragma once
@@ -31,22 +31,22 @@ __global__ void end_step_kernel(Ctl* ctl) {
 }
 __global__ void reset_max_kernel(Ctl* ctl) { ctl->maxspeed_bits = 0ull; }
 
-// W = (winv, p, a_x, a_y, a_z) of one cell from its conserved values (a2-a3).  EOS 0: p = e/3; EOS 1: p = p0,
-// whose characteristic speeds are all v_d, so a_d = |v_d|.
+// W = (v_x, v_y, v_z, p, a_x, a_y, a_z) of one cell from its conserved values (a2-a3).  EOS 0: p = e/3; EOS 1:
+// p = p0, whose characteristic speeds are all v_d, so a_d = |v_d|.
 template <class T, int EOS>
 __device__ __forceinline__ void prim_of_cell_t(const T u[NF], T w[NW], int& flag, T p0) {
-    T v2;
+    T v2, winv;
+    if (EOS == 1) con2prim_p0(u[0], u[1], u[2], u[3], p0, winv, w[W_P], v2, flag);
+    else con2prim(u[0], u[1], u[2], u[3], winv, w[W_P], v2, flag);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) w[W_V + d] = u[1 + d] * winv;
     if (EOS == 1) {
-        con2prim_p0(u[0], u[1], u[2], u[3], p0, w[W_INV], w[W_P], v2, flag);
-        w[W_AX + 0] = tabs(u[1] * w[W_INV]);
-        w[W_AX + 1] = tabs(u[2] * w[W_INV]);
-        w[W_AX + 2] = tabs(u[3] * w[W_INV]);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) w[W_AX + d] = tabs(w[W_V + d]);
     } else {
-        con2prim(u[0], u[1], u[2], u[3], w[W_INV], w[W_P], v2, flag);
         const T id = speed_inv_den(v2);
-        w[W_AX + 0] = signal_speed(u[1] * w[W_INV], v2, id);
-        w[W_AX + 1] = signal_speed(u[2] * w[W_INV], v2, id);
-        w[W_AX + 2] = signal_speed(u[3] * w[W_INV], v2, id);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) w[W_AX + d] = signal_speed(w[W_V + d], v2, id);
     }
 }
 struct EosArgs {
@@ -85,35 +85,43 @@ __global__ void unpack_kernel(Geom G, const T* __restrict__ pad, T* __restrict__
 }
 
 // ------------------------------------------------------------------------------------------------
-// (d) halo fill, a1 (reading Q9).  One thread per face-ghost cell; the three axes are independent
-// because only face ghosts exist.  Ghost cells of axis a are enumerated as (q1, l, side, q2) with q1
-// the lower-numbered other axis, so that for the y and z faces consecutive threads run along x.
-// bc: per axis 0 outflow (copy the nearest interior cell), 1 periodic (wrap), 2 analytic Hubble flow
-// at time ctl->t + tfrac * ctl->dt (stage times t, t+dt, t+dt/2, O8).
+// (d) halo fill, a1 (reading Q9).  One thread per face-ghost cell; the three axes are independent because only face
+// ghosts exist.  A ghost cell of axis a is (m, q1, q2): m = 0 .. 2g-1 numbers the ghost coordinates
+// -g .. -1, n .. n+g-1 in increasing order, q1 / q2 are the interior coordinates along the lower / higher of the
+// other two axes; for the y and z faces consecutive threads run along x.
+// bc per axis: 0 outflow (the coordinate is clamped into the interior: every ghost layer repeats the boundary cell),
+// 1 periodic (the coordinate is taken modulo n), 2 analytic Hubble flow at time ctl->t + tfrac * ctl->dt (stage
+// times t, t+dt, t+dt/2, O8), 3 external (z only: the caller wrote the planes, hydro_put_zhalo).
+
+// Closed-form d-dimensional Hubble flow (readings Q13, Q14) in conserved variables, written from the invariants of
+// the flow: with r^2 = sum of x_a^2 over the Hubble axes, tau^2 = t^2 - r^2 and gamma^2 = t^2 / tau^2,
+//   e = e0 q^(2d/3),  n = n0 q^(d/2) exp(-sigma/2),  q = t0^2 / tau^2,  sigma = sum (x_a / (b_a t))^2  (b_a > 0),
+//   E = e (3 t^2 + r^2) / (3 tau^2),  M_a = 4 e t x_a / (3 tau^2),  R = n t / tau.
 template <class T>
-__device__ void hubble_cons(const HubbleParams& H, const int bc[3], int i, int j, int k, double tt, T out[NF]) {
-    const int ix[3] = {i, j, k};
-    double r2 = 0, s = 0, v[3] = {0, 0, 0};
+__device__ void hubble_state(const HubbleParams& H, const int bc[3], const int cell[3], double t, T out[NF]) {
+    double x[3], r2 = 0.0, sigma = 0.0;
     int d = 0;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        if (bc[a] != 2) continue;
-        const double x = H.origin[a] + (ix[a] + 0.5) * H.dx;
-        ++d;
-        r2 += x * x;
-        v[a] = x / tt;
-        if (H.b[a] > 0) s += (x / tt) * (x / tt) / (H.b[a] * H.b[a]);
+        const bool on = bc[a] == 2;
+        x[a] = on ? fma((double)cell[a] + 0.5, H.dx, H.origin[a]) : 0.0;
+        d += on ? 1 : 0;
+        r2 = fma(x[a], x[a], r2);
+        if (on && H.b[a] > 0.0) {
+            const double z = x[a] / (H.b[a] * t);
+            sigma = fma(z, z, sigma);
+        }
     }
-    const double tau = sqrt(tt * tt - r2);
-    const double e = H.e0 * pow(H.t0 / tau, 4.0 * d / 3.0);
-    const double nn = H.n0 * pow(H.t0 / tau, (double)d) * exp(-0.5 * s);
-    const double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
-    const double g2 = 1.0 / (1.0 - v2), p = e / 3.0, w = (e + p) * g2;
-    out[0] = (T)(w - p);
-    out[1] = (T)(w * v[0]);
-    out[2] = (T)(w * v[1]);
-    out[3] = (T)(w * v[2]);
-    out[4] = (T)(nn * sqrt(g2));
+    const double tau2 = t * t - r2, itau2 = 1.0 / tau2;
+    const double q = H.t0 * H.t0 * itau2;
+    const double e = H.e0 * pow(q, (2.0 / 3.0) * d);
+    const double n = H.n0 * pow(q, 0.5 * d) * exp(-0.5 * sigma);
+    const double k = (4.0 / 3.0) * e * t * itau2;
+    out[0] = (T)(e * (3.0 * t * t + r2) * itau2 * (1.0 / 3.0));
+    out[1] = (T)(k * x[0]);
+    out[2] = (T)(k * x[1]);
+    out[3] = (T)(k * x[2]);
+    out[4] = (T)(n * t * sqrt(itau2));
 }
 
 struct HaloArgs {
@@ -134,53 +142,47 @@ __global__ void halo_fill_kernel(Geom G, HaloArgs A, Ctl* ctl, double tfrac, dou
     }
     if (a == 3) return;
     const int a1 = a == 0 ? 1 : 0, a2 = a == 2 ? 1 : 2;  // the other two axes, lower first
-    const int g = G.g[a];
-    int ix[3], src[3];
-    // id = ((q2 * 2 + side) * g + (l-1)) * n[a1] + q1   for y/z faces (q1 = x fastest)
-    // for x faces (a = 0): id = ((q2 * n[a1] + q1) * 2 + side) * g + (l-1)
-    int l, side, q1, q2;
-    if (a == 0) {
-        l = (int)(id % g) + 1; id /= g;
-        side = (int)(id % 2); id /= 2;
+    const int g = G.g[a], n = G.n[a];
+    int m, q1, q2;
+    if (a == 0) {   // x faces: m fastest
+        m = (int)(id % (2 * g)); id /= 2 * g;
         q1 = (int)(id % G.n[a1]); q2 = (int)(id / G.n[a1]);
-    } else {
+    } else {        // y and z faces: x fastest
         q1 = (int)(id % G.n[a1]); id /= G.n[a1];
-        l = (int)(id % g) + 1; id /= g;
-        side = (int)(id % 2); q2 = (int)(id / 2);
+        m = (int)(id % (2 * g)); q2 = (int)(id / (2 * g));
     }
-    ix[a1] = src[a1] = q1;
-    ix[a2] = src[a2] = q2;
-    ix[a] = side == 0 ? -l : G.n[a] - 1 + l;
+    int cell[3];
+    cell[a1] = q1;
+    cell[a2] = q2;
+    cell[a] = m < g ? m - g : n + (m - g);
+    const long long p = G.pidx(cell[0], cell[1], cell[2]);
     T val[NF];
     if (A.bc[a] == 3) {
-        // external ghosts (slab decomposition): the caller put them there (hydro_put_zhalo); only their
-        // primitives may have to be made below
+        // external ghosts (slab decomposition): only their primitives may have to be made below
         if (Wghost == nullptr) return;
-        const long long pg = G.pidx(ix[0], ix[1], ix[2]);
 #pragma unroll
-        for (int c = 0; c < NF; ++c) val[c] = pad[c * G.fs + pg];
-    } else if (A.bc[a] == 2) {
-        const double tt = use_abs ? t_abs : ctl->t + tfrac * ctl->dt;
-        hubble_cons<T>(A.H, A.bc, ix[0], ix[1], ix[2], tt, val);
+        for (int c = 0; c < NF; ++c) val[c] = pad[c * G.fs + p];
     } else {
-        if (A.bc[a] == 1) src[a] = side == 0 ? G.n[a] - l : l - 1;
-        else src[a] = side == 0 ? 0 : G.n[a] - 1;
-        const long long ps = G.pidx(src[0], src[1], src[2]);
+        if (A.bc[a] == 2) {
+            const double tt = use_abs ? t_abs : ctl->t + tfrac * ctl->dt;
+            hubble_state<T>(A.H, A.bc, cell, tt, val);
+        } else {
+            int from[3] = {cell[0], cell[1], cell[2]};
+            from[a] = A.bc[a] == 1 ? ((cell[a] % n) + n) % n : min(max(cell[a], 0), n - 1);
+            const long long ps = G.pidx(from[0], from[1], from[2]);
 #pragma unroll
-        for (int c = 0; c < NF; ++c) val[c] = pad[c * G.fs + ps];
-    }
-    const long long p = G.pidx(ix[0], ix[1], ix[2]);
-    if (A.bc[a] != 3) {
+            for (int c = 0; c < NF; ++c) val[c] = pad[c * G.fs + ps];
+        }
 #pragma unroll
         for (int c = 0; c < NF; ++c) pad[c * G.fs + p] = val[c];
     }
-    // when the interior primitives came from the previous stage's z-sweep epilogue, the ghost cells' are made here
+    // when the interior primitives came from the previous stage's epilogue, the ghost cells' are made here
     if (Wghost != nullptr) {
         T w[NW];
         int flag = 0;
         prim_of_cell(val, w, flag, A.eos);
 #pragma unroll
-        for (int a = 0; a < NW; ++a) Wghost[a * G.fs + p] = w[a];
+        for (int q = 0; q < NW; ++q) Wghost[q * G.fs + p] = w[q];
         if (flag) ctl->flag = 1;
     }
 }

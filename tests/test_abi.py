@@ -67,7 +67,7 @@ def test_workspace_size_follows_the_padded_layout(L, scheme, g):
         sx = -(-(n[0] + 2 * g) // (16 // es)) * (16 // es)
         vol = sx * (n[1] + 2 * g) * (n[2] + 2 * g)
         fs = -(-vol // (256 // es)) * (256 // es)
-        assert L.hydro_workspace_bytes(h) == 256 + 5 * 5 * fs * es
+        assert L.hydro_workspace_bytes(h) == 256 + (3 * 5 + 2 * 7) * fs * es   # three states, two primitive sets
     L.hydro_destroy(h)
 
 

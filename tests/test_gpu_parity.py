@@ -357,20 +357,20 @@ def test_unphysical_state_raises_the_sticky_flag(B, oracle):
 # ------------------------------------------------------------------ kernel variants agree
 @pytest.mark.parametrize("scheme", SCHEMES)
 @pytest.mark.parametrize("prec", [0, 1])
-@pytest.mark.parametrize("split_z,layout", [(1, 0), (1, 1), (0, 0)])
-def test_tiled_and_generic_kernels_agree(B, scheme, prec, split_z, layout):
-    """The tiled stage kernels (x/y tile kernel + z sweep, x/z marching kernel + y sweep, or the single kernel
-    with the z window inside)
-    against the one-thread-per-cell kernel on a grid spanning several tiles and z-chunks with ragged tails
-    in every direction."""
+@pytest.mark.parametrize("chunks", [None, (5, 7), (1, 1)])
+def test_marching_and_generic_kernels_agree(B, scheme, prec, chunks):
+    """The marching stage kernels (field-parallel pair for WENO, five-field pair for MUSTA-FORCE) against the
+    one-thread-per-cell kernel on a grid spanning several x-tiles and march chunks with ragged tails in every
+    direction; short chunks put many chunk seams (window re-prime, pipeline refill, epilogue batches) inside it."""
     w = small_workload(scheme, (150, 37, 29))
-    w.cons = np.ascontiguousarray(np.concatenate([w.cons] * 5, axis=1)[:, :141])   # nz = 141 > two z-chunks
+    w.cons = np.ascontiguousarray(np.concatenate([w.cons] * 5, axis=1)[:, :141])   # nz = 141 > one default z-chunk
     w.n = (150, 37, 141)
     outs = []
     for kern in (B.KERNEL_GENERIC, B.KERNEL_FUSED):
         h = B.from_workload(w, precision=prec, kernel=kern)
-        h.set_option("split_z", split_z)
-        h.set_option("layout", layout)
+        if chunks is not None:
+            h.set_option("tile_zc", chunks[0])
+            h.set_option("sweep_zc", chunks[1])
         h.step_cfl(0.2, 3)
         outs.append(h.get_state().cpu().numpy())
         assert h.status() == 0
