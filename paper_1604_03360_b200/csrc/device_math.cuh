@@ -195,9 +195,9 @@ HD T speed_inv_den(T v2) { return fast_rcp(tfma(v2, (T)(-1.0 / 3.0), (T)1)); }
 // Cross-multiplied weights need the products prod_{j != k} B_j^2 (B^4 for WENO5, B^6 for WENO7) to stay inside the
 // normal range.  fp64: they do for |data| < 1e25 (documented in include/hydro.h).  fp32: flux jumps of order 1e3
 // overflow B^6 and a tiny epsilon on flat data underflows it, so the B_k are first multiplied by the power of two
-// that brings the smallest of them to [1, 2) (exact, and it cancels in N/D) and clamped at 2^18: a sub-stencil
-// whose indicator is 2^18 times the smallest carries a weight below 2^-36 of the dominant one either way, far
-// under fp32 resolution; the products then stay below 2^108, which leaves room for the factors g_k of N.
+// that brings the smallest of them to [1, 2) (exact, and it cancels in N/D) and clamped at 2^17 (WENO7; 2^25 for
+// WENO5): a sub-stencil whose indicator is 2^17 times the smallest carries a weight below 2^-34 of the dominant one
+// either way, far under fp32 resolution; the products then stay below 2^102, which leaves room for the factors g_k.
 template <class T, int NB>
 HD void normalise_indicators(T (&B)[NB]) {}
 #ifdef __CUDA_ARCH__
@@ -205,7 +205,8 @@ template <>
 __device__ __forceinline__ void normalise_indicators<float, 3>(float (&B)[3]) {
     const float m = fminf(B[0], fminf(B[1], B[2]));
     const float s = __int_as_float(0x7f000000 - (__float_as_int(m) & 0x7f800000));   // 2^(127 - exponent(m)) / 2^0
-    const float cap = 262144.0f;
+    // WENO5 takes B only to the 4th power: the clamp can sit at 2^25 (products below 2^100)
+    const float cap = 33554432.0f;   // 2^25
 #pragma unroll
     for (int k = 0; k < 3; ++k) B[k] = fminf(B[k] * s, cap);
 }
@@ -213,7 +214,7 @@ template <>
 __device__ __forceinline__ void normalise_indicators<float, 4>(float (&B)[4]) {
     const float m = fminf(fminf(B[0], B[1]), fminf(B[2], B[3]));
     const float s = __int_as_float(0x7f000000 - (__float_as_int(m) & 0x7f800000));
-    const float cap = 262144.0f;
+    const float cap = 131072.0f;     // 2^17
 #pragma unroll
     for (int k = 0; k < 4; ++k) B[k] = fminf(B[k] * s, cap);
 }
@@ -227,11 +228,14 @@ HD void weno5_nd_d(T D1, T D2, T D3, T D4, T eps4, T& N, T& D) {
     const T u0 = tfma((T)3, D2, -D1);                      // a - 4b + 3c
     const T u1 = D2 + D3;                                  // d - b
     const T u2 = tfma((T)-3, D3, D4);                      // 3c - 4d + e, sign irrelevant (squared)
-    const T k = (T)(13.0 / 3.0);
+    // (13/3) t^2 as the square of sqrt(13/3) t: a fused multiply-add with a repeated operand reads two registers
+    // instead of three and issues in 2 cycles instead of 3
+    const T rk = (T)2.0816659994661327353;   // sqrt(13/3)
+    const T s0_ = rk * t0, s1_ = rk * t1, s2_ = rk * t2;
     T B[3];
-    B[0] = tfma(k * t0, t0, tfma(u0, u0, eps4));
-    B[1] = tfma(k * t1, t1, tfma(u1, u1, eps4));
-    B[2] = tfma(k * t2, t2, tfma(u2, u2, eps4));
+    B[0] = tfma(s0_, s0_, tfma(u0, u0, eps4));
+    B[1] = tfma(s1_, s1_, tfma(u1, u1, eps4));
+    B[2] = tfma(s2_, s2_, tfma(u2, u2, eps4));
     normalise_indicators<T, 3>(B);
     const T s0 = B[0] * B[0], s1 = B[1] * B[1], s2 = B[2] * B[2];
     const T P0 = s1 * s2, P1 = s0 * s2, P2 = s0 * s1;
@@ -265,17 +269,20 @@ HD void weno7_nd_d(T E1, T E2, T E3, T E4, T E5, T E6, T eps, T& N, T& D) {
     //   k=1: c3 = T2/6, c2 = S3/2,        c1 + c3/4 = (E3 + E4)/2 - T2/6
     //   k=2: c3 = T3/6, c2 = S3/2,        c1 + c3/4 = (E3 + E4)/2 - T3/6
     //   k=3: c3 = T4/6, c2 = (S4 - T4)/2, c1 + c3/4 = E4 - S4/2 + T4/3
-    const T k13 = (T)(13.0 / 3.0), k781 = (T)(781.0 / 20.0);
-    const T sixth = (T)(1.0 / 6.0);
-    const T c3_0 = T1 * sixth, c2_0 = (T)0.5 * (S2 + T1), m_0 = E3 + tfma((T)0.5, S2, (T)(1.0 / 3.0) * T1);
-    const T c3_1 = T2 * sixth, c2_1 = (T)0.5 * S3, m_1 = tfma((T)(-1.0 / 6.0), T2, (T)0.5 * (E3 + E4));
-    const T c3_2 = T3 * sixth, c2_2 = (T)0.5 * S3, m_2 = tfma((T)(-1.0 / 6.0), T3, (T)0.5 * (E3 + E4));
-    const T c3_3 = T4 * sixth, c2_3 = (T)0.5 * (S4 - T4), m_3 = E4 + tfma((T)-0.5, S4, (T)(1.0 / 3.0) * T4);
+    // the factors 13/3 and 781/20 go into the coefficients as their square roots, so that every term of an
+    // indicator is the square of ONE value: a fused multiply-add with a repeated operand reads two registers
+    // instead of three and issues in 2 cycles instead of 3
+    const T r13 = (T)2.0816659994661327353, r781 = (T)6.2489999199871975245;   // sqrt(13/3), sqrt(781/20)
+    const T c3s = r781 * (T)(1.0 / 6.0), c2s = r13 * (T)0.5;
+    const T c3_0 = T1 * c3s, c2_0 = c2s * (S2 + T1), m_0 = E3 + tfma((T)0.5, S2, (T)(1.0 / 3.0) * T1);
+    const T c3_1 = T2 * c3s, c2_1 = c2s * S3, m_1 = tfma((T)(-1.0 / 6.0), T2, (T)0.5 * (E3 + E4));
+    const T c3_2 = T3 * c3s, c2_2 = c2_1, m_2 = tfma((T)(-1.0 / 6.0), T3, (T)0.5 * (E3 + E4));
+    const T c3_3 = T4 * c3s, c2_3 = c2s * (S4 - T4), m_3 = E4 + tfma((T)-0.5, S4, (T)(1.0 / 3.0) * T4);
     T B[4];
-    B[0] = tfma(m_0, m_0, tfma(k13 * c2_0, c2_0, tfma(k781 * c3_0, c3_0, eps)));
-    B[1] = tfma(m_1, m_1, tfma(k13 * c2_1, c2_1, tfma(k781 * c3_1, c3_1, eps)));
-    B[2] = tfma(m_2, m_2, tfma(k13 * c2_2, c2_2, tfma(k781 * c3_2, c3_2, eps)));
-    B[3] = tfma(m_3, m_3, tfma(k13 * c2_3, c2_3, tfma(k781 * c3_3, c3_3, eps)));
+    B[0] = tfma(m_0, m_0, tfma(c2_0, c2_0, tfma(c3_0, c3_0, eps)));
+    B[1] = tfma(m_1, m_1, tfma(c2_1, c2_1, tfma(c3_1, c3_1, eps)));
+    B[2] = tfma(m_2, m_2, tfma(c2_2, c2_2, tfma(c3_2, c3_2, eps)));
+    B[3] = tfma(m_3, m_3, tfma(c2_3, c2_3, tfma(c3_3, c3_3, eps)));
     normalise_indicators<T, 4>(B);
     const T s0 = B[0] * B[0], s1 = B[1] * B[1], s2 = B[2] * B[2], s3 = B[3] * B[3];
     const T s01 = s0 * s1, s23 = s2 * s3;

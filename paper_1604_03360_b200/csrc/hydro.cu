@@ -13,7 +13,7 @@
 
 #include "../../include/hydro.h"
 #include "grid.cuh"
-#include "kernel_fp.cuh"
+#include "kernel_weno.cuh"
 #include "kernel_generic.cuh"
 #include "kernel_musta.cuh"
 #include "kernels_aux.cuh"
@@ -202,8 +202,8 @@ bool want_fused(const hydro_ctx* c) {
 template <class T>
 int configure_marching(hydro_ctx* c) {
     switch (c->scheme) {
-        case HYDRO_WENO5: return configure_fp<T, 3>(c->plan_err, sizeof c->plan_err);
-        case HYDRO_WENO7: return configure_fp<T, 4>(c->plan_err, sizeof c->plan_err);
+        case HYDRO_WENO5: return configure_weno<T, 3>(c->plan_err, sizeof c->plan_err);
+        case HYDRO_WENO7: return configure_weno<T, 4>(c->plan_err, sizeof c->plan_err);
         default: return configure_musta<T>(c->plan_err, sizeof c->plan_err);
     }
 }
@@ -224,11 +224,10 @@ struct StageTimer {
     }
 };
 
-// One stage: Uout = ca u^n + cb (Us + dt L(Us)), or L(Us) itself (mode 1).  Pbuf: scratch state buffer for the
-// partial result of the field-parallel pair (may be Uout unless Uout is u^n).
+// One stage: Uout = ca u^n + cb (Us + dt L(Us)), or L(Us) itself (mode 1).
 template <class T>
-int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, T* Pbuf, double ca, double cb, int mode,
-             T* Wnext = nullptr, int epi_max = 0) {
+int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double cb, int mode, T* Wnext = nullptr,
+             int epi_max = 0) {
     StageArgs A = stage_args(c, ca, cb, mode);
     A.epi_max = epi_max;
     StageTimer timer(c);
@@ -240,11 +239,11 @@ int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, T* Pbuf, double ca
             rc = launch_musta<T>(c->G, A, Us, Un, Uout, c->ctl, c->zc > 0 ? c->zc : 64, c->yc > 0 ? c->yc : 128,
                                  c->stream, &nl, c->plan_err, sizeof c->plan_err);
         else if (c->scheme == HYDRO_WENO5)
-            rc = launch_fp<T, 3>(c->G, A, Us, W, Un, Uout, Pbuf, Wnext, c->ctl, c->zc > 0 ? c->zc : FP_ZC,
-                                 c->yc > 0 ? c->yc : FP_YC, c->stream, &nl, c->plan_err, sizeof c->plan_err);
+            rc = launch_weno<T, 3>(c->G, A, Us, W, Un, Uout, Wnext, c->ctl, c->zc > 0 ? c->zc : WENO_ZC,
+                                   c->yc > 0 ? c->yc : WENO_YC, c->stream, &nl, c->plan_err, sizeof c->plan_err);
         else
-            rc = launch_fp<T, 4>(c->G, A, Us, W, Un, Uout, Pbuf, Wnext, c->ctl, c->zc > 0 ? c->zc : FP_ZC,
-                                 c->yc > 0 ? c->yc : FP_YC, c->stream, &nl, c->plan_err, sizeof c->plan_err);
+            rc = launch_weno<T, 4>(c->G, A, Us, W, Un, Uout, Wnext, c->ctl, c->zc > 0 ? c->zc : WENO_ZC,
+                                   c->yc > 0 ? c->yc : WENO_YC, c->stream, &nl, c->plan_err, sizeof c->plan_err);
         if (rc != 0) return fail(c, HYDRO_ECUDA, "stage launch: %s", c->plan_err);
         c->launches += nl;
         return HYDRO_OK;
@@ -280,7 +279,6 @@ int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl) {
     const double ca[3] = {0.0, 0.75, 1.0 / 3.0}, cb[3] = {1.0, 0.25, 2.0 / 3.0};
     T* const in[3] = {U[0], U[1], U[2]};
     T* const out[3] = {U[1], U[2], U[0]};   // stage 3 writes u^n in place: each cell reads only its own u^n
-    T* const scratch[3] = {U[1], U[2], U[1]};   // partial result of the field-parallel pair; U[1] is free in stage 3
     int rc;
     const bool have_w = c->w_ready;   // interior primitives of in[s] already in Wb[wcur] (previous stage's epilogue)
     if ((rc = do_halo<T>(c, in[s], tfrac[s], false, 0.0, (weno && have_w) ? (T*)c->Wb[c->wcur] : nullptr))) return rc;
@@ -300,8 +298,7 @@ int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl) {
         c->max_ready = false;
     }
     T* Wnext = epi ? (T*)c->Wb[c->wcur ^ 1] : nullptr;
-    if ((rc = do_stage<T>(c, in[s], U[0], out[s], scratch[s], ca[s], cb[s], 0, Wnext, (marching && s == 2) ? 1 : 0)))
-        return rc;
+    if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, Wnext, (marching && s == 2) ? 1 : 0))) return rc;
     if (epi) c->wcur ^= 1;
     c->w_ready = epi;
     if (s == 2) {
@@ -354,7 +351,7 @@ int eval_L_impl(hydro_ctx* c, const void* cons, double t_stage, void* L_out) {
     LAUNCHED(c, "pack_kernel");
     if ((rc = do_halo<T>(c, U1, 0.0, true, t_stage))) return rc;
     if (c->scheme != HYDRO_MUSTA_FORCE && (rc = do_prim<T>(c, U1, 0))) return rc;
-    if ((rc = do_stage<T>(c, U1, U1, U2, U2, 0.0, 1.0, 1))) return rc;
+    if ((rc = do_stage<T>(c, U1, U1, U2, 0.0, 1.0, 1))) return rc;
     unpack_kernel<T><<<g, b, 0, c->stream>>>(c->G, U2, (T*)L_out);
     LAUNCHED(c, "unpack_kernel");
     return HYDRO_OK;

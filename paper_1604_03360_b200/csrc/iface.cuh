@@ -24,6 +24,15 @@ HD T combine_pair(T centre, T Np, T Dp, T Nm, T Dm) {
     }
 }
 
+// alpha as the plain maximum of a_DIR over the 2r stencil cells of an accessor with w(W_AX + DIR, k)
+template <class T, int M, int DIR, class Acc>
+HD T alpha_of_cells(const Acc& acc) {
+    T al = acc.w(W_AX + DIR, 0);
+#pragma unroll
+    for (int k = 1; k < M; ++k) al = max_nonneg(al, acc.w(W_AX + DIR, k));
+    return al;
+}
+
 // a5-a7. Component-wise local Lax-Friedrichs flux with WENO_r reconstruction at interface i+1/2 along
 // axis DIR (O5, reading Q3):
 //   alpha = max_k a_d(k);  f+-_k = (F_d(u_k) +- alpha u_k)/2;
@@ -32,14 +41,15 @@ HD T combine_pair(T centre, T Np, T Dp, T Nm, T Dm) {
 // scaled with the square of the data, WENO_eps(g/2) = WENO_{4 eps}(g)/2, exactly in binary floating
 // point.  With v_d = M_d * winv the split fluxes are u (v_d +- alpha) for the fields that are simply
 // advected (M_j, j != d, and R), M_d (v_d +- alpha) + p for j = d, and M_d +- alpha E for E.
+// Returns TWICE the interface flux: the caller folds the 1/2 into its 1/dx factor (exact in binary floating point).
+// alpha comes from the accessor (acc.alpha<DIR, 2r>()): a stencil in registers carries pair maxima, the others take the
+// maximum of the 2r values.
 template <class T, int R, int DIR, class Acc>
-HD void llf_weno_iface(const Acc& acc, T eps, T fh[NF]) {
+HD void llf_weno_iface2(const Acc& acc, T eps, T fh[NF]) {
     constexpr int M = 2 * R;
     constexpr int I5 = (R == 4) ? 5 : 3, I6 = (R == 4) ? 6 : 4;  // only read when R == 4
     T md[M], vp[M], vm[M];
-    T al = acc.w(W_AX + DIR, 0);
-#pragma unroll
-    for (int k = 1; k < M; ++k) al = max_nonneg(al, acc.w(W_AX + DIR, k));
+    const T al = acc.template alpha<DIR, M>();
 #pragma unroll
     for (int k = 0; k < M; ++k) {
         md[k] = acc.u(1 + DIR, k);
@@ -79,10 +89,9 @@ HD void llf_weno_iface(const Acc& acc, T eps, T fh[NF]) {
             weno7_nd(fp[0], fp[1], fp[2], fp[3], fp[4], fp[I5], fp[I6], epsx, Np, Dp);
             weno7_nd(fm[0], fm[1], fm[2], fm[3], fm[4], fm[I5], fm[I6], epsx, Nm, Dm);
         }
-        fh[c] = (T)0.5 * combine_pair(fp[R - 1] + fm[R - 1], Np, Dp, Nm, Dm);
+        fh[c] = combine_pair(fp[R - 1] + fm[R - 1], Np, Dp, Nm, Dm);
     }
 }
-
 // The same flux for ONE field from first differences (the field-parallel kernels, kernel_fp.cuh).  With F the
 // physical flux of the field and u the field itself, the split fluxes are f+- = F +- alpha u (the factor 1/2 again
 // outside), so their first differences are one fused multiply-add each from the differences of F and of u, which

@@ -17,6 +17,8 @@ struct GlobalAcc {  // stencil cell k lives at base + k*stride; field c at + c*f
     long long fs, stride;
     __device__ __forceinline__ T u(int c, int k) const { return __ldg(ub + c * fs + k * stride); }
     __device__ __forceinline__ T w(int a, int k) const { return __ldg(wb + a * fs + k * stride); }
+    template <int DIR, int M>
+    __device__ __forceinline__ T alpha() const { return alpha_of_cells<T, M, DIR>(*this); }
 };
 
 struct StageArgs {
@@ -39,7 +41,11 @@ __device__ __forceinline__ void iface_generic(const Geom& G, const StageArgs& A,
     constexpr int R = SCHEME == 0 ? 3 : (SCHEME == 1 ? 4 : 2);
     GlobalAcc<T> acc{U + p - (R - 1) * stride, W + p - (R - 1) * stride, G.fs, stride};
     if constexpr (SCHEME == 2) musta_force_iface<T, DIR>(acc, A.musta_K, (T)A.musta_C, A.limiter, A.eos.kind, (T)A.eos.p0, fh, flag);
-    else llf_weno_iface<T, R, DIR>(acc, (T)A.eps, fh);
+    else {
+        llf_weno_iface2<T, R, DIR>(acc, (T)A.eps, fh);   // twice the flux
+#pragma unroll
+        for (int c = 0; c < NF; ++c) fh[c] *= (T)0.5;
+    }
 }
 
 template <class T, int SCHEME, int DIR>

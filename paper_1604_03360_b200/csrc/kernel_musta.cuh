@@ -217,11 +217,13 @@ musta_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl,
     T* park = sm + D * NVO * TH + tid;
     const int i = blockIdx.x * 32 + threadIdx.x;
     const int kz = blockIdx.y * MUSTA_ROWS + threadIdx.y;
-    const bool active = i < G.n[0] && kz < G.n[2];          // idle threads follow along on a clamped column
+    // lanes beyond the grid leave; the ballot (taken while the warp is whole) is the mask of the final reduction
+    const unsigned wmask = __ballot_sync(0xffffffffu, i < G.n[0] && kz < G.n[2]);
+    if (i >= G.n[0] || kz >= G.n[2]) return;
     const long long ms = G.sx;
     const int j0 = (int)blockIdx.z * yc;
     const int j1 = min(j0 + yc, G.n[1]);
-    const long long p0 = G.pidx(min(i, G.n[0] - 1), j0, min(kz, G.n[2] - 1));
+    const long long p0 = G.pidx(i, j0, kz);
     int flag = 0;
     auto issue = [&](int j) {
         if (j < j1) {
@@ -267,18 +269,18 @@ musta_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl,
 #pragma unroll
         for (int c = 0; c < NF; ++c) {
             o[c] = tfma(coef, park[c * TH] - f[c], src[(NF + c) * TH]);   // old output: read late
-            if (active) Uout[c * G.fs + q] = o[c];
+            Uout[c * G.fs + q] = o[c];
             park[c * TH] = f[c];
         }
         issue(j + D);             // refill the slot just consumed
         if (EPI) {   // a4 of the finished cell (all three axes are active whenever this kernel runs)
             T w[NW];
             prim_of_cell(o, w, flag, A.eos);
-            if (active) amax = fmax(amax, fmax((double)w[W_AX], fmax((double)w[W_AX + 1], (double)w[W_AX + 2])));
+            amax = fmax(amax, fmax((double)w[W_AX], fmax((double)w[W_AX + 1], (double)w[W_AX + 2])));
         }
     }
-    if (EPI) warp_max_to(amax, &ctl->maxspeed_next_bits);
-    if (flag && active) ctl->flag = 1;
+    if (EPI) warp_max_to(amax, &ctl->maxspeed_next_bits, wmask);
+    if (flag) ctl->flag = 1;
 }
 
 template <class T>

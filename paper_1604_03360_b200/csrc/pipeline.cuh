@@ -15,6 +15,11 @@ template <int BYTES>
 __device__ __forceinline__ void cp_async(void* smem, const void* gmem) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(smem_u32(smem)), "l"(gmem), "n"(BYTES) : "memory");
 }
+// the same with the shared-memory address already converted (keeps the generic -> shared conversion out of loops)
+template <int BYTES>
+__device__ __forceinline__ void cp_async_s(unsigned smem_addr, const void* gmem) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(smem_addr), "l"(gmem), "n"(BYTES) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
@@ -22,11 +27,19 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 template <class T>
 __device__ __forceinline__ T shfl_up1(T v) { return __shfl_up_sync(0xffffffffu, v, 1); }
 
-// warp-wide max of a non-negative double (all 32 lanes must call), pushed to *bits by lane 0
-__device__ __forceinline__ void warp_max_to(double m, unsigned long long* bits) {
+// warp-wide max of a non-negative double over the lanes of `mask` (a ballot taken while all 32 lanes were still
+// present: lanes outside it have exited), pushed to *bits by the lowest lane of the mask.  The butterfly runs over
+// all five offsets; a partner outside the mask contributes nothing.
+__device__ __forceinline__ void warp_max_to(double m, unsigned long long* bits, unsigned mask = 0xffffffffu) {
+    const unsigned lane = threadIdx.x & 31;
+    __syncwarp(mask);
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
-    if ((threadIdx.x & 31) == 0 && m > 0.0) atomicMax(bits, (unsigned long long)__double_as_longlong(m));
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned partner = lane ^ o;
+        const unsigned src = (mask >> partner) & 1u ? partner : lane;   // own value when the partner is gone
+        m = fmax(m, __shfl_sync(mask, m, src));
+    }
+    if (lane == (unsigned)(__ffs(mask) - 1) && m > 0.0) atomicMax(bits, (unsigned long long)__double_as_longlong(m));
 }
 
 }  // namespace hydro

@@ -150,52 +150,52 @@ def test_two_dimensional_hubble_flow(oracle):
     assert abs(errs[(True, True, False)] - errs[(False, True, True)]) < 1e-13
 
 
-@pytest.fixture(scope="module")
-def config2_errors(oracle):
-    out = {}
-    for scheme in (W.WENO5, W.WENO7):
-        w = W.hubble(n=24, scheme=scheme, nsteps=12)
-        o = oracle.from_workload(w)
-        oracle.run(o, w)
-        c = W.cell_centres(24, w.dx, -4.0)
-        e, n, vx, vy, vz = W.hubble_fields(c[None, None, :], c[None, :, None], c[:, None, None], o.time, 8.0, 1.0, 1.0)
-        exact = W.prim_to_cons(e, n, vx, vy, vz)
-        u = o.get_state()
-        out[scheme] = (np.max(np.abs(u[0] - exact[0]) / exact[0]), np.max(np.abs(u - exact)), o.time)
-    return out
+def _hubble3d_errors(oracle, w, t0, b, half, inner_half):
+    """(max rel error of E on the whole box, on the inner box, mean rel error of E, max error of R / max R inner)."""
+    o = oracle.from_workload(w)
+    oracle.run(o, w)
+    n = w.n[0]
+    c = W.cell_centres(n, w.dx, -half)
+    e, nn, vx, vy, vz = W.hubble_fields(c[None, None, :], c[None, :, None], c[:, None, None], o.time, t0, 1.0, 1.0, b=b)
+    exact = W.prim_to_cons(e, nn, vx, vy, vz)
+    u = o.get_state()
+    rel = np.abs(u[0] - exact[0]) / exact[0]
+    inner = np.abs(c) <= inner_half
+    sel = np.ix_(inner, inner, inner)
+    return rel.max(), rel[sel].max(), rel.mean(), np.max(np.abs(u[4] - exact[4])[sel]) / np.max(exact[4]), o.time
 
 
-def test_config2_reduced_against_the_closed_form(config2_errors):
-    """BASELINE configs[1] at 24^3 (same box, t0 = 8, dt = 0.1 dx, analytic ghosts): d = 3, e ~ tau^-4."""
-    rel5, abs5, t = config2_errors[W.WENO5]
-    assert abs(t - (8.0 + 12 * 0.1 * 8.0 / 24)) < 1e-12
-    assert rel5 < 1.5 * 1.5e-3, rel5           # measured 1.5e-3 relative in E at 24 cells per axis
-    rel7, abs7, _ = config2_errors[W.WENO7]
-    assert rel7 <= rel5                        # PAPER.md:50 "higher order simulations were slightly more accurate"
+def test_config2_reduced_against_the_closed_form(oracle):
+    """BASELINE configs[1] at 24^3 (same box, t0 = 8, dt = 0.1 dx, analytic ghosts): d = 3, e ~ tau^-4.  Thresholds
+    are 1.5x the oracle's measured errors (E, relative: WENO5 1.36e-3, WENO7 3.85e-3 at the corners, where |v| = 0.87
+    and 24 cells per axis do not resolve tau^-4; 2.1e-5 and 3.1e-7 on |x_i| <= 2)."""
+    r5 = _hubble3d_errors(oracle, W.hubble(n=24, scheme=W.WENO5, nsteps=12), 8.0, (0, 0, 0), 4.0, 2.0)
+    r7 = _hubble3d_errors(oracle, W.hubble(n=24, scheme=W.WENO7, nsteps=12), 8.0, (0, 0, 0), 4.0, 2.0)
+    assert abs(r5[4] - (8.0 + 12 * 0.1 * 8.0 / 24)) < 1e-12
+    assert 0.3 * 1.36e-3 < r5[0] < 1.5 * 1.36e-3 and r5[1] < 1.5 * 2.13e-5, r5
+    assert r7[0] < 1.5 * 3.85e-3 and r7[1] < 1.5 * 3.1e-7, r7
+    # PAPER.md:50 "higher order simulations were slightly more accurate": where the flow is resolved, and on average
+    assert r7[1] < r5[1] and r7[2] < r5[2]
 
 
 @pytest.mark.parametrize("bc", [W.BC_HUBBLE, W.BC_OUTFLOW])
 def test_config3_reduced_against_the_closed_form(oracle, bc):
-    """BASELINE configs[2] at 24^3 (reading Q14: Hubble velocity field with the ellipsoidal charge profile): with the
-    analytic fill everywhere, and with the config's zero-gradient outflow on the part of the box the boundary cannot
-    have reached.  Pins the exp(-sigma/2) factor of the charge."""
-    errs = {}
+    """BASELINE configs[2] at 24^3 (reading Q14: Hubble velocity field with the ellipsoidal charge profile, t0 = 12):
+    with the analytic fill everywhere, and with the config's zero-gradient outflow on the part of the box the
+    boundary cannot have reached in 6 steps.  Pins the exp(-sigma/2) factor of the charge."""
+    res = {}
     for scheme in (W.WENO5, W.WENO7):
         w = W.ellipsoidal(n=24, scheme=scheme, nsteps=6, bc=bc)
         w.cfl, w.dt = None, 0.1 * w.dx
-        o = oracle.from_workload(w)
-        oracle.run(o, w)
-        c = W.cell_centres(24, w.dx, -6.0)
-        e, n, vx, vy, vz = W.hubble_fields(c[None, None, :], c[None, :, None], c[:, None, None], o.time, 12.0, 1.0, 1.0,
-                                           b=W.ELLIPSOID_B)
-        exact = W.prim_to_cons(e, n, vx, vy, vz)
-        u = o.get_state()
-        inner = np.abs(c) <= (6.0 if bc == W.BC_HUBBLE else 2.0)
-        sel = np.ix_(range(5), inner, inner, inner)
-        errs[scheme] = (np.max(np.abs(u[sel][0] - exact[sel][0]) / exact[sel][0]),
-                        np.max(np.abs(u[sel][4] - exact[sel][4])) / np.max(exact[4]))
-    assert errs[W.WENO5][0] < 3e-4 and errs[W.WENO5][1] < 2e-2, errs
-    assert errs[W.WENO7][0] <= errs[W.WENO5][0] * 1.05 and errs[W.WENO7][1] <= errs[W.WENO5][1] * 1.05, errs
+        res[scheme] = _hubble3d_errors(oracle, w, 12.0, W.ELLIPSOID_B, 6.0, 2.0)
+    r5, r7 = res[W.WENO5], res[W.WENO7]
+    # measured on |x_i| <= 2: E 5.1e-6 (WENO5), 7e-8 (WENO7); R 5.8e-6, 4.9e-7 of max R
+    assert r5[1] < 1.5 * 5.1e-6 and r5[3] < 1.5 * 5.8e-6, r5
+    assert r7[1] < 1.5 * 7.1e-8 and r7[3] < 1.5 * 4.9e-7, r7
+    if bc == W.BC_HUBBLE:   # whole box: 6.2e-4 / 2.2e-3 at the corners
+        assert 0.3 * 6.2e-4 < r5[0] < 1.5 * 6.2e-4 and r7[0] < 1.5 * 2.2e-3, (r5, r7)
+    else:                   # the zero-gradient boundary is wrong by O(1) for this flow, and must be seen to be
+        assert r5[0] > 0.05
 
 
 # ------------------------------------------------------------------ (b) the zero-gradient outflow rule (Q9)
@@ -252,7 +252,7 @@ def test_musta_force_flux_with_different_velocities_on_the_two_sides(oracle, d):
     pl, _ = oracle.con2prim(UL)
     pr, _ = oracle.con2prim(UR)
     aL, aR = oracle.signal_speed(pl[3:6], d), oracle.signal_speed(pr[3:6], d)
-    assert abs(aL - aR) > 0.2                                                  # max and min really differ
+    assert abs(aL - aR) > 0.15                                                 # max and min really differ
     f1, FL, FR, tau = _force_flux(oracle, UL, UR, d, 0.9)
     got1 = oracle.musta_force_flux(cells, d, K=1, C=0.9)
     assert np.max(np.abs(got1 - f1)) <= 4e-15 * np.max(np.abs(f1))
@@ -287,18 +287,19 @@ def _advect_error(oracle, scheme, n, axis, t_end, dt):
     return np.sum(np.abs(out[4] - exact)) / n
 
 
-@pytest.mark.parametrize("scheme,lo,hi", [(W.WENO5, 4.7, 5.6), (W.WENO7, 6.5, 8.0), (W.MUSTA_FORCE, 1.7, 2.6)])
-def test_charge_advection_has_the_stated_order(oracle, scheme, lo, hi):
+@pytest.mark.parametrize("scheme,lo,hi,n1,n2", [(W.WENO5, 4.6, 5.5, 32, 64), (W.WENO7, 6.5, 8.3, 32, 48),
+                                                 (W.MUSTA_FORCE, 1.6, 2.4, 80, 160)])
+def test_charge_advection_has_the_stated_order(oracle, scheme, lo, hi, n1, n2):
     """PAPER.md:7 "second (MUSTA-FORCE), fifth and seventh (WENO) order of accuracy": L1 error of the advected
-    charge at two resolutions, with a time step small enough that the RK3 error does not mask the spatial one."""
-    n1, n2 = (20, 40) if scheme != W.WENO7 else (16, 32)
+    charge at two resolutions, with a time step small enough that the RK3 error does not mask the spatial one
+    (measured 5.04 / 7.48 / 1.80)."""
     t_end = 0.25
     errs = []
     for n in (n1, n2):
         p = {W.WENO5: 5.0, W.WENO7: 7.0, W.MUSTA_FORCE: 2.0}[scheme]
         dt = 0.3 * (1.0 / n) ** (p / 3.0) / 4.0 if scheme != W.MUSTA_FORCE else 0.2 / n
         errs.append(_advect_error(oracle, scheme, n, 0, t_end, dt))
-    order = math.log2(errs[0] / errs[1])
+    order = math.log(errs[0] / errs[1]) / math.log(n2 / n1)
     assert lo < order < hi, (errs, order)
 
 
@@ -419,4 +420,6 @@ def test_q16_clamp_values(oracle):
     assert np.allclose(bad[3:6] / np.linalg.norm(bad[3:6]), Mdir, atol=1e-12)
     assert abs(bad[0] - ref[0]) <= 1e-3 * abs(ref[0]) + 1e-14 and 0 < bad[0] < 1e-10 * E
     low, flag = oracle.con2prim(np.array([0.0, 0.0, 0.0, 0.0, 0.0]))
-    assert flag == 1 and abs(low[0] - 1e-300) < 1e-310 and np.all(low[3:6] == 0.0)
+    assert flag == 1 and 0.0 <= low[0] <= 1e-300 and np.all(low[3:6] == 0.0)       # E raised to the floor, fluid at rest
+    neg, flag = oracle.con2prim(np.array([-1.0, 0.1, 0.0, 0.0, 1.0]))
+    assert flag == 1                                                               # a negative energy is flagged
