@@ -92,33 +92,6 @@ HD void llf_weno_iface2(const Acc& acc, T eps, T fh[NF]) {
         fh[c] = combine_pair(fp[R - 1] + fm[R - 1], Np, Dp, Nm, Dm);
     }
 }
-// The same flux for ONE field from first differences (the field-parallel kernels, kernel_fp.cuh).  With F the
-// physical flux of the field and u the field itself, the split fluxes are f+- = F +- alpha u (the factor 1/2 again
-// outside), so their first differences are one fused multiply-add each from the differences of F and of u, which
-// do not depend on the interface and are carried along the marched axis:
-//   f+_{k+1} - f+_k = dF_k + alpha du_k  (cells 0..2r-2),   mirrored f-: f-_{(k)} - f-_{(k+1)} = -dF_k + alpha du_k,
-//   centre values f+_{r-1} + f-_{r} = (F_{r-1} + F_r) - alpha du_{r-1}.
-// dF[k] = F_{k+1} - F_k, du[k] = u_{k+1} - u_k for the 2r-1 pairs of the 2r stencil cells; Fsum = F_{r-1} + F_r.
-// Returns TWICE the interface flux (the caller folds the 1/2 into 1/dx: exact in binary floating point).
-template <class T, int R>
-HD T llf_weno_field2(const T (&dF)[2 * R - 1], const T (&du)[2 * R - 1], T Fsum, T al, T eps) {
-    const T epsx = (R == 3 ? (T)16 : (T)4) * eps;
-    T Np, Dp, Nm, Dm;
-    if (R == 3) {
-        weno5_nd_d(tfma(al, du[0], dF[0]), tfma(al, du[1], dF[1]), tfma(al, du[2], dF[2]), tfma(al, du[3], dF[3]),
-                   epsx, Np, Dp);
-        weno5_nd_d(tfma(al, du[4], -dF[4]), tfma(al, du[3], -dF[3]), tfma(al, du[2], -dF[2]), tfma(al, du[1], -dF[1]),
-                   epsx, Nm, Dm);
-    } else {
-        constexpr int J5 = (R == 4) ? 5 : 0, J6 = (R == 4) ? 6 : 0;   // only read when R == 4
-        weno7_nd_d(tfma(al, du[0], dF[0]), tfma(al, du[1], dF[1]), tfma(al, du[2], dF[2]), tfma(al, du[3], dF[3]),
-                   tfma(al, du[4], dF[4]), tfma(al, du[J5], dF[J5]), epsx, Np, Dp);
-        weno7_nd_d(tfma(al, du[J6], -dF[J6]), tfma(al, du[J5], -dF[J5]), tfma(al, du[4], -dF[4]),
-                   tfma(al, du[3], -dF[3]), tfma(al, du[2], -dF[2]), tfma(al, du[1], -dF[1]), epsx, Nm, Dm);
-    }
-    return combine_pair(tfma(-al, du[R - 1], Fsum), Np, Dp, Nm, Dm);
-}
-
 // ------------------------------------------------------------------------------------------------
 // a7'. MUSTA-FORCE flux with MUSCL/minmod data (O6, O7; readings Q6-Q8).
 template <class T>
@@ -128,18 +101,16 @@ HD T minmod(T a, T b) {
     return a > (T)0 ? m : -m;
 }
 #ifdef __CUDA_ARCH__
-// fp64 on the device: the same function on the bit patterns, in the integer pipe (an fp64 compare or select
-// occupies the fp64 pipe, which is the one this path is bound by).  Opposite signs -> 0; otherwise the smaller
-// magnitude with the common sign (a zero operand has magnitude 0, so the result is +-0).  Differs from the
-// product test only when a*b underflows (both |a|, |b| < 1e-154), where it returns that tiny slope instead of 0.
+// fp64 on the device: the same function on the bit patterns, in the integer pipe (an fp64 compare, select or |x|
+// occupies the fp64 pipe, which is the one this path is bound by).  Doubles are sign-magnitude, so among two doubles
+// of the SAME sign the one of smaller magnitude is the smaller one as a signed 64-bit integer, whatever that sign:
+// minmod = opposite signs ? 0 : min_s64(a, b).  Differs from the product test only when a*b underflows (both |a|,
+// |b| < 1e-154), where it returns that tiny slope instead of 0, and for a zero operand, where it returns +-0.
 template <>
 __device__ __forceinline__ double minmod<double>(double a, double b) {
     const long long ia = __double_as_longlong(a), ib = __double_as_longlong(b);
-    if ((ia ^ ib) < 0) return 0.0;
-    const unsigned long long ma = (unsigned long long)ia & 0x7fffffffffffffffull;
-    const unsigned long long mb = (unsigned long long)ib & 0x7fffffffffffffffull;
-    const unsigned long long m = ma < mb ? ma : mb;
-    return __longlong_as_double((long long)(m | ((unsigned long long)ia & 0x8000000000000000ull)));
+    const long long m = ia < ib ? ia : ib;
+    return __longlong_as_double((ia ^ ib) < 0 ? 0ll : m);
 }
 #endif
 
@@ -186,6 +157,35 @@ HD void flux_only(const T Q[NF], T F[NF], int& flag, int eos, T p0) {
     F[4] = Q[4] * vd;
 }
 
+// The same two evaluations for the default closure p = e/3, arranged for the predictor-corrector loop, which runs six
+// of them per interface: ONE test sends every state the Q16 clamp could touch (E below the floor, |M| > (1 - 1e-12) E,
+// NaN) to the general functions above, so the common path carries no clamp selects; it needs one reciprocal,
+// 1/(2E+s) -- the pressure is (s - E)/3, whose cancellation error, an ulp of E, is an ulp of the flux it enters.
+template <class T, int DIR, bool SPEED>
+HD void musta_flux(const T Q[NF], T F[NF], T& a, int& flag) {
+    const T E = Q[0];
+    const T m2 = tfma(Q[1], Q[1], tfma(Q[2], Q[2], Q[3] * Q[3]));
+    const T t = E * E;
+    const T c2 = ((T)1 - (T)1e-12) * ((T)1 - (T)1e-12);
+    if (below_floor(E) || !(m2 <= c2 * t)) {   // rare (kept inline: out of line, Q and F would live in local memory)
+        if (SPEED) flux_and_speed<T, DIR, false>(Q, F, a, flag, 0, (T)0);
+        else flux_only<T, DIR, false>(Q, F, flag, 0, (T)0);
+        return;
+    }
+    const T s = fast_sqrt(tfma((T)4, t, (T)-3 * m2));
+    const T w = (T)3 * fast_rcp(tfma((T)2, E, s));   // v_i = M_i w
+    const T p = (s - E) * (T)(1.0 / 3.0);
+    const T vd = Q[1 + DIR] * w;
+    F[0] = Q[1 + DIR];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) F[1 + j] = (j == DIR) ? tfma(Q[1 + j], vd, p) : Q[1 + j] * vd;
+    F[4] = Q[4] * vd;
+    if (SPEED) {
+        const T v2 = m2 * w * w;
+        a = signal_speed(vd, v2, speed_inv_den(v2));
+    }
+}
+
 // acc.u(c, k), k = 0..3 for cells i-1 .. i+2.  K stages, local Courant number C (tau = C/S).
 // KS > 0: the number of stages is the compile-time constant KS (fully unrolled, the default K = 2 takes this
 // path); KS = 0: run-time K.
@@ -202,13 +202,18 @@ HD void musta_force_stages(const Acc& acc, int K, T C, int lim, int eos, T p0, T
         QL[c] = tfma((T)0.5, LIMS == 0 ? minmod(dm, d0) : limited_slope(lim, dm, d0), u1);
         QR[c] = tfma((T)-0.5, LIMS == 0 ? minmod(d0, dp) : limited_slope(lim, d0, dp), u2);
     }
-    const T invC = (T)1 / C;
+    const T invC = fast_rcp(C);   // (one MUFU-seeded reciprocal per interface; a true division costs a subroutine)
     const int nst = KS > 0 ? KS : K;
 #pragma unroll
     for (int stage = 1; stage <= nst; ++stage) {
         T FL[NF], FR[NF], QM[NF], FM[NF], aL, aR;
-        flux_and_speed<T, DIR, EOSRT>(QL, FL, aL, flag, eos, p0);
-        flux_and_speed<T, DIR, EOSRT>(QR, FR, aR, flag, eos, p0);
+        if (EOSRT) {
+            flux_and_speed<T, DIR, true>(QL, FL, aL, flag, eos, p0);
+            flux_and_speed<T, DIR, true>(QR, FR, aR, flag, eos, p0);
+        } else {
+            musta_flux<T, DIR, true>(QL, FL, aL, flag);
+            musta_flux<T, DIR, true>(QR, FR, aR, flag);
+        }
         const T S = max_nonneg(aL, aR);
         // p = p0: S = max |v_d| vanishes where the fluid is at rest and tau = C/S is then infinite, in the oracle
         // as here (reading Q7 has no finite local step without a sound speed): MUSTA-FORCE with that closure is
@@ -216,7 +221,11 @@ HD void musta_force_stages(const Acc& acc, int K, T C, int lim, int eos, T p0, T
         const T tau = C * fast_rcp(S), itau = S * invC;
 #pragma unroll
         for (int c = 0; c < NF; ++c) QM[c] = (T)0.5 * ((QL[c] + QR[c]) - tau * (FR[c] - FL[c]));
-        flux_only<T, DIR, EOSRT>(QM, FM, flag, eos, p0);
+        if (EOSRT) flux_only<T, DIR, true>(QM, FM, flag, eos, p0);
+        else {
+            T unused;
+            musta_flux<T, DIR, false>(QM, FM, unused, flag);
+        }
 #pragma unroll
         for (int c = 0; c < NF; ++c)
             fh[c] = (T)0.25 * (FL[c] + (T)2 * FM[c] + FR[c] - (QR[c] - QL[c]) * itau);

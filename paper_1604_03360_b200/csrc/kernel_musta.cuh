@@ -2,7 +2,7 @@
 // the SSP-RK3 combination (a9), every interface flux computed once.
 //
 // The predictor-corrector flux runs con2prim on face states that mix all five fields, so one thread carries all
-// five fields of its stencil (the WENO schemes split the fields over threads instead, kernel_fp.cuh).
+// five fields of its stencil.
 //   musta_xz_kernel<T>     x and z fluxes in ONE marching kernel without block barriers.  A warp is a row of 32
 //       consecutive x positions (lane 0 is the helper column one cell below the 31 cells the warp owns), a block is
 //       four such rows, and every thread marches along z through a chunk of planes:
@@ -58,10 +58,15 @@ struct RowAcc {
     __device__ __forceinline__ T u(int c, int k) const { return ub[c * astride + k]; }
 };
 
-template <class T, int DIR, class Acc>
+// FAST: the default configuration (K = 2, minmod, p = e/3) with everything a compile-time constant; otherwise the
+// run-time K / limiter / closure.  The choice is made per KERNEL, not per interface: with both bodies inlined the
+// marching loops outgrew the instruction cache (stall reason "no instruction").
+template <class T, int DIR, bool FAST, class Acc>
 __device__ __forceinline__ void musta_iface(const Acc& acc, const StageArgs& A, T fh[NF], int& flag) {
-    musta_force_iface<T, DIR>(acc, A.musta_K, (T)A.musta_C, A.limiter, A.eos.kind, (T)A.eos.p0, fh, flag);
+    if (FAST) musta_force_stages<T, DIR, 2, 0>(acc, 2, (T)A.musta_C, 0, 0, (T)0, fh, flag);
+    else musta_force_stages<T, DIR, 0, -1>(acc, A.musta_K, (T)A.musta_C, A.limiter, A.eos.kind, (T)A.eos.p0, fh, flag);
 }
+inline bool musta_fast(const StageArgs& A) { return A.musta_K == 2 && A.limiter == 0 && A.eos.kind == 0; }
 
 // ---------------------------------------------------------------------------------------------------------
 template <class T>
@@ -77,7 +82,7 @@ struct MustaXZShape {
     }
 };
 
-template <class T>
+template <class T, bool FAST>
 __global__ void __launch_bounds__(MUSTA_THREADS, 3)
 musta_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* Un, T* Uout, Ctl* ctl, int zc) {
     using S = MustaXZShape<T>;
@@ -139,7 +144,7 @@ musta_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* Un, T* U
     int zflag = 0;
     {
         T f0[NF];
-        musta_iface<T, 2>(zw, A, f0, zflag);   // face k0 - 1/2
+        musta_iface<T, 2, FAST>(zw, A, f0, zflag);   // face k0 - 1/2
 #pragma unroll
         for (int c = 0; c < NF; ++c) park[c * TH] = f0[c];
     }
@@ -168,7 +173,7 @@ musta_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* Un, T* U
         }
         __syncwarp();
         T L[NF], f[NF];
-        musta_iface<T, 2>(zw, A, f, zflag);
+        musta_iface<T, 2, FAST>(zw, A, f, zflag);
 #pragma unroll
         for (int c = 0; c < NF; ++c) {
             L[c] = park[c * TH] - f[c];
@@ -178,7 +183,7 @@ musta_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* Un, T* U
         for (int c = 0; c < NF; ++c) f[c] = (T)0;
         if (need_x) {
             RowAcc<T> acc{row + lane, RWX};
-            musta_iface<T, 0>(acc, A, f, flag);
+            musta_iface<T, 0, FAST>(acc, A, f, flag);
         }
 #pragma unroll
         for (int c = 0; c < NF; ++c) L[c] += shfl_up1<T>(f[c]) - f[c];
@@ -207,8 +212,8 @@ constexpr size_t musta_y_smem_bytes() {
     return sizeof(T) * ((size_t)MUSTA_DEPTH * (NF + NF) + NF) * MUSTA_THREADS;
 }
 
-template <class T, bool EPI>
-__global__ void __launch_bounds__(MUSTA_THREADS, 3)
+template <class T, bool EPI, bool FAST>
+__global__ void __launch_bounds__(MUSTA_THREADS, 4)
 musta_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl, int yc) {
     constexpr int R = MUSTA_R, M = 2 * R, NVO = NF + NF, D = MUSTA_DEPTH, TH = MUSTA_THREADS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -250,7 +255,7 @@ musta_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl,
     }
     {
         T f0[NF];
-        musta_iface<T, 1>(zw, A, f0, flag);
+        musta_iface<T, 1, FAST>(zw, A, f0, flag);
 #pragma unroll
         for (int c = 0; c < NF; ++c) park[c * TH] = f0[c];
     }
@@ -264,7 +269,7 @@ musta_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl,
         for (int c = 0; c < NF; ++c) nxt[c] = src[c * TH];
         zw.shift();
         zw.put(M - 1, nxt);
-        musta_iface<T, 1>(zw, A, f, flag);
+        musta_iface<T, 1, FAST>(zw, A, f, flag);
         const long long q = p0 + (long long)(j - j0) * ms;
 #pragma unroll
         for (int c = 0; c < NF; ++c) {
@@ -285,14 +290,14 @@ musta_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl,
 
 template <class T>
 int configure_musta(char* err, size_t errlen) {
-    cudaError_t e = cudaFuncSetAttribute(musta_xz_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)MustaXZShape<T>::smem_bytes());
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(musta_y_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)musta_y_smem_bytes<T>());
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(musta_y_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)musta_y_smem_bytes<T>());
+    const int sxz = (int)MustaXZShape<T>::smem_bytes(), sy = (int)musta_y_smem_bytes<T>();
+    const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+    cudaError_t e = cudaFuncSetAttribute(musta_xz_kernel<T, true>, attr, sxz);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(musta_xz_kernel<T, false>, attr, sxz);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(musta_y_kernel<T, false, true>, attr, sy);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(musta_y_kernel<T, true, true>, attr, sy);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(musta_y_kernel<T, false, false>, attr, sy);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(musta_y_kernel<T, true, false>, attr, sy);
     if (e != cudaSuccess) {
         snprintf(err, errlen, "cudaFuncSetAttribute (musta): %s", cudaGetErrorString(e));
         return -1;
@@ -306,12 +311,18 @@ int launch_musta(const Geom& G, const StageArgs& A, const T* Us, const T* Un, T*
                  cudaStream_t st, int* launches, char* err, size_t errlen) {
     const dim3 b(32, MUSTA_ROWS, 1);
     const dim3 g((G.n[0] + 30) / 31, (G.n[1] + MUSTA_ROWS - 1) / MUSTA_ROWS, (G.n[2] + zc - 1) / zc);
-    musta_xz_kernel<T><<<g, b, MustaXZShape<T>::smem_bytes(), st>>>(G, A, Us, Un, Uout, ctl, zc);
     const dim3 gy((G.n[0] + 31) / 32, (G.n[2] + MUSTA_ROWS - 1) / MUSTA_ROWS, (G.n[1] + yc - 1) / yc);
-    if (A.epi_max && A.mode != 1)
-        musta_y_kernel<T, true><<<gy, b, musta_y_smem_bytes<T>(), st>>>(G, A, Us, Uout, ctl, yc);
-    else
-        musta_y_kernel<T, false><<<gy, b, musta_y_smem_bytes<T>(), st>>>(G, A, Us, Uout, ctl, yc);
+    const size_t sxz = MustaXZShape<T>::smem_bytes(), sy = musta_y_smem_bytes<T>();
+    const bool epi = A.epi_max && A.mode != 1;
+    if (musta_fast(A)) {
+        musta_xz_kernel<T, true><<<g, b, sxz, st>>>(G, A, Us, Un, Uout, ctl, zc);
+        if (epi) musta_y_kernel<T, true, true><<<gy, b, sy, st>>>(G, A, Us, Uout, ctl, yc);
+        else musta_y_kernel<T, false, true><<<gy, b, sy, st>>>(G, A, Us, Uout, ctl, yc);
+    } else {
+        musta_xz_kernel<T, false><<<g, b, sxz, st>>>(G, A, Us, Un, Uout, ctl, zc);
+        if (epi) musta_y_kernel<T, true, false><<<gy, b, sy, st>>>(G, A, Us, Uout, ctl, yc);
+        else musta_y_kernel<T, false, false><<<gy, b, sy, st>>>(G, A, Us, Uout, ctl, yc);
+    }
     *launches = 2;
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) {
