@@ -24,7 +24,9 @@ template <> HD float tfma<float>(float a, float b, float c) { return fmaf(a, b, 
 template <class T> HD T tsqrt(T x);
 template <> HD double tsqrt<double>(double x) { return sqrt(x); }
 template <> HD float tsqrt<float>(float x) { return sqrtf(x); }
-template <class T> HD T tabs(T x) { return x < (T)0 ? -x : x; }
+template <class T> HD T tabs(T x);   // |x| as an operand modifier, not a compare and two selects
+template <> HD double tabs<double>(double x) { return fabs(x); }
+template <> HD float tabs<float>(float x) { return fabsf(x); }
 template <class T> HD T tmax(T a, T b);
 template <> HD double tmax<double>(double a, double b) { return fmax(a, b); }
 template <> HD float tmax<float>(float a, float b) { return fmaxf(a, b); }
@@ -66,19 +68,18 @@ HD float fast_rcp(float x) {
 #endif
 }
 
-// Square root of a positive, finite, normal number.  fp64: MUFU.RSQ64H seed plus two coupled Newton steps
-// on s = sqrt(x) (5 DFMA-pipe instructions, error about 1 ulp, no special-case path).  fp32: sqrtf.
+// Square root of a positive, finite, normal number.  fp64: MUFU.RSQ64H seed y (relative error below 2^-20) plus ONE
+// cubically convergent step on s = x y: with e = 1 - s y = 1 - x y^2 the root is s (1 - e)^(-1/2) =
+// s (1 + e/2 + 3 e^2/8 + O(e^3)), remainder below 2^-58; 5 fp64-pipe instructions, error about 1 ulp, no special-case
+// path.  fp32: the hardware square root.
 HD double fast_sqrt(double x) {
 #ifdef __CUDA_ARCH__
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double s = x * y;
-    const double h = 0.5 * y;
-    double e = fma(-s, s, x);
-    s = fma(e, h, s);
-    e = fma(-s, s, x);
-    s = fma(e, h, s);
-    return s;
+    const double s = x * y;
+    const double e = fma(-s, y, 1.0);
+    const double pe = fma(0.375, e, 0.5) * e;
+    return fma(s, pe, s);
 #else
     return sqrt(x);
 #endif
@@ -171,14 +172,17 @@ HD void con2prim_p0(T E, T M0, T M1, T M2, T p0, T& winv, T& p, T& v2, int& flag
 
 // a3. directional characteristic speeds, c_s^2 = 1/3 (a3):
 //   a_d = ( |v_d| (1-cs2) + cs sqrt((1-v^2)(1 - v_d^2 - (v^2 - v_d^2) cs2)) ) / (1 - v^2 cs2)
-template <class T>
+// FLOOR = false: for states known to be well inside |v| < 1 (the branch-free MUSTA path), where disc > 0 holds with
+// a wide margin and the floor is dead weight.
+template <class T, bool FLOOR = true>
 HD T signal_speed(T vd, T v2, T inv_den) {
     const T cs2 = (T)(1.0 / 3.0);
     const T cs = (T)0.57735026918962576451;
     const T vd2 = vd * vd;
     // disc >= 0 analytically; the floor keeps the reciprocal-square-root seed finite when a clamped state
     // (reading Q16) drives it to zero
-    const T disc = max_nonneg(((T)1 - v2) * ((T)1 - vd2 - (v2 - vd2) * cs2), (T)1e-30);   // (a negative value loses too)
+    T disc = ((T)1 - v2) * ((T)1 - vd2 - (v2 - vd2) * cs2);
+    if (FLOOR) disc = max_nonneg(disc, (T)1e-30);   // (a negative value loses too)
     return (tabs(vd) * ((T)1 - cs2) + cs * fast_sqrt(disc)) * inv_den;
 }
 template <class T>

@@ -186,22 +186,15 @@ HD void musta_flux(const T Q[NF], T F[NF], T& a, int& flag) {
     }
 }
 
-// acc.u(c, k), k = 0..3 for cells i-1 .. i+2.  K stages, local Courant number C (tau = C/S).
-// KS > 0: the number of stages is the compile-time constant KS (fully unrolled, the default K = 2 takes this
-// path); KS = 0: run-time K.
-// LIMS >= 0: the limiter is the compile-time constant LIMS (the default minmod takes this path at full speed: a
-// run-time limiter inside the interface code cost 17 % of the MUSTA step); LIMS < 0: run-time `lim`.
-template <class T, int DIR, int KS, int LIMS, class Acc>
-HD void musta_force_stages(const Acc& acc, int K, T C, int lim, int eos, T p0, T fh[NF], int& flag) {
-    constexpr bool EOSRT = LIMS < 0;   // the fast path (compile-time K, minmod) is also the default closure's
-    T QL[NF], QR[NF];
-#pragma unroll
-    for (int c = 0; c < NF; ++c) {
-        const T u0 = acc.u(c, 0), u1 = acc.u(c, 1), u2 = acc.u(c, 2), u3 = acc.u(c, 3);
-        const T dm = u1 - u0, d0 = u2 - u1, dp = u3 - u2;
-        QL[c] = tfma((T)0.5, LIMS == 0 ? minmod(dm, d0) : limited_slope(lim, dm, d0), u1);
-        QR[c] = tfma((T)-0.5, LIMS == 0 ? minmod(d0, dp) : limited_slope(lim, d0, dp), u2);
-    }
+// Limited slope of a cell from its backward and forward differences (O6); LIMS == 0: minmod at compile time.
+template <class T, int LIMS>
+HD T musta_slope(int lim, T dm, T dp) { return LIMS == 0 ? minmod(dm, dp) : limited_slope(lim, dm, dp); }
+
+// The predictor-corrector loop (O7, readings Q7, Q8) from the two face states, general form: every con2prim carries
+// the Q16 clamp, K and the closure may be run-time values.  QL, QR are overwritten by the corrected states.
+// KS > 0: the number of stages is the compile-time constant KS; KS = 0: run-time K.
+template <class T, int DIR, int KS, bool EOSRT>
+HD void musta_force_core(T QL[NF], T QR[NF], int K, T C, int eos, T p0, T fh[NF], int& flag) {
     const T invC = fast_rcp(C);   // (one MUFU-seeded reciprocal per interface; a true division costs a subroutine)
     const int nst = KS > 0 ? KS : K;
 #pragma unroll
@@ -237,6 +230,113 @@ HD void musta_force_stages(const Acc& acc, int K, T C, int lim, int eos, T p0, T
             }
         }
     }
+}
+
+// acc.u(c, k), k = 0..3 for cells i-1 .. i+2.  K stages, local Courant number C (tau = C/S).
+// LIMS >= 0: the limiter is the compile-time constant LIMS and the closure the default one; LIMS < 0: run-time
+// limiter and closure.
+template <class T, int DIR, int KS, int LIMS, class Acc>
+HD void musta_force_stages(const Acc& acc, int K, T C, int lim, int eos, T p0, T fh[NF], int& flag) {
+    constexpr bool EOSRT = LIMS < 0;
+    T QL[NF], QR[NF];
+#pragma unroll
+    for (int c = 0; c < NF; ++c) {
+        const T u0 = acc.u(c, 0), u1 = acc.u(c, 1), u2 = acc.u(c, 2), u3 = acc.u(c, 3);
+        const T dm = u1 - u0, d0 = u2 - u1, dp = u3 - u2;
+        QL[c] = tfma((T)0.5, musta_slope<T, LIMS>(lim, dm, d0), u1);
+        QR[c] = tfma((T)-0.5, musta_slope<T, LIMS>(lim, d0, dp), u2);
+    }
+    musta_force_core<T, DIR, KS, EOSRT>(QL, QR, K, C, eos, p0, fh, flag);
+}
+
+// ------------------------------------------------------------------------------------------------
+// The same loop for the default configuration (p = e/3, compile-time K), arranged for the fp64 pipe (DESIGN.md
+// section 6); the marching kernels use it.  It is ONE basic block: no clamp, no branch, so that the compiler can
+// interleave the independent evaluations F(Q_L), F(Q_R) of a stage and the two interfaces a thread works on.  A state
+// the Q16 clamp could touch (E below the floor or not finite, |M| close to or above E, NaN) only sets `bad`; the
+// caller then discards the result and runs the general form above on the same face states.
+//
+// Rearrangements (rounding only): with G_L = Q_L + tau F_L and G_R = Q_R - tau F_R,
+//   2 Q_M = G_L + G_R,   F(2 Q_M) = 2 F(Q_M)  (the flux is homogeneous of degree one in Q, exactly so in binary
+//   floating point),   4 F* = (F_L + Q_L/tau) + (F_R - Q_R/tau) + F(2 Q_M) = (G_L - G_R)/tau + F(2 Q_M),
+//   corrector: Q_L' = G_L - (tau/4)(4 F*),  Q_R' = G_R + (tau/4)(4 F*).
+// Returns FOUR TIMES the flux: the caller folds the 1/4 into its 1/dx factor (exact).
+template <class T>
+HD bool musta_fast_ok(T E, T t, T D) { return !below_floor(E) && D >= t * (T)1.0001; }
+template <class T>
+HD bool musta_finite(T x) { return tabs(x) <= (T)3e38; }
+#ifdef __CUDA_ARCH__
+template <>
+__device__ __forceinline__ bool musta_fast_ok<double>(double E, double t, double D) {
+    // two signed compares of high words (integer pipe).  E above the floor (a negative E is a negative integer);
+    // D = 4 E^2 - 3 M^2 against t = E^2: hi(D) >= hi(t) + 2 means D > t (1 + 2^-21), i.e. |M| < (1 - 1e-7) E, well
+    // inside the Q16 bound, and a negative D fails.  Infinities and NaNs can pass here: they make the flux
+    // non-finite, which musta_force_fast4 tests once at its end.
+    return __double2hiint(E) > 0x01a56e1f && __double2hiint(D) > __double2hiint(t) + 1;
+}
+template <>
+__device__ __forceinline__ bool musta_finite<double>(double x) {
+    return (unsigned)(__double2hiint(x) << 1) < 0xffe00000u;
+}
+#endif
+
+template <class T, int DIR, bool SPEED>
+HD void musta_eval_fast(const T Q[NF], T F[NF], T& a, bool& bad) {
+    const T E = Q[0], md = Q[1 + DIR];
+    const T m2 = tfma(Q[1], Q[1], tfma(Q[2], Q[2], Q[3] * Q[3]));
+    const T t = E * E;
+    const T D = tfma((T)4, t, (T)-3 * m2);
+    bad |= !musta_fast_ok(E, t, D);
+    const T s = fast_sqrt(D);
+    const T w = (T)3 * fast_rcp(tfma((T)2, E, s));   // v_i = M_i w
+    const T p = (s - E) * (T)(1.0 / 3.0);            // cancellation error: an ulp of E, i.e. an ulp of the flux it enters
+    const T vd = md * w;
+    F[0] = md;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) F[1 + j] = (j == DIR) ? tfma(Q[1 + j], vd, p) : Q[1 + j] * vd;
+    F[4] = Q[4] * vd;
+    if (SPEED) {
+        const T v2 = m2 * w * w;
+        a = signal_speed<T, false>(vd, v2, speed_inv_den(v2));
+    }
+}
+
+template <class T, int DIR, int KS>
+HD void musta_force_fast4(const T QL0[NF], const T QR0[NF], T C, T invC, T fh4[NF], bool& bad) {
+    T QL[NF], QR[NF];
+#pragma unroll
+    for (int c = 0; c < NF; ++c) {
+        QL[c] = QL0[c];
+        QR[c] = QR0[c];
+    }
+#pragma unroll
+    for (int stage = 1; stage <= KS; ++stage) {
+        T FL[NF], FR[NF], GL[NF], GR[NF], Q2[NF], F2[NF], aL, aR, unused;
+        musta_eval_fast<T, DIR, true>(QL, FL, aL, bad);
+        musta_eval_fast<T, DIR, true>(QR, FR, aR, bad);
+        const T S = max_nonneg(aL, aR);
+        const T tau = C * fast_rcp(S), itau = S * invC;
+#pragma unroll
+        for (int c = 0; c < NF; ++c) {
+            GL[c] = tfma(tau, FL[c], QL[c]);
+            GR[c] = tfma(-tau, FR[c], QR[c]);
+            Q2[c] = GL[c] + GR[c];
+        }
+        musta_eval_fast<T, DIR, false>(Q2, F2, unused, bad);
+        // (F_L + Q_L/tau) + (F_R - Q_R/tau) = (G_L - G_R)/tau
+#pragma unroll
+        for (int c = 0; c < NF; ++c) fh4[c] = tfma(itau, GL[c] - GR[c], F2[c]);
+        if (stage < KS) {
+            const T t4 = (T)0.25 * tau;
+#pragma unroll
+            for (int c = 0; c < NF; ++c) {
+                QL[c] = tfma(-t4, fh4[c], GL[c]);
+                QR[c] = tfma(t4, fh4[c], GR[c]);
+            }
+        }
+    }
+    // a NaN or an infinity anywhere above has reached the flux
+    bad |= !musta_finite(((fh4[0] + fh4[1]) + (fh4[2] + fh4[3])) + fh4[4]);
 }
 
 template <class T, int DIR, class Acc>

@@ -32,47 +32,70 @@ constexpr int MUSTA_ROWS = 4;    // warps per block
 constexpr int MUSTA_THREADS = 32 * MUSTA_ROWS;
 constexpr int MUSTA_R = 2, MUSTA_M = 4;
 
-// 4-cell stencil of the five conserved fields of one column, in registers (all indices compile-time constants)
-template <class T>
-struct MustaWindow {
-    T uu[NF][MUSTA_M];
-    __device__ __forceinline__ T u(int c, int k) const { return uu[c][k]; }
-    __device__ __forceinline__ void put(int m, const T v[NF]) {
+// Marching state of one column along the marched axis: the MUSCL slope (O6) belongs to a CELL, so it is made once per
+// cell and serves both of the cell's faces.  With cell m the one whose upper face is being computed:
+//   u0 = u_m, u1 = u_{m+1}, db = u_{m+1} - u_m, ql = Q_L of face m+1/2 = u_m + slope_m / 2.
+// advance(u2) takes u_{m+2}, makes slope_{m+1} and returns Q_R of face m+1/2 = u_{m+1} - slope_{m+1}/2; commit() then
+// moves on to cell m+1.
+template <class T, int LIMS>
+struct MustaColumn {
+    T u0[NF], u1[NF], db[NF], ql[NF];
+    T df[NF], qn[NF];   // between advance() and commit(): u_{m+2} - u_{m+1}, Q_L of face m+3/2
+    __device__ __forceinline__ void init(const T a[NF], const T b[NF], const T c[NF], int lim) {   // cells m-1, m, m+1
 #pragma unroll
-        for (int c = 0; c < NF; ++c) uu[c][m] = v[c];
+        for (int f = 0; f < NF; ++f) {
+            u0[f] = b[f];
+            u1[f] = c[f];
+            db[f] = c[f] - b[f];
+            ql[f] = tfma((T)0.5, musta_slope<T, LIMS>(lim, b[f] - a[f], db[f]), b[f]);
+        }
     }
-    __device__ __forceinline__ void shift() {
+    __device__ __forceinline__ void advance(const T u2[NF], int lim, T qr[NF]) {
 #pragma unroll
-        for (int m = 0; m + 1 < MUSTA_M; ++m) {
+        for (int f = 0; f < NF; ++f) {
+            df[f] = u2[f] - u1[f];
+            const T h = (T)0.5 * musta_slope<T, LIMS>(lim, db[f], df[f]);
+            qr[f] = u1[f] - h;
+            qn[f] = u1[f] + h;
+        }
+    }
+    __device__ __forceinline__ void commit(const T u2[NF]) {
 #pragma unroll
-            for (int c = 0; c < NF; ++c) uu[c][m] = uu[c][m + 1];
+        for (int f = 0; f < NF; ++f) {
+            u0[f] = u1[f];
+            u1[f] = u2[f];
+            db[f] = df[f];
+            ql[f] = qn[f];
         }
     }
 };
 
-// stencil accessor into a shared-memory row: conserved field c of stencil cell k at ub[c * astride + k]
-template <class T>
-struct RowAcc {
-    const T* ub;
-    int astride;
-    __device__ __forceinline__ T u(int c, int k) const { return ub[c * astride + k]; }
-};
-
-// FAST: the default configuration (K = 2, minmod, p = e/3) with everything a compile-time constant; otherwise the
-// run-time K / limiter / closure.  The choice is made per KERNEL, not per interface: with both bodies inlined the
-// marching loops outgrew the instruction cache (stall reason "no instruction").
-template <class T, int DIR, bool FAST, class Acc>
-__device__ __forceinline__ void musta_iface(const Acc& acc, const StageArgs& A, T fh[NF], int& flag) {
-    if (FAST) musta_force_stages<T, DIR, 2, 0>(acc, 2, (T)A.musta_C, 0, 0, (T)0, fh, flag);
-    else musta_force_stages<T, DIR, 0, -1>(acc, A.musta_K, (T)A.musta_C, A.limiter, A.eos.kind, (T)A.eos.p0, fh, flag);
-}
+// FAST: the default configuration (K = 2, minmod, p = e/3) with everything a compile-time constant and the branch-free
+// core (iface.cuh); otherwise the run-time K / limiter / closure.  The choice is made per KERNEL, not per interface:
+// with both bodies inlined the marching loops outgrew the instruction cache (stall reason "no instruction").
 inline bool musta_fast(const StageArgs& A) { return A.musta_K == 2 && A.limiter == 0 && A.eos.kind == 0; }
+
+// general form on a copy of the face states; returns four times the flux like the fast core
+template <class T, int DIR, bool FAST>
+__device__ __forceinline__ void musta_general4(const T QL[NF], const T QR[NF], const StageArgs& A, T C, T f4[NF],
+                                               int& flag) {
+    T a[NF], b[NF];
+#pragma unroll
+    for (int c = 0; c < NF; ++c) {
+        a[c] = QL[c];
+        b[c] = QR[c];
+    }
+    if (FAST) musta_force_core<T, DIR, 2, false>(a, b, 2, C, 0, (T)0, f4, flag);
+    else musta_force_core<T, DIR, 0, true>(a, b, A.musta_K, C, A.eos.kind, (T)A.eos.p0, f4, flag);
+#pragma unroll
+    for (int c = 0; c < NF; ++c) f4[c] *= (T)4;
+}
 
 // ---------------------------------------------------------------------------------------------------------
 template <class T>
 struct MustaXZShape {
     static constexpr int R = MUSTA_R, D = MUSTA_DEPTH;
-    static constexpr int NS = NF + NF;                       // window cell k+R, u^n of plane k: slots per thread
+    static constexpr int NS = NF + NF;                       // cell k+R, u^n of plane k: slots per thread
     static constexpr int NHL = 2 * R - 1;                    // halo lanes: R-1 cells below, R cells above the row
     static constexpr int RWX = 32 + 2 * R - 1;               // cells of a row with halo
     static constexpr int STAGE = NS * MUSTA_THREADS + MUSTA_ROWS * NHL * NF;
@@ -82,11 +105,19 @@ struct MustaXZShape {
     }
 };
 
+#ifndef MUSTA_XZ_MINB
+#define MUSTA_XZ_MINB 2
+#endif
+#ifndef MUSTA_Y_MINB
+#define MUSTA_Y_MINB 2
+#endif
+
 template <class T, bool FAST>
-__global__ void __launch_bounds__(MUSTA_THREADS, 3)
+__global__ void __launch_bounds__(MUSTA_THREADS, MUSTA_XZ_MINB)
 musta_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* Un, T* Uout, Ctl* ctl, int zc) {
     using S = MustaXZShape<T>;
-    constexpr int R = S::R, M = 2 * R, NS = S::NS, NHL = S::NHL, RWX = S::RWX, D = S::D, TH = MUSTA_THREADS;
+    constexpr int R = S::R, NS = S::NS, NHL = S::NHL, RWX = S::RWX, D = S::D, TH = MUSTA_THREADS;
+    constexpr int LIMS = FAST ? 0 : -1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* sm = reinterpret_cast<T*>(smem_raw);
     const int lane = threadIdx.x, wy = threadIdx.y, tid = wy * 32 + lane;
@@ -106,6 +137,8 @@ musta_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* Un, T* U
     const long long p0 = G.pidx(il, j, k0);
     const long long ph = G.pidx(min(hcell, imax), j, k0);
     const bool use_un = A.mode != 1 && A.ca != 0.0;
+    const int lim = A.limiter;
+    const T C = (T)A.musta_C, invC = fast_rcp(C);
     int flag = 0;
 
     auto issue = [&](int k) {
@@ -131,95 +164,137 @@ musta_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* Un, T* U
 #pragma unroll
     for (int d = 0; d < D; ++d) issue(k0 + d);
 
-    MustaWindow<T> zw;
-    T nxt[NF];
-#pragma unroll
-    for (int m = 0; m < M; ++m) {   // cells k0-R .. k0+R-1
-#pragma unroll
-        for (int c = 0; c < NF; ++c) nxt[c] = __ldg(Us + c * G.fs + p0 + (long long)(m - R) * G.sxy);
-        zw.put(m, nxt);
-    }
     // the helper lane and the idle lanes of a ragged last tile march through x-ghost columns, whose z-ghost cells
     // are edge ghosts nobody fills: their z-fluxes are discarded, and so must be their unphysical-state flag
     int zflag = 0;
-    {
-        T f0[NF];
-        musta_iface<T, 2, FAST>(zw, A, f0, zflag);   // face k0 - 1/2
+    MustaColumn<T, LIMS> zc_;
+    {   // face k0 - 1/2 from cells k0-2 .. k0+1, then the column state of cell k0
+        T c[4][NF];
 #pragma unroll
-        for (int c = 0; c < NF; ++c) park[c * TH] = f0[c];
+        for (int m = 0; m < 4; ++m) {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) c[m][f] = __ldg(Us + f * G.fs + p0 + (long long)(m - R) * G.sxy);
+        }
+        zc_.init(c[0], c[1], c[2], lim);   // column at cell k0-1: ql = Q_L of face k0-1/2
+        T qr[NF], f0[NF];
+        zc_.advance(c[3], lim, qr);
+        if (FAST) {
+            bool bad = false;
+            musta_force_fast4<T, 2, 2>(zc_.ql, qr, C, invC, f0, bad);
+            if (bad) musta_general4<T, 2, FAST>(zc_.ql, qr, A, C, f0, zflag);
+        } else {
+            musta_general4<T, 2, FAST>(zc_.ql, qr, A, C, f0, zflag);
+        }
+        zc_.commit(c[3]);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) park[f * TH] = f0[f];
     }
-    const T dt = (T)ctl->dt, ca = (T)A.ca, cb = (T)A.cb, inv_dx = (T)A.inv_dx;
+    // the interface functions return four times the flux: the 1/4 of the FORCE average goes into dt/dx
+    const T dtdx = (T)(A.mode == 1 ? 0.25 * A.inv_dx : 0.25 * ctl->dt * A.inv_dx), ca = (T)A.ca, cb = (T)A.cb;
 
     for (int k = k0; k < k1; ++k) {
         cp_async_wait<D - 1>();   // plane k's stage has landed
         const T* st = sm + ((k - k0) % D) * S::STAGE;
         const T* src = st + tid;
-        T hv[NF];
+        T u2[NF], hv[NF];
 #pragma unroll
-        for (int c = 0; c < NF; ++c) nxt[c] = src[c * TH];
+        for (int c = 0; c < NF; ++c) u2[c] = src[c * TH];
         if (lane < NHL) {
             const T* hs = st + NS * TH + (wy * NHL + lane) * NF;
 #pragma unroll
             for (int c = 0; c < NF; ++c) hv[c] = hs[c];
         }
-        zw.shift();
-        zw.put(M - 1, nxt);
         __syncwarp();             // every lane is done with the row of plane k-1
 #pragma unroll
-        for (int c = 0; c < NF; ++c) row[c * RWX + lane + R - 1] = zw.uu[c][R - 1];
+        for (int c = 0; c < NF; ++c) row[c * RWX + lane + R - 1] = zc_.u0[c];
         if (lane < NHL) {
 #pragma unroll
             for (int c = 0; c < NF; ++c) row[c * RWX + hq] = hv[c];
         }
         __syncwarp();
-        T L[NF], f[NF];
-        musta_iface<T, 2, FAST>(zw, A, f, zflag);
+        // z: face k + 1/2
+        T qrz[NF], qlx[NF], qrx[NF];
+        zc_.advance(u2, lim, qrz);
+        // x: this lane's cell makes its slope once, keeps Q_L of its upper face and hands Q_R of its lower face to
+        // the lane below; the last lane makes the slope of the first cell beyond the row as well
+        {
+            T up[NF], dp[NF];
+#pragma unroll
+            for (int c = 0; c < NF; ++c) {
+                const T um = row[c * RWX + lane + R - 2];
+                up[c] = row[c * RWX + lane + R];
+                dp[c] = up[c] - zc_.u0[c];
+                const T h = (T)0.5 * musta_slope<T, LIMS>(lim, zc_.u0[c] - um, dp[c]);
+                qlx[c] = zc_.u0[c] + h;
+                qrx[c] = __shfl_down_sync(0xffffffffu, zc_.u0[c] - h, 1);
+            }
+            if (lane == 31) {
+#pragma unroll
+                for (int c = 0; c < NF; ++c) {
+                    const T upp = row[c * RWX + lane + R + 1];
+                    qrx[c] = tfma((T)-0.5, musta_slope<T, LIMS>(lim, dp[c], upp - up[c]), up[c]);
+                }
+            }
+        }
+        T fz[NF], fx[NF];
+        if (FAST) {   // both interfaces in one basic block; the rare repairs afterwards
+            bool badz = false, badx = false;
+            musta_force_fast4<T, 2, 2>(zc_.ql, qrz, C, invC, fz, badz);
+            musta_force_fast4<T, 0, 2>(qlx, qrx, C, invC, fx, badx);
+            if (badz) musta_general4<T, 2, FAST>(zc_.ql, qrz, A, C, fz, zflag);
+            if (badx && need_x) musta_general4<T, 0, FAST>(qlx, qrx, A, C, fx, flag);
+        } else {
+            musta_general4<T, 2, FAST>(zc_.ql, qrz, A, C, fz, zflag);
+            int xf = 0;
+            musta_general4<T, 0, FAST>(qlx, qrx, A, C, fx, xf);
+            if (need_x) flag |= xf;
+        }
+        T L[NF];
 #pragma unroll
         for (int c = 0; c < NF; ++c) {
-            L[c] = park[c * TH] - f[c];
-            park[c * TH] = f[c];
+            L[c] = (park[c * TH] - fz[c]) + (shfl_up1<T>(fx[c]) - fx[c]);
+            park[c * TH] = fz[c];
         }
-#pragma unroll
-        for (int c = 0; c < NF; ++c) f[c] = (T)0;
-        if (need_x) {
-            RowAcc<T> acc{row + lane, RWX};
-            musta_iface<T, 0, FAST>(acc, A, f, flag);
-        }
-#pragma unroll
-        for (int c = 0; c < NF; ++c) L[c] += shfl_up1<T>(f[c]) - f[c];
         if (own) {
             const long long q = p0 + (long long)(k - k0) * G.sxy;
             if (A.mode == 1) {
 #pragma unroll
-                for (int c = 0; c < NF; ++c) Uout[c * G.fs + q] = L[c] * inv_dx;
+                for (int c = 0; c < NF; ++c) Uout[c * G.fs + q] = L[c] * dtdx;
             } else {
 #pragma unroll
                 for (int c = 0; c < NF; ++c) {
-                    T v = tfma(dt, L[c] * inv_dx, zw.uu[c][R - 1]);
+                    T v = tfma(dtdx, L[c], zc_.u0[c]);
                     if (use_un) v = tfma(ca, src[(NF + c) * TH], cb * v);   // u^n: read late, it is only needed here
                     Uout[c * G.fs + q] = v;
                 }
             }
         }
+        zc_.commit(u2);
         issue(k + D);             // refill the slot just consumed
     }
     if (flag || (own && zflag)) ctl->flag = 1;
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// The y sweep advances TWO cells per iteration: the two interfaces j+1/2 and j+3/2 are independent, and in one basic
+// block they give the fp64 pipe four independent con2prim chains (two face states each) to interleave; a dependent fp64
+// instruction issues only every 8 cycles, and more warps do not replace that instruction-level parallelism
+// (DESIGN.md section 8).
+constexpr int MUSTA_YG = 2;      // cp.async groups in flight, two cells each
 template <class T>
 constexpr size_t musta_y_smem_bytes() {
-    return sizeof(T) * ((size_t)MUSTA_DEPTH * (NF + NF) + NF) * MUSTA_THREADS;
+    return sizeof(T) * ((size_t)2 * MUSTA_YG * (NF + NF) + NF) * MUSTA_THREADS;
 }
 
 template <class T, bool EPI, bool FAST>
-__global__ void __launch_bounds__(MUSTA_THREADS, 4)
+__global__ void __launch_bounds__(MUSTA_THREADS, MUSTA_Y_MINB)
 musta_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl, int yc) {
-    constexpr int R = MUSTA_R, M = 2 * R, NVO = NF + NF, D = MUSTA_DEPTH, TH = MUSTA_THREADS;
+    constexpr int R = MUSTA_R, NVO = NF + NF, TH = MUSTA_THREADS, NG = MUSTA_YG;
+    constexpr int LIMS = FAST ? 0 : -1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* sm = reinterpret_cast<T*>(smem_raw);   // [D][NVO][TH], then [NF][TH]
+    T* sm = reinterpret_cast<T*>(smem_raw);   // [NG][2][NVO][TH], then [NF][TH]
     const int tid = threadIdx.x + 32 * threadIdx.y;
-    T* park = sm + D * NVO * TH + tid;
+    T* park = sm + 2 * NG * NVO * TH + tid;
     const int i = blockIdx.x * 32 + threadIdx.x;
     const int kz = blockIdx.y * MUSTA_ROWS + threadIdx.y;
     // lanes beyond the grid leave; the ballot (taken while the warp is whole) is the mask of the final reduction
@@ -229,59 +304,110 @@ musta_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl,
     const int j0 = (int)blockIdx.z * yc;
     const int j1 = min(j0 + yc, G.n[1]);
     const long long p0 = G.pidx(i, j0, kz);
+    const int lim = A.limiter;
+    const T C = (T)A.musta_C, invC = fast_rcp(C);
     int flag = 0;
-    auto issue = [&](int j) {
-        if (j < j1) {
-            T* dst = sm + ((j - j0) % D) * NVO * TH + tid;
-            const long long q = p0 + (long long)(j - j0) * ms;
-            const long long qr = q + (long long)R * ms;
+    // group g = cells j0 + 2g, j0 + 2g + 1: per cell the stencil cell R ahead and the old output
+    auto issue = [&](int g) {
 #pragma unroll
-            for (int c = 0; c < NF; ++c) cp_async<sizeof(T)>(dst + c * TH, Us + c * G.fs + qr);
+        for (int h = 0; h < 2; ++h) {
+            const int j = j0 + 2 * g + h;
+            if (j < j1) {
+                T* dst = sm + ((g % NG) * 2 + h) * NVO * TH + tid;
+                const long long q = p0 + (long long)(j - j0) * ms;
+                const long long qr = q + (long long)R * ms;
 #pragma unroll
-            for (int c = 0; c < NF; ++c) cp_async<sizeof(T)>(dst + (NF + c) * TH, Uout + c * G.fs + q);
+                for (int c = 0; c < NF; ++c) cp_async<sizeof(T)>(dst + c * TH, Us + c * G.fs + qr);
+#pragma unroll
+                for (int c = 0; c < NF; ++c) cp_async<sizeof(T)>(dst + (NF + c) * TH, Uout + c * G.fs + q);
+            }
         }
         cp_async_commit();
     };
 #pragma unroll
-    for (int d = 0; d < D; ++d) issue(j0 + d);
+    for (int g = 0; g < NG; ++g) issue(g);
 
-    MustaWindow<T> zw;
-    T nxt[NF];
+    MustaColumn<T, LIMS> col;
+    {   // face j0 - 1/2 from cells j0-2 .. j0+1, then the column state of cell j0
+        T c[4][NF];
 #pragma unroll
-    for (int m = 0; m < M; ++m) {
+        for (int m = 0; m < 4; ++m) {
 #pragma unroll
-        for (int c = 0; c < NF; ++c) nxt[c] = __ldg(Us + c * G.fs + p0 + (long long)(m - R) * ms);
-        zw.put(m, nxt);
+            for (int f = 0; f < NF; ++f) c[m][f] = __ldg(Us + f * G.fs + p0 + (long long)(m - R) * ms);
+        }
+        col.init(c[0], c[1], c[2], lim);
+        T qr[NF], f0[NF];
+        col.advance(c[3], lim, qr);
+        if (FAST) {
+            bool bad = false;
+            musta_force_fast4<T, 1, 2>(col.ql, qr, C, invC, f0, bad);
+            if (bad) musta_general4<T, 1, FAST>(col.ql, qr, A, C, f0, flag);
+        } else {
+            musta_general4<T, 1, FAST>(col.ql, qr, A, C, f0, flag);
+        }
+        col.commit(c[3]);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) park[f * TH] = f0[f];
     }
-    {
-        T f0[NF];
-        musta_iface<T, 1, FAST>(zw, A, f0, flag);
-#pragma unroll
-        for (int c = 0; c < NF; ++c) park[c * TH] = f0[c];
-    }
-    const T coef = A.mode == 1 ? (T)A.inv_dx : (T)(A.cb * ctl->dt * A.inv_dx);
+    // four times the flux comes in
+    const T coef = A.mode == 1 ? (T)(0.25 * A.inv_dx) : (T)(0.25 * A.cb * ctl->dt * A.inv_dx);
     double amax = 0.0;
-    for (int j = j0; j < j1; ++j) {
-        T f[NF], o[NF];
-        cp_async_wait<D - 1>();   // the oldest stage (cell j) has landed
-        const T* src = sm + ((j - j0) % D) * NVO * TH + tid;
-#pragma unroll
-        for (int c = 0; c < NF; ++c) nxt[c] = src[c * TH];
-        zw.shift();
-        zw.put(M - 1, nxt);
-        musta_iface<T, 1, FAST>(zw, A, f, flag);
-        const long long q = p0 + (long long)(j - j0) * ms;
+    const int ng = (j1 - j0 + 1) / 2;
+    for (int g = 0; g < ng; ++g) {
+        const int j = j0 + 2 * g;
+        const bool second = j + 1 < j1;   // an odd chunk ends on a half group: its second cell is computed on stale
+                                          // slots and thrown away
+        cp_async_wait<NG - 1>();          // the oldest group has landed
+        const T* src = sm + (g % NG) * 2 * NVO * TH + tid;
+        T ua[NF], ub[NF], qla[NF], qra[NF], qlb[NF], qrb[NF], fa[NF], fb[NF];
 #pragma unroll
         for (int c = 0; c < NF; ++c) {
-            o[c] = tfma(coef, park[c * TH] - f[c], src[(NF + c) * TH]);   // old output: read late
-            Uout[c * G.fs + q] = o[c];
-            park[c * TH] = f[c];
+            ua[c] = src[c * TH];
+            ub[c] = src[(NVO + c) * TH];
+            qla[c] = col.ql[c];
         }
-        issue(j + D);             // refill the slot just consumed
-        if (EPI) {   // a4 of the finished cell (all three axes are active whenever this kernel runs)
+        col.advance(ua, lim, qra);
+        col.commit(ua);
+#pragma unroll
+        for (int c = 0; c < NF; ++c) qlb[c] = col.ql[c];
+        col.advance(ub, lim, qrb);
+        col.commit(ub);
+        if (FAST) {   // both interfaces in one basic block; the rare repairs afterwards
+            bool bada = false, badb = false;
+            musta_force_fast4<T, 1, 2>(qla, qra, C, invC, fa, bada);
+            musta_force_fast4<T, 1, 2>(qlb, qrb, C, invC, fb, badb);
+            if (bada) musta_general4<T, 1, FAST>(qla, qra, A, C, fa, flag);
+            if (badb && second) musta_general4<T, 1, FAST>(qlb, qrb, A, C, fb, flag);
+        } else {
+            musta_general4<T, 1, FAST>(qla, qra, A, C, fa, flag);
+            int f2 = 0;
+            musta_general4<T, 1, FAST>(qlb, qrb, A, C, fb, f2);
+            if (second) flag |= f2;
+        }
+        const long long q = p0 + (long long)(j - j0) * ms;
+        T oa[NF], ob[NF];
+#pragma unroll
+        for (int c = 0; c < NF; ++c) {
+            oa[c] = tfma(coef, park[c * TH] - fa[c], src[(NF + c) * TH]);   // old output: read late
+            Uout[c * G.fs + q] = oa[c];
+        }
+        if (second) {
+#pragma unroll
+            for (int c = 0; c < NF; ++c) {
+                ob[c] = tfma(coef, fa[c] - fb[c], src[(NVO + NF + c) * TH]);
+                Uout[c * G.fs + q + ms] = ob[c];
+                park[c * TH] = fb[c];
+            }
+        }
+        issue(g + NG);            // refill the slots just consumed
+        if (EPI) {   // a4 of the finished cells (all three axes are active whenever this kernel runs)
             T w[NW];
-            prim_of_cell(o, w, flag, A.eos);
+            prim_of_cell(oa, w, flag, A.eos);
             amax = fmax(amax, fmax((double)w[W_AX], fmax((double)w[W_AX + 1], (double)w[W_AX + 2])));
+            if (second) {
+                prim_of_cell(ob, w, flag, A.eos);
+                amax = fmax(amax, fmax((double)w[W_AX], fmax((double)w[W_AX + 1], (double)w[W_AX + 2])));
+            }
         }
     }
     if (EPI) warp_max_to(amax, &ctl->maxspeed_next_bits, wmask);
