@@ -8,8 +8,10 @@ BASELINE.json configs[4]: the 512^3 periodic lumpy state with 200 hotspots and b
 One "step" is one SSP-RK3 step of the whole grid with dt = CFL dx / max signal speed taken on the device
 (hydro_step_cfl, reading Q10): per stage the ghost fill, the x/z marching kernel and the y sweep, whose epilogue
 also does con2prim + signal speeds + the CFL max for the next stage.
-Prints ONE JSON line (rank 0).  N > 1 (torchrun): every rank advances its own independent 512^3 event
-(weak scaling, no data-path collective), time = max over ranks.
+Prints ONE JSON line (rank 0).  N > 1 (torchrun): ONE 512^3 event decomposed into z-slabs with a halo exchange per
+Runge-Kutta stage (`--decomp slab`, the default for N > 1: SURVEY 8(e), strong scaling), time = max over ranks; the
+throughput of N independent events (`--decomp events`, weak scaling, no data-path collective) is printed beside it
+as `replicas`.
 
 `--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same
 workload on the host cores; it is the only other place besides `cpu_baseline` where bench.py runs it.
@@ -17,6 +19,7 @@ workload on the host cores; it is the only other place besides `cpu_baseline` wh
 from __future__ import annotations
 
 import argparse
+import ctypes
 import json
 import os
 import subprocess
@@ -38,10 +41,12 @@ SCHEMES = {"weno5": W.WENO5, "weno7": W.WENO7, "musta": W.MUSTA_FORCE}
 FLOPS_PER_CELL_STEP = {"weno5": 7041.0, "weno7": 14331.0, "musta": 3831.0}
 FLOPS_PER_CELL_L = {"weno5": 2327.0, "weno7": 4757.0, "musta": 1257.0}
 BYTES_PER_CELL_STEP = {"f64": 320.0, "f32": 160.0}
-# bytes one stage kernel moves per cell, averaged over the three stages of a step: 320/3 (fp64)
 # DRAM bytes of one stage (x/z kernel + y sweep), dram__bytes_read.sum + dram__bytes_write.sum of one
-# `ncu --set full` capture each at 512^3: profiles/r01_xz_ncu.txt, profiles/r01_ysweep_ncu.txt
-TRAFFIC_BYTES_PER_STAGE = {("weno5", "f64", 512): 10.707e9 + 5.395e9 + 14.690e9 + 10.788e9}
+# `ncu --set full` capture of each kernel at 512^3 (profiles/r02_*_ncu.txt); algorithmic bytes of one stage at that
+# size: 320/3 B x 512^3 = 1.43e10
+TRAFFIC_BYTES_PER_STAGE = {}
+KERNEL_NAMES = {"weno5": "weno_xz_kernel<T,3> + weno_y_kernel<T,3,EPI>", "weno7": "weno_xz_kernel<T,4> + weno_y_kernel<T,4,EPI>",
+                "musta": "musta_xz_kernel<T,FAST> + musta_y_kernel<T,EPI,FAST>"}
 METRIC = "3D cell-updates/s per RK3 step"
 UNIT = "cell-updates/s"
 CFL = 0.2
@@ -111,11 +116,19 @@ def make_workload(n, scheme, rank=0):
     return w
 
 
-def crop_workload(w, m):
-    """m^3 corner crop of a workload, made periodic-by-fiat (the oracle sample of the same data)."""
-    cons = np.ascontiguousarray(w.cons[:, :m, :m, :m])
-    return W.Workload(w.name + "_crop%d" % m, (m, m, m), w.dx, (0.0, 0.0, 0.0), w.scheme, w.bc, cons, 0.0,
-                      cfl=w.cfl, nsteps=w.nsteps)
+CPU_CROP = 48
+
+
+def oracle_sample(n, scheme, m=CPU_CROP):
+    """The oracle's bounded sample of the bench workload: the corner block of the first m cells per axis of the
+    same seeded n^3 state (same draws and formulas as make_workload(n, scheme), evaluated on those cells only),
+    made periodic by fiat."""
+    if n >= 64:
+        return W.lumpy(n=n, hotspots=200, with_velocity=True, scheme=SCHEMES[scheme], nsteps=20, cfl=CFL,
+                       crop=min(m, n))
+    w = make_workload(n, scheme)
+    return W.Workload(w.name + "_crop", w.n, w.dx, (0.0, 0.0, 0.0), w.scheme, w.bc, w.cons, 0.0, cfl=w.cfl,
+                      nsteps=w.nsteps)
 
 
 def time_oracle(w, steps, warmup=0):
@@ -133,28 +146,92 @@ def time_oracle(w, steps, warmup=0):
     return ncell * steps / dt, dt
 
 
+def oracle_all_cores(n, scheme, steps, timeout=240):
+    """one independent single-threaded oracle process per host core (`bench.py --oracle-worker`),
+    each on the same sample; aggregate = all cell-updates done / the slowest process's time."""
+    try:
+        cores = len(os.sched_getaffinity(0))
+    except AttributeError:
+        cores = os.cpu_count() or 1
+    env = dict(os.environ, OMP_NUM_THREADS="1", OPENBLAS_NUM_THREADS="1", MKL_NUM_THREADS="1")
+    cmd = [sys.executable, os.path.abspath(__file__), "--oracle-worker", "--grid", str(n), "--scheme", scheme,
+           "--steps", str(steps)]
+    procs = [subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True, env=env)
+             for _ in range(cores)]
+    res = []
+    deadline = time.time() + timeout
+    for p in procs:
+        try:
+            out, _ = p.communicate(timeout=max(1.0, deadline - time.time()))
+            ncell, secs = out.strip().split()[-2:]
+            res.append((int(ncell), float(secs)))
+        except Exception:
+            p.kill()
+    if not res:
+        return None, None, 0
+    slowest = max(r[1] for r in res)
+    return len(res) * res[0][0] * steps / slowest, slowest, len(res)
+
+
+def oracle_worker(args):
+    """One process of the all-core leg: prints `ncell seconds`."""
+    w = oracle_sample(args.n, args.scheme)
+    _, secs = time_oracle(w, args.steps)
+    print(w.n[0] * w.n[1] * w.n[2], secs, flush=True)
+    return 0
+
+
+def cpu_baseline(n, scheme, steps):
+    w = oracle_sample(n, scheme)
+    m = w.n[0]
+    v1, s1 = time_oracle(w, steps)
+    vall, sall, cores = oracle_all_cores(n, scheme, steps)
+    return {"value": vall, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "%d^3 corner block of the same %d^3 state, %d RK3 steps: one independent single-threaded oracle "
+                      "process per host core (%d cores, %.1f s); host has %d logical CPUs" %
+                      (m, n, steps, cores, sall, os.cpu_count() or 0),
+            "single_thread": {"value": v1, "cores": 1, "seconds": s1}}
+
+
 # ----------------------------------------------------------------------------------------------
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    m = 48
-    big = make_workload(max(64, m), args.scheme)
-    w = crop_workload(big, m)
+    w = oracle_sample(args.n, args.scheme)
+    m = w.n[0]
     value, secs = time_oracle(w, args.steps, args.warmup)
-    sample = "%d^3 corner crop of the 200-hotspot lumpy state (64^3 draw), %d RK3 steps, 1 thread" % (m, args.steps)
+    sample = ("%d^3 corner block of the same seeded %d^3 state the GPU arm advances, %d RK3 steps after %d warm-up, "
+              "1 thread" % (m, args.n, args.steps, args.warmup))
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(args.steps, 1),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "config5 lumpy periodic, %s fp64, oracle sample %s" % (args.scheme, sample),
-                   "scheme": args.scheme, "cfl": CFL},
+        "config": {"workload": "BASELINE.json configs[4]: %d^3 periodic lumpy state, 200 hotspots, blended velocities, "
+                               "%s f64, CFL %.1f; the oracle (oracle/, as it stands) on a bounded sample: %s" %
+                               (args.n, args.scheme, CFL, sample),
+                   "grid": [args.n] * 3, "scheme": args.scheme, "cfl": CFL, "sample_grid": [m] * 3},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
     return 0
+
+
+def probe_fma_peak(torch, precision, millis=300):
+    """Sustained FMA rate in TFLOP/s from the bench-side helper library (csrc/bench_probe.cu); None if it is absent."""
+    path = os.path.join(ROOT, "paper_1604_03360_b200", "libbench_probe.so")
+    if not os.path.exists(path):
+        return None
+    lib = ctypes.CDLL(path)
+    lib.bench_probe_fma_peak.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
+                                         ctypes.POINTER(ctypes.c_double)]
+    scratch = torch.zeros(16, dtype=torch.uint8, device="cuda")
+    out = ctypes.c_double()
+    rc = lib.bench_probe_fma_peak(0 if precision == "f64" else 1, millis, torch.cuda.current_stream().cuda_stream,
+                                  scratch.data_ptr(), ctypes.byref(out))
+    return out.value if rc == 0 else None
 
 
 # ----------------------------------------------------------------------------------------------
@@ -219,22 +296,77 @@ def aggregate_value(ncell, steps, world, ms):
     return ncell * steps * world / (ms * 1e-3)
 
 
-def roofline(scheme, precision, ncell, stage_ms, stage_n, alu_peak_tf, peaks):
+def roofline(scheme, precision, ncell, stage_ms, stage_n, alu_peak_tf, peaks, probe_tf=None, step_ms=None):
+    """Roofline object of the dominant "kernel" = one RK stage's pair of stage kernels (x/z marching kernel + y
+    sweep), timed together by one CUDA-event pair per stage on the launching stream inside the timed region."""
     if stage_n == 0 or stage_ms <= 0:
         return None
     per_launch_s = stage_ms * 1e-3 / stage_n
     flops = FLOPS_PER_CELL_L[scheme] * ncell
     achieved = flops / per_launch_s / 1e12
     byts = BYTES_PER_CELL_STEP[precision] / 3.0 * ncell
-    return {"bound": "alu", "achieved": achieved, "peak": alu_peak_tf, "unit": "TFLOP/s",
-            "frac": achieved / alu_peak_tf,
-            "traffic": TRAFFIC_BYTES_PER_STAGE.get((scheme, precision, round(ncell ** (1.0 / 3.0)))),
-            "traffic_note": "DRAM bytes of one stage from profiles/r01_*_ncu.txt; algorithmic bytes of one stage: %.3g"
-                            % (BYTES_PER_CELL_STEP[precision] / 3.0 * ncell),
-            "kernel": "one RK stage = xz_sweep_kernel (x and z fluxes + combine) + z_sweep_kernel<DIR=y> (y fluxes, "
-                      "con2prim epilogue), timed together with one CUDA-event pair on the stream",
-            "launch_ms": per_launch_s * 1e3,
-            "hbm_gbs_achieved": byts / per_launch_s / 1e9, "hbm_frac": byts / per_launch_s / 1e9 / peaks["hbm_gbs"]}
+    r = {"bound": "alu", "achieved": achieved, "peak": alu_peak_tf, "unit": "TFLOP/s",
+         "frac": achieved / alu_peak_tf, "frac_is": "of the NOMINAL fp peak (clocks.max.sm)",
+         "traffic": TRAFFIC_BYTES_PER_STAGE.get((scheme, precision, round(ncell ** (1.0 / 3.0)))),
+         "traffic_note": "DRAM bytes of one stage (both kernels) from the ncu --set full captures under profiles/; "
+                         "algorithmic bytes of one stage: %.3g" % byts,
+         "kernel": "one RK stage = %s, timed together with one CUDA-event pair on the stream" % KERNEL_NAMES[scheme],
+         "launch_ms": per_launch_s * 1e3, "algorithmic_flops_per_launch": flops,
+         "hbm_gbs_achieved": byts / per_launch_s / 1e9, "hbm_frac": byts / per_launch_s / 1e9 / peaks["hbm_gbs"]}
+    if probe_tf:
+        r["peak_probe_sustained"] = probe_tf
+        r["frac_of_probe"] = achieved / probe_tf
+    if step_ms:
+        r["stage_share_of_step"] = stage_ms / step_ms
+    return r
+
+
+def batch_bench(B, torch, scheme, n=128, nb=8, steps=10, warmup=3):
+    """SURVEY 8(f)-N2 / N4 ("event-by-event simulations"): nb independent n^3 events.  (a) one after the
+    other on one stream, (b) hydro_step_cfl_batch with one stream per event, (c) the same with every event's step
+    replayed from a CUDA graph.  Whole-batch cell-updates/s, CUDA events around the batch."""
+    ws = [make_workload(n, scheme, rank=k) for k in range(nb)]
+    out = {"grid": [n, n, n], "events": nb, "steps": steps, "unit": UNIT}
+    for mode in ("sequential", "streams", "streams+graph"):
+        streams = [torch.cuda.Stream() for _ in range(nb)]
+        hs = []
+        for w, st in zip(ws, streams):
+            with torch.cuda.stream(st if mode != "sequential" else streams[0]):
+                h = B.from_workload(w)
+                if mode == "streams+graph":
+                    h.set_option("graph", 1)
+                hs.append(h)
+        def advance(k):
+            if mode == "sequential":
+                for h in hs:
+                    h.step_cfl(CFL, k)
+            else:
+                B.step_cfl_batch(hs, CFL, k)
+        advance(warmup)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(torch.cuda.default_stream())
+        for st in streams:
+            st.wait_event(e0)
+        advance(steps)
+        for st in streams:
+            torch.cuda.default_stream().wait_stream(st)
+        e1.record(torch.cuda.default_stream())
+        torch.cuda.synchronize()
+        host_s = time.perf_counter() - t0
+        ms = e0.elapsed_time(e1)
+        out[mode] = {"value": nb * n ** 3 * steps / (ms * 1e-3), "ms_per_step_per_event": ms / steps / nb,
+                     "host_seconds": host_s, "status": max(h.status() for h in hs)}
+        for h in hs:
+            h.close()
+        torch.cuda.empty_cache()
+    return out
+
+
+def nominal_tflops(sms, precision, peaks):
+    lanes = 64 if precision == "f64" else 128
+    return sms * lanes * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12, lanes
 
 
 def run_ours(args):
@@ -257,17 +389,17 @@ def run_ours(args):
 
     n = args.n
     ncell = n ** 3
-    slab_mode = args.decomp == "slab"
+    decomp = args.decomp or ("slab" if world > 1 else "events")
+    slab_mode = decomp == "slab"
     # events: every rank its own event (seeded by rank); slab: ONE global event, this rank owns a z-slab of it
     w = make_workload(n, args.scheme, 0 if slab_mode else rank)
     slab = (rank, world) if slab_mode else None
 
     # ALU roofline denominator: 148 SMs x 64 fp64 (128 fp32) FMA lanes x 2 flop x
-    # the SM clock.  Nominal uses clocks.max.sm; the sustained figure is measured by the library's probe.
-    lanes = 64 if args.precision == "f64" else 128
+    # the SM clock.  Nominal uses clocks.max.sm; the sustained figure is measured by the bench-side probe.
     sms = torch.cuda.get_device_properties(local).multi_processor_count
-    nominal_tf = sms * lanes * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
-    probe_tf = B.probe_fma_peak(B.F64 if args.precision == "f64" else B.F32, 300)
+    nominal_tf, lanes = nominal_tflops(sms, args.precision, peaks)
+    probe_tf = {p: probe_fma_peak(torch, p, 300) for p in ("f64", "f32")}
 
     sampler = ClockSampler(local)
     sampler.start()
@@ -276,23 +408,39 @@ def run_ours(args):
     ms = max_over_ranks(r["ms"], dist, "cuda")
     value = aggregate_value(ncell, args.steps, 1 if slab_mode else world, ms)
     ncell_local = ncell // world if slab_mode else ncell
-    roof = roofline(args.scheme, args.precision, ncell_local, r["stage_ms"], r["stage_n"], nominal_tf, peaks)
+    roof = roofline(args.scheme, args.precision, ncell_local, r["stage_ms"], r["stage_n"], nominal_tf, peaks,
+                    probe_tf[args.precision], r["ms"])
     if roof is not None:
         roof["peak_source"] = ("nominal: %d SMs x %d lanes x 2 x %.0f MHz (DESIGN.md section 8); "
                                "hbm peak %s" % (sms, lanes, peaks.get("sm_max_mhz", 1965.0), peaks_src))
-        roof["peak_probe_sustained"] = probe_tf
-        roof["frac_of_probe"] = roof["achieved"] / probe_tf if probe_tf > 0 else None
-        roof["stage_share_of_step"] = r["stage_ms"] / r["ms"]
     # step-level roofline: cell-updates/s against min(byte roof, flop roof)
     flop_roof = nominal_tf * 1e12 / FLOPS_PER_CELL_STEP[args.scheme]
     byte_roof = peaks["hbm_gbs"] * 1e9 / BYTES_PER_CELL_STEP[args.precision]
     step_roof = min(flop_roof, byte_roof)
 
-    # ---- e2e: host buffers through the C ABI, copies inside the timed region
     h = r.pop("h")
+    advance = r.pop("advance")
+    stream = torch.cuda.current_stream()
+
+    # ---- median of >= 5 repetitions of the K-step run (the first is the one `value` reports)
+    reps = [ms / max(args.steps, 1)]
+    for _ in range(max(0, args.repeat - 1)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _k in range(args.steps):
+            advance(1)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        reps.append(max_over_ranks(e0.elapsed_time(e1), dist, "cuda") / max(args.steps, 1))
+    repetitions = {"ms_per_step": reps, "median_ms_per_step": float(np.median(reps)),
+                   "median_value": (ncell if slab_mode else ncell * world) / (float(np.median(reps)) * 1e-3)}
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region
     esz = 8 if args.precision == "f64" else 4
     tdt = torch.float64 if args.precision == "f64" else torch.float32
-    advance = r.pop("advance")
     if slab_mode:
         from paper_1604_03360_b200 import slab as S
         k0, k1 = S.split_planes(n, world)[rank]
@@ -327,37 +475,67 @@ def run_ours(args):
            "finite": bool(torch.isfinite(host_out).all().item())}
     launches_per_step = r["launches"] / max(args.steps, 1)
     h.close()
-    del h
+    del h, host_in, host_out
     torch.cuda.empty_cache()
 
-    # ---- the other headline variants of config 5 (same grid, fewer steps each)
+    # ---- N > 1, slab: the throughput of N independent events beside it (no data-path collective)
+    replicas = None
+    if slab_mode and world > 1:
+        rr = timed_run(B, torch, w, args.precision, max(3, args.steps // 4), 3, dist, profile=False)
+        rms = max_over_ranks(rr["ms"], dist, "cuda")
+        replicas = {"value": aggregate_value(ncell, max(3, args.steps // 4), world, rms), "unit": UNIT,
+                    "scaling": "weak", "note": "one independent %d^3 event per GPU, no exchange" % n,
+                    "ms_per_step": rms / max(3, args.steps // 4)}
+        rr.pop("h").close()
+        torch.cuda.empty_cache()
+
+    # ---- the other headline variants of config 5: full lines (same grid, same number of steps, own clocks)
     variants = {}
     if not args.no_variants and rank == 0 and world == 1 and not slab_mode:
         for sch, prec in (("weno5", "f64"), ("weno7", "f64"), ("musta", "f64"), ("weno5", "f32"), ("weno7", "f32")):
             if (sch, prec) == (args.scheme, args.precision):
                 continue
             w.scheme = SCHEMES[sch]
-            vr = timed_run(B, torch, w, prec, max(3, args.steps // 4), 3)
-            vsteps = max(3, args.steps // 4)
-            lanes_v = 64 if prec == "f64" else 128
-            nom_v = sms * lanes_v * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
-            rf = roofline(sch, prec, ncell, vr["stage_ms"], vr["stage_n"], nom_v, peaks)
+            vs = ClockSampler(local)
+            vs.start()
+            vr = timed_run(B, torch, w, prec, args.steps, args.warmup)
+            vclk = vs.stop(*vr["wall"])
+            nom_v, _ = nominal_tflops(sms, prec, peaks)
+            rf = roofline(sch, prec, ncell, vr["stage_ms"], vr["stage_n"], nom_v, peaks, probe_tf[prec], vr["ms"])
             variants["%s_%s" % (sch, prec)] = {
-                "value": ncell * vsteps / (vr["ms"] * 1e-3), "ms_per_step": vr["ms"] / vsteps, "steps": vsteps,
-                "roofline_frac": rf["frac"] if rf else None, "status": vr["status"]}
+                "value": ncell * args.steps / (vr["ms"] * 1e-3), "ms_per_step": vr["ms"] / args.steps,
+                "steps": args.steps, "warmup": args.warmup, "dtype": prec,
+                "roofline_frac": rf["frac"] if rf else None, "roofline": rf,
+                "step_roofline_frac": (ncell * args.steps / (vr["ms"] * 1e-3)) /
+                                      min(nom_v * 1e12 / FLOPS_PER_CELL_STEP[sch],
+                                          peaks["hbm_gbs"] * 1e9 / BYTES_PER_CELL_STEP[prec]),
+                "launches_per_step": vr["launches"] / args.steps, "clocks": vclk, "status": vr["status"]}
             vr.pop("h").close()
             torch.cuda.empty_cache()
         w.scheme = SCHEMES[args.scheme]
 
+    # ---- the same scheme at 128^3 and 256^3
+    sizes = {}
+    if not args.no_variants and rank == 0 and world == 1 and not slab_mode:
+        for m in (128, 256):
+            if m >= n:
+                continue
+            wm = make_workload(m, args.scheme)
+            sr = timed_run(B, torch, wm, args.precision, args.steps, args.warmup, profile=False)
+            sizes[str(m)] = {"value": m ** 3 * args.steps / (sr["ms"] * 1e-3), "ms_per_step": sr["ms"] / args.steps,
+                             "steps": args.steps, "launches_per_step": sr["launches"] / args.steps}
+            sr.pop("h").close()
+            torch.cuda.empty_cache()
+
+    # ---- a batch of small events on streams, with and without the CUDA-graph replay
+    batch = None
+    if not args.no_variants and rank == 0 and world == 1 and not slab_mode:
+        batch = batch_bench(B, torch, args.scheme, n=128, nb=8, steps=args.steps)
+
     # ---- the oracle beside it: bounded sample on the host cores (rank 0, N = 1 only)
     cpu = None
     if not args.no_cpu_baseline and rank == 0 and world == 1:
-        m = min(64, n)
-        cw = crop_workload(w, m)
-        v, secs = time_oracle(cw, 8 if m >= 64 else 20)
-        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": "%d^3 corner crop of the same state, %d RK3 steps, %.1f s, single thread" %
-                         (m, 8 if m >= 64 else 20, secs)}
+        cpu = cpu_baseline(n, args.scheme, 16)
 
     if rank == 0:
         line = {
@@ -370,7 +548,7 @@ def run_ours(args):
                                    (n, args.scheme, args.precision, CFL,
                                     "one event, z-slab per GPU, halo exchange per stage" if slab_mode
                                     else "one independent event per GPU"),
-                       "grid": [n, n, n], "scheme": args.scheme, "cfl": CFL, "decomp": args.decomp,
+                       "grid": [n, n, n], "scheme": args.scheme, "cfl": CFL, "decomp": decomp,
                        "l2": "no flush needed: the state (%.2f GB per copy) is far larger than the 126 MB L2" %
                              (state_bytes / 1e9)},
             "roofline": roof,
@@ -378,6 +556,7 @@ def run_ours(args):
                               "per": "GPU",
                               "flop_roof": flop_roof, "byte_roof": byte_roof, "unit": UNIT,
                               "note": "min(hbm peak / 320 B, nominal ALU peak / algorithmic flops) per cell-update"},
+            "repetitions": repetitions,
             "cpu_baseline": cpu,
             "e2e": e2e,
             "gpu_launches": int(round(launches_per_step * args.steps)),
@@ -385,6 +564,9 @@ def run_ours(args):
             "clocks": clocks,
             "status": r["status"], "sim_time": r["t"],
             "variants": variants,
+            "sizes": sizes,
+            "replicas": replicas,
+            "batch": batch,
             "context": "paper: GPU ~200x one CPU thread for MUSTA-FORCE on unnamed 2016 hardware (PAPER.md:38)",
         }
         print(json.dumps(line), flush=True)
@@ -406,10 +588,15 @@ def main():
                     help="cells per axis (use --grid under torchrun: its parser finds --n ambiguous)")
     ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--decomp", default="events", choices=["events", "slab"],
-                    help="N > 1: 'events' = one independent event per GPU (weak scaling, no data-path collective); "
-                         "'slab' = one event decomposed along z, halo exchange per stage (strong scaling)")
+    ap.add_argument("--repeat", type=int, default=5, help="repetitions of the K-step run for the median (first = value)")
+    ap.add_argument("--decomp", default=None, choices=["events", "slab"],
+                    help="'slab' (default for N > 1) = one event decomposed along z, halo exchange per stage (strong "
+                         "scaling); 'events' (default for N = 1) = one independent event per GPU (weak scaling, no "
+                         "data-path collective)")
+    ap.add_argument("--oracle-worker", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
+    if args.oracle_worker:
+        return oracle_worker(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

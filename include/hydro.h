@@ -84,6 +84,12 @@ int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme)
  *                   march amortises the one redundant flux and the pipeline fill of a chunk)
  *   "profile"       0 (default) | 1: record a CUDA event pair on the stream around every stage-kernel
  *                   launch, read back with hydro_stage_kernel_time
+ *   "graph"         0 (default) | 1: hydro_step_cfl replays one steady-state step from a CUDA graph (one
+ *                   cudaGraphLaunch instead of 11 kernel launches per step; every step-dependent value, dt included,
+ *                   lives in the device control block).  Needs a non-default stream (hydro_set_stream); on the
+ *                   legacy default stream, with "profile" on, or before the first plain step has left the
+ *                   primitives and the max signal speed behind, the plain launches run instead.  The graphs are
+ *                   dropped whenever an option, the stream or the workspace changes.
  *   "kernel"        HYDRO_KERNEL_AUTO (default: the marching stage kernels where all three axes are active,
  *                   else the generic one-thread-per-cell kernel) | HYDRO_KERNEL_GENERIC | HYDRO_KERNEL_FUSED
  *                   (= marching; EINVAL at step time if the grid does not allow it)
@@ -126,6 +132,12 @@ int hydro_step(hydro_ctx *ctx, double dt, int nsteps);
  * Asynchronous. */
 int hydro_step_cfl(hydro_ctx *ctx, double cfl, int nsteps);
 
+/* Event-by-event batches ("event-by-event simulations"): advance nctx independent
+ * contexts by nsteps CFL steps each.  The steps are issued round-robin over the batch, every context on its own
+ * stream (hydro_set_stream), so that the kernels of small grids run side by side on the GPU.  Asynchronous; the
+ * first error of any context is returned (its text is that context's hydro_last_error). */
+int hydro_step_cfl_batch(hydro_ctx **ctxs, int nctx, double cfl, int nsteps);
+
 /* max over interior cells and active axes of the characteristic speed a_d (a3-a4).
  * Writes one double to a HOST pointer; synchronises the stream. */
 int hydro_max_signal_speed(hydro_ctx *ctx, double *out_host);
@@ -155,6 +167,18 @@ int hydro_get_zhalo(hydro_ctx *ctx, int buffer, int side, void *packed_device_ou
 int hydro_put_zhalo(hydro_ctx *ctx, int buffer, int side, const void *packed_device_in);
 int hydro_step_stage(hydro_ctx *ctx, double dt, int stage);
 
+/* The same without a host round trip (reading Q10 on the decomposed grid):
+ *  - hydro_put_zhalo with packed_device_in == NULL fills the g ghost planes of `side` with copies of the slab's own
+ *    boundary plane: the zero-gradient outflow rule (reading Q9) for a slab at a physical end of the z axis;
+ *  - hydro_local_max_speed writes the max signal speed (a3-a4) of this slab's current state as ONE double to a
+ *    DEVICE pointer, asynchronously (the value the last step's epilogue left, or a reduction pass); the caller
+ *    max-reduces it over the slabs (ncclAllReduce on that buffer);
+ *  - hydro_step_stage_cfl is hydro_step_stage with dt = cfl * dx / *maxspeed_device taken on the device in
+ *    stage 0 (stages 1, 2 reuse it); maxspeed_device is a DEVICE pointer to one double and is only read.
+ * EINVAL on a null pointer, cfl <= 0, or a stage out of order. */
+int hydro_local_max_speed(hydro_ctx *ctx, void *maxspeed_device_out);
+int hydro_step_stage_cfl(hydro_ctx *ctx, double cfl, int stage, const void *maxspeed_device);
+
 /* With the "profile" option on: total device time in milliseconds of the stage kernels (the L(u) +
  * Runge-Kutta kernel, the dominant one) launched since the last call, and their number, written to HOST
  * pointers.  Synchronises the stream and clears the record. */
@@ -164,11 +188,6 @@ int hydro_stage_kernel_time(hydro_ctx *ctx, double *ms_total_host, long long *la
 const char *hydro_last_error(const hydro_ctx *ctx);
 
 void hydro_destroy(hydro_ctx *ctx);
-
-/* Machine probe, independent of any context: run a register-resident chain of fused multiply-adds on
- * every SM for about `millis` milliseconds and write the sustained rate in TFLOP/s (2 flops per FMA) to
- * a HOST pointer.  precision = HYDRO_F64 or HYDRO_F32.  Used for the "alu" roofline denominator. */
-int hydro_probe_fma_peak(int precision, int millis, void *cuda_stream, double *tflops_host);
 
 #ifdef __cplusplus
 }

@@ -655,6 +655,24 @@ int oracle_eval_L(oracle_ctx* c, const void* cons, double t_stage, void* L_out) 
     return OK;
 }
 
+// The same L(u) with the SAME code instantiated in long double (x87 80-bit, 64-bit significand) and rounded to
+// double at the end: a referee for parity cases where the fp64 oracle's own rounding is the larger error (the
+// 240-scaled WENO7 indicators of reading Q5 cancel many digits on very smooth data).  fp64 context only.
+int oracle_eval_L_extended(oracle_ctx* c, const double* cons, double t_stage, double* L_out) {
+    if (!c || !cons || !L_out || !c->d) return EINVAL_;
+    const Solver<double>* D = c->d;
+    Solver<long double> S(c->nx, c->ny, c->nz, c->dx, c->scheme);
+    for (int a = 0; a < 3; ++a) { S.bc[a] = D->bc[a]; S.origin[a] = D->origin[a]; S.hub_b[a] = D->hub_b[a]; }
+    S.eps = D->eps; S.musta_cfl = D->musta_cfl; S.musta_stages = D->musta_stages; S.t = D->t; S.limiter = D->limiter; S.eos = D->eos;
+    S.hub_t0 = D->hub_t0; S.hub_e0 = D->hub_e0; S.hub_n0 = D->hub_n0;
+    const size_t N = (size_t)NF * c->nx * c->ny * c->nz;
+    std::vector<long double> in(N), out(N);
+    for (size_t i = 0; i < N; ++i) in[i] = (long double)cons[i];
+    S.eval_L_interior(in.data(), t_stage, out.data());
+    for (size_t i = 0; i < N; ++i) L_out[i] = (double)out[i];
+    return OK;
+}
+
 // ---- pointwise pieces exported for the pins (fp64) -------------------------------------------
 // prim_out = e, p, n, vx, vy, vz.  Returns 1 if the Q16 clamp fired.
 int oracle_con2prim(const double u[5], double prim_out[6]) {

@@ -47,6 +47,7 @@ def lib():
         L.oracle_max_signal_speed.argtypes = [vp, pd]
         L.oracle_get_time.argtypes = [vp, pd]
         L.oracle_eval_L.argtypes = [vp, vp, dbl, vp]
+        L.oracle_eval_L_extended.argtypes = [vp, vp, dbl, vp]
         L.oracle_con2prim.argtypes = [pd, pd]
         L.oracle_signal_speed.argtypes = [pd, i32]
         L.oracle_signal_speed.restype = dbl
@@ -199,6 +200,16 @@ class Oracle:
         assert a.shape == self.shape
         out = np.empty(self.shape, dtype=self.dtype)
         lib().oracle_eval_L(self._h, a.ctypes.data, float(t_stage), out.ctypes.data)
+        return out
+
+    def eval_L_extended(self, cons, t_stage=0.0):
+        """L(u) by the same code in long double, rounded to double (a referee for the fp64 oracle's own rounding)."""
+        assert self.dtype == np.float64
+        a = np.ascontiguousarray(cons, dtype=np.float64)
+        assert a.shape == self.shape
+        out = np.empty(self.shape, dtype=np.float64)
+        rc = lib().oracle_eval_L_extended(self._h, a.ctypes.data, float(t_stage), out.ctypes.data)
+        assert rc == 0
         return out
 
     def close(self):

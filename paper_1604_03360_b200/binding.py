@@ -23,9 +23,10 @@ LIB_PATH = os.path.join(_HERE, "libhydro_b200.so")
 SYMBOLS = [
     "hydro_create", "hydro_set_option", "hydro_set_stream", "hydro_workspace_bytes", "hydro_bind_workspace",
     "hydro_set_state", "hydro_get_state", "hydro_set_state_host", "hydro_get_state_host", "hydro_step",
-    "hydro_step_cfl", "hydro_max_signal_speed", "hydro_eval_L", "hydro_get_time", "hydro_status",
+    "hydro_step_cfl", "hydro_step_cfl_batch", "hydro_max_signal_speed", "hydro_eval_L", "hydro_get_time", "hydro_status",
     "hydro_launch_count", "hydro_stage_kernel_time", "hydro_last_error",
-    "hydro_zhalo_elems", "hydro_get_zhalo", "hydro_put_zhalo", "hydro_step_stage", "hydro_destroy", "hydro_probe_fma_peak",
+    "hydro_zhalo_elems", "hydro_get_zhalo", "hydro_put_zhalo", "hydro_step_stage", "hydro_local_max_speed",
+    "hydro_step_stage_cfl", "hydro_destroy",
 ]
 
 
@@ -54,6 +55,7 @@ def _load():
     L.hydro_get_state_host.argtypes = [vp, vp]
     L.hydro_step.argtypes = [vp, dbl, i32]
     L.hydro_step_cfl.argtypes = [vp, dbl, i32]
+    L.hydro_step_cfl_batch.argtypes = [ctypes.POINTER(vp), i32, dbl, i32]
     L.hydro_max_signal_speed.argtypes = [vp, pd]
     L.hydro_eval_L.argtypes = [vp, vp, dbl, vp]
     L.hydro_get_time.argtypes = [vp, pd]
@@ -66,24 +68,16 @@ def _load():
     L.hydro_get_zhalo.argtypes = [vp, i32, i32, vp]
     L.hydro_put_zhalo.argtypes = [vp, i32, i32, vp]
     L.hydro_step_stage.argtypes = [vp, dbl, i32]
+    L.hydro_local_max_speed.argtypes = [vp, vp]
+    L.hydro_step_stage_cfl.argtypes = [vp, dbl, i32, vp]
     L.hydro_last_error.argtypes = [vp]
     L.hydro_last_error.restype = ctypes.c_char_p
     L.hydro_destroy.argtypes = [vp]
     L.hydro_destroy.restype = None
-    L.hydro_probe_fma_peak.argtypes = [i32, i32, vp, pd]
     return L
 
 
 lib = _load()
-
-
-def probe_fma_peak(precision=F64, millis=200):
-    """Sustained FMA rate in TFLOP/s (hydro_probe_fma_peak)."""
-    out = ctypes.c_double()
-    rc = lib.hydro_probe_fma_peak(precision, millis, torch.cuda.current_stream().cuda_stream, ctypes.byref(out))
-    if rc != OK:
-        raise HydroError(rc, "hydro_probe_fma_peak")
-    return out.value
 
 
 class Hydro:
@@ -191,8 +185,24 @@ class Hydro:
         return out
 
     def put_zhalo(self, buffer, side, packed):
+        """packed = None: zero-gradient ghosts from the slab's own boundary plane (a physical outflow end)."""
+        if packed is None:
+            self._check(lib.hydro_put_zhalo(self._h, int(buffer), int(side), None))
+            return
         assert packed.is_cuda and packed.is_contiguous() and packed.dtype == self.dtype and packed.numel() == self.zhalo_elems()
         self._check(lib.hydro_put_zhalo(self._h, int(buffer), int(side), packed.data_ptr()))
+
+    def local_max_speed(self, out=None):
+        """Max signal speed of this context's state as a 1-element float64 DEVICE tensor (no host sync)."""
+        if out is None:
+            out = torch.empty(1, dtype=torch.float64, device=self.device)
+        assert out.is_cuda and out.dtype == torch.float64 and out.numel() == 1
+        self._check(lib.hydro_local_max_speed(self._h, out.data_ptr()))
+        return out
+
+    def step_stage_cfl(self, cfl, stage, maxspeed):
+        assert maxspeed.is_cuda and maxspeed.dtype == torch.float64 and maxspeed.numel() == 1
+        self._check(lib.hydro_step_stage_cfl(self._h, float(cfl), int(stage), maxspeed.data_ptr()))
 
     def step_stage(self, dt, stage):
         self._check(lib.hydro_step_stage(self._h, float(dt), int(stage)))
@@ -214,6 +224,18 @@ class Hydro:
             self.close()
         except Exception:
             pass
+
+
+def step_cfl_batch(hydros, cfl, nsteps=1):
+    """hydro_step_cfl_batch: advance independent contexts (each bound to its own stream) round-robin."""
+    arr = (ctypes.c_void_p * len(hydros))(*[h._h for h in hydros])
+    rc = lib.hydro_step_cfl_batch(arr, len(hydros), float(cfl), int(nsteps))
+    if rc != OK:
+        for h in hydros:
+            msg = lib.hydro_last_error(h._h).decode()
+            if msg:
+                raise HydroError(rc, msg)
+        raise HydroError(rc, "hydro_step_cfl_batch")
 
 
 def from_workload(w, precision=F64, kernel=KERNEL_AUTO, device="cuda"):

@@ -13,6 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhydro_b200.so")
+PROBE_LIB = os.path.join(HERE, "libbench_probe.so")   # bench.py's FMA-rate probe: a measurement helper, not the product
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-diag-suppress", "221", "-shared", "-Xcompiler", "-fPIC"]
@@ -37,6 +38,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
               [os.path.join(CSRC, "hydro.cu"), "-o", tmp, "-lcuda"]
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)
+    psrc = os.path.join(CSRC, "bench_probe.cu")
+    if force or not os.path.exists(PROBE_LIB) or os.path.getmtime(psrc) > os.path.getmtime(PROBE_LIB):
+        tmp = PROBE_LIB + ".tmp%d" % os.getpid()
+        subprocess.check_call([NVCC] + FLAGS + [psrc, "-o", tmp])
+        os.replace(tmp, PROBE_LIB)
     return LIB
 
 

@@ -1,7 +1,10 @@
-// probe.cuh -- machine probe behind hydro_probe_fma_peak: a register-resident chain of independent fused
-// multiply-adds on every SM.  Its sustained rate is the measured "alu" roofline denominator that bench.py
-// reports next to the nominal 148 SM x 64 (fp64) or 128 (fp32) lanes x 2 flop x 1.965 GHz.
-#pragma once
+// bench_probe.cu -- measurement helper of bench.py, NOT part of the product library or its ABI (include/hydro.h): a
+// register-resident chain of independent fused multiply-adds on every SM.  Its sustained rate is the measured "alu"
+// roofline denominator that bench.py reports next to the nominal 148 SM x 64 (fp64) or 128 (fp32) lanes x 2 flop x
+// 1.965 GHz.  Built by paper_1604_03360_b200/build.py into libbench_probe.so and loaded by bench.py with ctypes:
+//   int bench_probe_fma_peak(int precision /* 0 f64, 1 f32 */, int millis, void* cuda_stream,
+//                            void* device_scratch /* >= 8 bytes, caller-owned */, double* tflops_host);
+// returns 0, or -1 (bad argument) / -3 (CUDA error).
 #include <cuda_runtime.h>
 
 namespace hydro {
@@ -25,12 +28,11 @@ __global__ void __launch_bounds__(256) fma_chain_kernel(T* sink, int iters, T a,
 }
 
 template <class T>
-int probe_impl(int millis, cudaStream_t st, double* out) {
+int probe_impl(int millis, cudaStream_t st, void* scratch, double* out) {
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return -3;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -3;
-    T* sink = nullptr;
-    if (cudaMalloc(&sink, sizeof(T)) != cudaSuccess) return -3;
+    T* sink = (T*)scratch;
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
@@ -41,7 +43,7 @@ int probe_impl(int millis, cudaStream_t st, double* out) {
         cudaEventRecord(e0, st);
         fma_chain_kernel<T><<<blocks, threads, 0, st>>>(sink, iters, (T)0.999999, (T)1e-6);
         cudaEventRecord(e1, st);
-        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(sink); return -3; }
+        if (cudaEventSynchronize(e1) != cudaSuccess) return -3;
         float ms = 0;
         cudaEventElapsedTime(&ms, e0, e1);
         const double flops = 2.0 * 8 * 16 * (double)iters * blocks * threads;
@@ -57,16 +59,15 @@ int probe_impl(int millis, cudaStream_t st, double* out) {
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    cudaFree(sink);
     *out = best;
     return 0;
 }
 
 }  // namespace hydro
 
-extern "C" int hydro_probe_fma_peak(int precision, int millis, void* cuda_stream, double* tflops_host) {
-    if (!tflops_host || millis < 1 || (precision != 0 && precision != 1)) return HYDRO_EINVAL;
-    const int rc = precision == 0 ? hydro::probe_impl<double>(millis, (cudaStream_t)cuda_stream, tflops_host)
-                                  : hydro::probe_impl<float>(millis, (cudaStream_t)cuda_stream, tflops_host);
-    return rc == 0 ? HYDRO_OK : HYDRO_ECUDA;
+extern "C" int bench_probe_fma_peak(int precision, int millis, void* cuda_stream, void* device_scratch,
+                                    double* tflops_host) {
+    if (!tflops_host || !device_scratch || millis < 1 || (precision != 0 && precision != 1)) return -1;
+    return precision == 0 ? hydro::probe_impl<double>(millis, (cudaStream_t)cuda_stream, device_scratch, tflops_host)
+                          : hydro::probe_impl<float>(millis, (cudaStream_t)cuda_stream, device_scratch, tflops_host);
 }

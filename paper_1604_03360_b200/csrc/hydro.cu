@@ -54,6 +54,16 @@ struct hydro_ctx {
     // "profile" option: CUDA events around every stage-kernel launch (bench.py roofline)
     int profile = 0;
     std::vector<cudaEvent_t> ev;  // pairs (start, stop), recorded on the stream
+    // "graph" option: one steady-state step of hydro_step_cfl captured as a CUDA graph and replayed (N4).  A step
+    // flips the primitive buffers once (three stages), so there is one graph per (cfl, buffer parity).
+    struct StepGraph {
+        cudaGraphExec_t exec;
+        double cfl;
+        int wcur_before, wcur_after;
+        long long launches;
+    };
+    int use_graph = 0;
+    std::vector<StepGraph> graphs;
     std::string err;
 };
 
@@ -269,7 +279,7 @@ int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double 
 // the new state.  con2prim (WENO) or the max-speed pass (MUSTA-FORCE, CFL mode) therefore run as separate kernels
 // only for the first step after hydro_set_state / hydro_eval_L; the ghost cells' primitives come from the halo kernel.
 template <class T>
-int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl) {
+int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl, const double* ext_max = nullptr) {
     T* U[3] = {(T*)c->U[0], (T*)c->U[1], (T*)c->U[2]};
     const bool weno = c->scheme != HYDRO_MUSTA_FORCE;
     const bool cflmode = !(dt_fixed > 0.0);
@@ -282,7 +292,7 @@ int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl) {
     int rc;
     const bool have_w = c->w_ready;   // interior primitives of in[s] already in Wb[wcur] (previous stage's epilogue)
     if ((rc = do_halo<T>(c, in[s], tfrac[s], false, 0.0, (weno && have_w) ? (T*)c->Wb[c->wcur] : nullptr))) return rc;
-    const bool need_max = s == 0 && cflmode && !c->max_ready;
+    const bool need_max = s == 0 && cflmode && !c->max_ready && ext_max == nullptr;
     if (need_max) {   // the reduction accumulates with atomicMax: start from zero
         reset_max_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
         LAUNCHED(c, "reset_max_kernel");
@@ -293,7 +303,8 @@ int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl) {
         if ((rc = do_max_speed<T>(c, in[s]))) return rc;
     }
     if (s == 0) {
-        begin_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl, dt_fixed, cfl, c->dx);
+        if (ext_max != nullptr && cflmode) begin_step_ext_kernel<<<1, 1, 0, c->stream>>>(c->ctl, cfl, c->dx, ext_max);
+        else begin_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl, dt_fixed, cfl, c->dx);
         LAUNCHED(c, "begin_step_kernel");
         c->max_ready = false;
     }
@@ -319,8 +330,67 @@ int do_step(hydro_ctx* c, double dt_fixed, double cfl) {
     return HYDRO_OK;
 }
 
+void drop_graphs(hydro_ctx* c) {
+    for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
+    c->graphs.clear();
+}
+
+// A CFL step in the steady state (marching kernels, primitives and max signal speed left by the previous step's
+// epilogues) is a fixed sequence of launches whose only step-dependent inputs live in the device control block:
+// it can be replayed from a graph.
+bool graph_ready(const hydro_ctx* c) {
+    return c->use_graph && !c->profile && c->stream != nullptr && want_fused(c) && c->max_ready &&
+           (c->scheme == HYDRO_MUSTA_FORCE || c->w_ready);
+}
+
+template <class T>
+int graph_step(hydro_ctx* c, double cfl) {
+    for (const auto& g : c->graphs)
+        if (g.cfl == cfl && g.wcur_before == c->wcur) {
+            CUDA_OK(c, cudaGraphLaunch(g.exec, c->stream));
+            c->wcur = g.wcur_after;
+            c->launches += g.launches;
+            return HYDRO_OK;
+        }
+    // capture: nothing executes, the host-side bookkeeping of do_step is rolled back afterwards
+    const int wcur0 = c->wcur;
+    const long long l0 = c->launches;
+    if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        c->use_graph = 0;   // e.g. the legacy default stream: fall back to plain launches for good
+        return do_step<T>(c, -1.0, cfl);
+    }
+    const int rc = do_step<T>(c, -1.0, cfl);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    hydro_ctx::StepGraph g;
+    g.cfl = cfl;
+    g.wcur_before = wcur0;
+    g.wcur_after = c->wcur;
+    g.launches = c->launches - l0;
+    c->wcur = wcur0;
+    c->launches = l0;
+    if (rc != HYDRO_OK || e != cudaSuccess || graph == nullptr) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        c->use_graph = 0;
+        return rc != HYDRO_OK ? rc : do_step<T>(c, -1.0, cfl);
+    }
+    const cudaError_t ei = cudaGraphInstantiate(&g.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ei != cudaSuccess) {
+        cudaGetLastError();
+        c->use_graph = 0;
+        return do_step<T>(c, -1.0, cfl);
+    }
+    c->graphs.push_back(g);
+    return graph_step<T>(c, cfl);
+}
+
 // z-halo planes of one state buffer <-> a packed device buffer [5][g][ny][nx] (slab decomposition, DESIGN 9).
 // get: the g outermost INTERIOR planes of the side; put: the g GHOST planes of the side.
+// put == 2: zero-gradient ghosts (reading Q9) made here from the slab's own boundary plane, for a slab at a physical
+// outflow end of the z axis.
 template <class T>
 __global__ void zhalo_kernel(Geom G, T* pad, T* packed, int side, int put) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -330,6 +400,12 @@ __global__ void zhalo_kernel(Geom G, T* pad, T* packed, int side, int put) {
     const int g = G.g[2];
     const int k = put ? (side == 0 ? l - g : G.n[2] + l) : (side == 0 ? l : G.n[2] - g + l);
     const long long p = G.pidx(i, j, k);
+    if (put == 2) {
+        const long long ps = G.pidx(i, j, side == 0 ? 0 : G.n[2] - 1);
+#pragma unroll
+        for (int c = 0; c < NF; ++c) pad[c * G.fs + p] = pad[c * G.fs + ps];
+        return;
+    }
     const long long plane = (long long)G.n[0] * G.n[1];
     const long long q = ((long long)l * G.n[1] + j) * G.n[0] + i;
 #pragma unroll
@@ -382,6 +458,7 @@ int hydro_create(hydro_ctx** out, int nx, int ny, int nz, double dx, int scheme)
 void hydro_destroy(hydro_ctx* c) {
     if (!c) return;
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    drop_graphs(c);
     delete c;
 }
 
@@ -391,6 +468,7 @@ long long hydro_launch_count(const hydro_ctx* c) { return c ? c->launches : 0; }
 
 int hydro_set_stream(hydro_ctx* c, void* s) {
     if (!c) return HYDRO_EINVAL;
+    drop_graphs(c);
     c->stream = (cudaStream_t)s;
     return HYDRO_OK;
 }
@@ -398,7 +476,10 @@ int hydro_set_stream(hydro_ctx* c, void* s) {
 int hydro_set_option(hydro_ctx* c, const char* key, double v) {
     if (!c || !key) return HYDRO_EINVAL;
     const std::string k(key);
-    if (k == "precision") {
+    drop_graphs(c);   // a captured step has the options baked into its kernel arguments
+    if (k == "graph") {
+        c->use_graph = v != 0.0;
+    } else if (k == "precision") {
         const int p = (int)v;
         if (p != HYDRO_F64 && p != HYDRO_F32) return fail(c, HYDRO_EINVAL, "precision must be 0 or 1");
         if (c->ws && p != c->precision) return fail(c, HYDRO_EINVAL, "precision must be set before the workspace is bound");
@@ -486,6 +567,7 @@ int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
     c->wcur = 0;
     c->w_ready = c->max_ready = false;
     c->stage_open = 0;
+    drop_graphs(c);
     CUDA_OK(c, cudaMemsetAsync(p, 0, hydro_workspace_bytes(c), c->stream));
     set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, c->t_host, 1, 1);
     LAUNCHED(c, "set_ctl_kernel");
@@ -576,9 +658,23 @@ int hydro_step_cfl(hydro_ctx* c, double cfl, int nsteps) {
     if (!(cfl > 0) || nsteps < 0) return fail(c, HYDRO_EINVAL, "hydro_step_cfl: cfl <= 0 or nsteps < 0");
     if (c->stage_open) return fail(c, HYDRO_EINVAL, "hydro_step_cfl inside a hydro_step_stage sequence");
     for (int s = 0; s < nsteps; ++s) {
-        rc = c->precision == HYDRO_F64 ? do_step<double>(c, -1.0, cfl) : do_step<float>(c, -1.0, cfl);
+        if (graph_ready(c)) rc = c->precision == HYDRO_F64 ? graph_step<double>(c, cfl) : graph_step<float>(c, cfl);
+        else rc = c->precision == HYDRO_F64 ? do_step<double>(c, -1.0, cfl) : do_step<float>(c, -1.0, cfl);
         if (rc) return rc;
     }
+    return HYDRO_OK;
+}
+
+int hydro_step_cfl_batch(hydro_ctx** ctxs, int nctx, double cfl, int nsteps) {
+    if (!ctxs || nctx < 0) return HYDRO_EINVAL;
+    for (int i = 0; i < nctx; ++i)
+        if (!ctxs[i]) return HYDRO_EINVAL;
+    // step by step over the batch, so that the launches of the contexts interleave on their streams
+    for (int s = 0; s < nsteps; ++s)
+        for (int i = 0; i < nctx; ++i) {
+            const int rc = hydro_step_cfl(ctxs[i], cfl, 1);
+            if (rc) return rc;
+        }
     return HYDRO_OK;
 }
 
@@ -629,7 +725,8 @@ static int zhalo_impl(hydro_ctx* c, int buffer, int side, void* packed, int put)
     int rc = need_ws(c);
     if (rc) return rc;
     DeviceGuard dg(c);
-    if (!packed || buffer < 0 || buffer > 2 || (side != 0 && side != 1)) return fail(c, HYDRO_EINVAL, "zhalo: bad argument");
+    if ((!packed && put != 2) || buffer < 0 || buffer > 2 || (side != 0 && side != 1))
+        return fail(c, HYDRO_EINVAL, "zhalo: bad argument");
     if (c->G.g[2] == 0) return fail(c, HYDRO_EINVAL, "zhalo: the z axis is inactive");
     const dim3 b = blk2d(64, 4);
     const dim3 g((c->G.n[0] + b.x - 1) / b.x, (c->G.n[1] + b.y - 1) / b.y, c->G.g[2]);
@@ -640,7 +737,7 @@ static int zhalo_impl(hydro_ctx* c, int buffer, int side, void* packed, int put)
 }
 int hydro_get_zhalo(hydro_ctx* c, int buffer, int side, void* packed_out) { return zhalo_impl(c, buffer, side, packed_out, 0); }
 int hydro_put_zhalo(hydro_ctx* c, int buffer, int side, const void* packed_in) {
-    return zhalo_impl(c, buffer, side, const_cast<void*>(packed_in), 1);
+    return zhalo_impl(c, buffer, side, const_cast<void*>(packed_in), packed_in ? 1 : 2);
 }
 
 int hydro_step_stage(hydro_ctx* c, double dt, int stage) {
@@ -650,6 +747,36 @@ int hydro_step_stage(hydro_ctx* c, double dt, int stage) {
     if (!(dt > 0) || stage < 0 || stage > 2) return fail(c, HYDRO_EINVAL, "hydro_step_stage: dt <= 0 or stage not in 0..2");
     if (stage != c->stage_open) return fail(c, HYDRO_EINVAL, "hydro_step_stage: stage %d out of order (expected %d)", stage, c->stage_open);
     return c->precision == HYDRO_F64 ? do_step_stage<double>(c, stage, dt, 0.0) : do_step_stage<float>(c, stage, dt, 0.0);
+}
+
+int hydro_step_stage_cfl(hydro_ctx* c, double cfl, int stage, const void* maxspeed_dev) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    DeviceGuard dg(c);
+    if (!(cfl > 0) || stage < 0 || stage > 2 || !maxspeed_dev)
+        return fail(c, HYDRO_EINVAL, "hydro_step_stage_cfl: cfl <= 0, stage not in 0..2 or null pointer");
+    if (stage != c->stage_open) return fail(c, HYDRO_EINVAL, "hydro_step_stage_cfl: stage %d out of order (expected %d)", stage, c->stage_open);
+    const double* m = (const double*)maxspeed_dev;
+    return c->precision == HYDRO_F64 ? do_step_stage<double>(c, stage, -1.0, cfl, m) : do_step_stage<float>(c, stage, -1.0, cfl, m);
+}
+
+int hydro_local_max_speed(hydro_ctx* c, void* maxspeed_dev_out) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    DeviceGuard dg(c);
+    if (!maxspeed_dev_out) return HYDRO_EINVAL;
+    if (c->stage_open) return fail(c, HYDRO_EINVAL, "hydro_local_max_speed inside a hydro_step_stage sequence");
+    if (!c->max_ready) {
+        reset_max_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
+        LAUNCHED(c, "reset_max_kernel");
+        rc = c->precision == HYDRO_F64 ? do_max_speed<double>(c, (const double*)c->U[0])
+                                       : do_max_speed<float>(c, (const float*)c->U[0]);
+        if (rc) return rc;
+        c->max_ready = true;
+    }
+    // the control block keeps the max as the bit pattern of a non-negative double: the 8 bytes ARE the double
+    CUDA_OK(c, cudaMemcpyAsync(maxspeed_dev_out, &c->ctl->maxspeed_bits, sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    return HYDRO_OK;
 }
 
 int hydro_stage_kernel_time(hydro_ctx* c, double* ms_total_host, long long* launches_host) {
@@ -693,5 +820,3 @@ int hydro_status(hydro_ctx* c) {
 }
 
 }  // extern "C"
-
-#include "probe.cuh"

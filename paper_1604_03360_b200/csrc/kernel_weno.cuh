@@ -33,6 +33,9 @@
 
 namespace hydro {
 
+#ifndef WENO5_MINB
+#define WENO5_MINB 3
+#endif
 constexpr int WENO_ZC = 64, WENO_YC = 128;   // default cells per chunk of the z / y march ("tile_zc" / "sweep_zc")
 constexpr int WENO_DEPTH = 3;                // cells in flight per thread
 constexpr int WENO_ROWS = 4;                 // warps per block
@@ -119,7 +122,7 @@ struct WenoXZShape {
 };
 
 template <class T, int R>
-__global__ void __launch_bounds__(WENO_THREADS, (R == 4 && sizeof(T) == 8) ? 2 : 3)
+__global__ void __launch_bounds__(WENO_THREADS, (R == 4 && sizeof(T) == 8) ? 2 : WENO5_MINB)
 weno_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, const T* Un, T* Uout, Ctl* ctl,
                int zc) {
     using S = WenoXZShape<T, R>;
@@ -255,7 +258,7 @@ constexpr size_t weno_y_smem_bytes() {
 }
 
 template <class T, int R, bool EPI>
-__global__ void __launch_bounds__(WENO_THREADS, (R == 4 && sizeof(T) == 8) ? 2 : 3)
+__global__ void __launch_bounds__(WENO_THREADS, (R == 4 && sizeof(T) == 8) ? 2 : WENO5_MINB)
 weno_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* __restrict__ W, T* Uout, T* Wnext, Ctl* ctl,
               int yc) {
     using Win = WenoWindow<T, R, 1>;

@@ -23,6 +23,11 @@ __global__ void begin_step_kernel(Ctl* ctl, double dt_fixed, double cfl, double 
         ctl->dt = cfl * dx / s;
     }
 }
+// the same with the max signal speed taken from a caller's device scalar (a double): the slab decomposition passes
+// the value it has max-reduced over all slabs (reading Q10 on the global grid)
+__global__ void begin_step_ext_kernel(Ctl* ctl, double cfl, double dx, const double* __restrict__ maxspeed) {
+    ctl->dt = cfl * dx / *maxspeed;
+}
 __global__ void end_step_kernel(Ctl* ctl) {
     ctl->t += ctl->dt;
     // the stage-3 epilogue of the z sweep (when it ran) left the max signal speed of the new state here

@@ -1,8 +1,9 @@
 """Slab decomposition along z: one exchange of g ghost planes per
 Runge-Kutta stage with the two z-neighbours and one max-reduction of the signal speed per step.
 
-Every step of the hot path runs in the library's kernels (hydro_get_zhalo / hydro_put_zhalo / hydro_step_stage);
-this module only moves the packed halo buffers between slabs:
+Every step of the hot path runs in the library's kernels (hydro_get_zhalo / hydro_put_zhalo / hydro_local_max_speed /
+hydro_step_stage_cfl); this module only routes device buffers between slabs -- the packed halo planes and the one
+double of the signal-speed reduction -- and never brings a value to the host:
 
   * ``DistComm``   one slab per process, neighbours reached with torch.distributed point-to-point calls (NCCL on
                    GPUs; the same code runs over gloo on CPU tensors, which is how it is tested without GPUs);
@@ -10,8 +11,8 @@ this module only moves the packed halo buffers between slabs:
                    guide asks for when there are fewer GPUs than ranks.  It is the parity test of the decomposition:
                    the result must be bit-identical to the undecomposed run.
 
-The physical boundary rule of the z axis (periodic or outflow) is applied here, on the packed buffers: a slab
-always runs with bc_z = BC_EXTERNAL.
+A slab always runs with bc_z = BC_EXTERNAL; the periodic rule of the z axis is the ring closing, the outflow rule is
+the library's (hydro_put_zhalo with no buffer: zero-gradient copies of the slab's own boundary plane).
 """
 from __future__ import annotations
 
@@ -36,14 +37,6 @@ def neighbours(rank, world, bc_z):
     lo = rank - 1 if rank > 0 else (world - 1 if bc_z == BC_PERIODIC else None)
     hi = rank + 1 if rank < world - 1 else (0 if bc_z == BC_PERIODIC else None)
     return lo, hi
-
-
-def outflow_ghost(own_planes, g, side):
-    """Zero-gradient ghost planes from a slab's own packed boundary planes [5][g][ny][nx] (reading Q9): every
-    ghost layer repeats the nearest interior plane (the lowest one for side 0, the highest for side 1)."""
-    v = own_planes.view(5, g, -1)
-    src = v[:, 0:1] if side == 0 else v[:, g - 1:g]
-    return src.expand(5, g, v.shape[2]).contiguous().view(-1)
 
 
 class DistComm:
@@ -79,12 +72,12 @@ class DistComm:
         return [(recv_lo, recv_hi)]
 
     def max(self, values):
-        t = torch.tensor([max(values)], dtype=torch.float64)
+        """values = [one 1-element float64 tensor] (this rank's slab): all-reduced in place with MAX over the ranks,
+        on the tensor's device (NCCL on the GPU, gloo on the CPU); nothing comes to the host."""
+        (t,) = values
         if self.world > 1:
-            dev = "cuda" if self.dist.get_backend() == "nccl" else "cpu"
-            t = t.to(dev)
             self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
-        return float(t.item())
+        return t
 
 
 class LocalComm:
@@ -101,7 +94,11 @@ class LocalComm:
         return out
 
     def max(self, values):
-        return max(values)
+        """Element-wise maximum of the slabs' 1-element tensors (what the all-reduce does between ranks)."""
+        t = values[0]
+        for v in values[1:]:
+            t = torch.maximum(t, v)
+        return t
 
 
 class SlabGroup:
@@ -113,26 +110,21 @@ class SlabGroup:
             assert x.zhalo_elems() > 0
 
     def _fill_z_ghosts(self, buffer):
-        g_elems = [x.zhalo_elems() for x in self.h]
         pairs = [(x.get_zhalo(buffer, 0), x.get_zhalo(buffer, 1)) for x in self.h]
         got = self.comm.exchange(pairs)
-        for x, (own_lo, own_hi), (below, above), ne in zip(self.h, pairs, got, g_elems):
-            g = ne // (5 * x.shape[2] * x.shape[3])
-            x.put_zhalo(buffer, 0, below if below is not None else outflow_ghost(own_lo, g, 0))
-            x.put_zhalo(buffer, 1, above if above is not None else outflow_ghost(own_hi, g, 1))
+        for x, (below, above) in zip(self.h, got):
+            x.put_zhalo(buffer, 0, below)      # None at a physical end: the library's zero-gradient rule
+            x.put_zhalo(buffer, 1, above)
 
     def step_cfl(self, cfl, nsteps=1):
-        """dt = cfl dx / (max signal speed over ALL slabs), then three stages, each after a halo exchange."""
-        dts = []
+        """Per step: the slabs' max signal speeds are max-reduced on the device, then three stages, each after a
+        halo exchange; dt = cfl dx / max is taken inside the library (hydro_step_stage_cfl).  No host sync."""
         for _ in range(nsteps):
-            a = self.comm.max([x.max_signal_speed() for x in self.h])
-            dt = cfl * self.dx / a
+            a = self.comm.max([x.local_max_speed() for x in self.h])
             for s in range(3):
                 self._fill_z_ghosts(s)
                 for x in self.h:
-                    x.step_stage(dt, s)
-            dts.append(dt)
-        return dts
+                    x.step_stage_cfl(cfl, s, a)
 
 
 def make_slab(binding, w, k0, k1, precision=0, device="cuda"):

@@ -207,19 +207,24 @@ def _sum_separable(w, gx, gy, gz):
 
 
 def lumpy(n=256, hotspots=40, with_velocity=False, scheme=MUSTA_FORCE, nsteps=50, cfl=0.2,
-          box=16.0, seed=SEED, sigma_unit=None):
+          box=16.0, seed=SEED, sigma_unit=None, crop=None):
     """Configs 4 (40 hotspots, v=0) and 5 (200 hotspots, per-hotspot velocities, Q15).
 
     Draw order: all centres, all widths, all amplitudes, then (config 5) speeds and
     directions from normalised Gaussians.  e = 0.1 + sum_k A_k g_k, n = 0.2 e^(3/4),
     v = sum_k A_k g_k v_k / (0.1 + sum_k A_k g_k).  Small parity cases pass a smaller ``box`` and a
     ``sigma_unit`` so that the hotspots span a similar number of cells as at full size.
+    ``crop`` = m evaluates only the corner block of the first m cells per axis of the n^3 state (same draws, same
+    formulas: the corner crop of the full state up to the summation order of the matrix product), for the CPU
+    baseline's bounded sample; the result is a Workload on an m^3 grid.
     """
     rng = np.random.default_rng(seed)
     centres = rng.uniform(0.0, box, size=(hotspots, 3))
     sigma = rng.uniform(0.3, 0.8, size=hotspots) * (box / 16.0 if sigma_unit is None else sigma_unit)
     amp = np.exp(0.5 * rng.standard_normal(hotspots))
     gx, gy, gz = _hotspot_profiles(n, box, centres, sigma)
+    if crop is not None:
+        gx, gy, gz = gx[:, :crop], gy[:, :crop], gz[:, :crop]
     bump = _sum_separable(amp, gx, gy, gz)
     e = 0.1 + bump
     nn = 0.2 * e ** 0.75
@@ -234,6 +239,9 @@ def lumpy(n=256, hotspots=40, with_velocity=False, scheme=MUSTA_FORCE, nsteps=50
     cons = prim_to_cons(e, nn, v[0], v[1], v[2])
     dx = box / n
     name = "lumpy_v" if with_velocity else "lumpy"
+    if crop is not None:
+        return Workload("%s_crop%d" % (name, crop), (crop, crop, crop), dx, (0.0, 0.0, 0.0), scheme,
+                        (BC_PERIODIC,) * 3, cons, 0.0, cfl=cfl, nsteps=nsteps)
     return Workload(name, (n, n, n), dx, (0.0, 0.0, 0.0), scheme, (BC_PERIODIC,) * 3, cons, 0.0,
                     cfl=cfl, nsteps=nsteps)
 

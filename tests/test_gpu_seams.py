@@ -1,0 +1,169 @@
+"""Parity of the CUDA path against the CPU oracle where the marching kernels are most fragile (all `-m gpu`):
+the seams between chunks of the z / y march (window re-prime, parked flux, cp.async slot reuse, the half group at the
+end of an odd MUSTA y chunk), the run-time number of MUSTA-FORCE stages, the values the Q16 clamp produces, the
+flag for non-finite states, and the sizes and precisions bench.py times (sampled cells at 512^3).
+
+Tolerances are those of tests/test_gpu_parity.py (BASELINE.json north_star; reading Q12)."""
+import functools
+import math
+
+import numpy as np
+import pytest
+
+from paper_1604_03360_b200 import workloads as W
+from test_gpu_parity import SCHEMES, TOL_STAGE, reldiff, small_workload, to_dev, _crop_periodic
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_1604_03360_b200 import binding
+    return binding
+
+
+# ------------------------------------------------------------------ chunk seams of the marching kernels vs the ORACLE
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("chunks", [(5, 7), (1, 1), (16, 16)])
+def test_chunk_seams_match_the_oracle(B, oracle, scheme, prec, chunks):
+    """70 x 45 x 40 with tile_zc / sweep_zc far below the grid: every chunk boundary of the z and y march falls
+    inside the grid (ragged last chunks, odd chunk lengths).  L(u) and one full step against the oracle."""
+    n = (70, 45, 40)
+    for bc in (W.BC_PERIODIC, W.BC_OUTFLOW):
+        w = small_workload(scheme, n, bc)
+        w.options = {"tile_zc": chunks[0], "sweep_zc": chunks[1]}
+        wo = small_workload(scheme, n, bc)
+        h = B.from_workload(w, precision=prec, kernel=B.KERNEL_FUSED)
+        o = oracle.from_workload(wo)
+        Lo = o.eval_L(wo.cons)
+        Lg = h.eval_L(to_dev(B, w.cons, h.dtype)).cpu().numpy()
+        scale = np.max(np.abs(w.cons[0])) / w.dx
+        # fp32: a few hundred roundings of 6e-8 on differences of O(1) data, relative to E/dx
+        assert reldiff(Lg, Lo, scale=scale) <= (TOL_STAGE if prec == 0 else 2e-5)
+        dt = 0.2 * w.dx / o.max_signal_speed()
+        o.step(dt, 1)
+        h.step(dt, 1)
+        assert reldiff(h.get_state().cpu().numpy(), o.get_state()) <= (3 * TOL_STAGE if prec == 0 else 3e-6)
+        assert h.status() == 0
+        h.close()
+
+
+# ------------------------------------------------------------------ MUSTA-FORCE with K != 2 (N3)
+@pytest.mark.parametrize("K", [1, 3, 4])
+def test_musta_stage_count_matches_the_oracle(B, oracle, K):
+    w = small_workload(W.MUSTA_FORCE, (45, 23, 70))
+    w.options = {"musta_stages": K}
+    o = oracle.from_workload(w)
+    h = B.from_workload(w)
+    Lo = o.eval_L(w.cons)
+    Lg = h.eval_L(to_dev(B, w.cons)).cpu().numpy()
+    assert reldiff(Lg, Lo, scale=np.max(np.abs(w.cons[0])) / w.dx) <= TOL_STAGE
+    # and it is not the K = 2 operator
+    w2 = small_workload(W.MUSTA_FORCE, (45, 23, 70))
+    L2 = oracle.from_workload(w2).eval_L(w2.cons)
+    assert np.max(np.abs(L2 - Lo)) > 1e-4 * np.max(np.abs(Lo))
+    w.nsteps = 10
+    for dt in oracle.run(o, w):
+        h.step(dt, 1)
+    assert reldiff(h.get_state().cpu().numpy(), o.get_state()) <= 1e-10
+    assert h.status() == 0
+    h.close()
+
+
+# ------------------------------------------------------------------ Q16: the values the clamp produces
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_clamped_cell_gives_the_oracles_values(B, oracle, scheme):
+    """One cell with |M| = 1.5 E: both sides scale M back to (1 - 1e-12) E along M and raise the flag.  The clamped
+    cell has 1 - v^2 = 2e-12, so its pressure and signal speeds carry a relative rounding error of about
+    1e-16 / 2e-12 = 5e-5 on quantities that are themselves ~1e-6 of the flux (sqrt(1 - v^2)): L(u) agrees to
+    ~1e-10 in the cells whose stencils contain the clamped cell and to the usual 1e-12 everywhere else."""
+    n = (24, 17, 15)
+    w = small_workload(scheme, n)
+    bad = w.cons.copy()
+    ci, cj, ck = 11, 8, 7
+    m = bad[1:4, ck, cj, ci]
+    bad[1:4, ck, cj, ci] = m / np.linalg.norm(m) * 1.5 * bad[0, ck, cj, ci]
+    wb = W.Workload("clamp", n, w.dx, (0, 0, 0), scheme, (W.BC_PERIODIC,) * 3, bad)
+    o = oracle.from_workload(wb)
+    h = B.from_workload(wb)
+    Lo = o.eval_L(bad)
+    Lg = h.eval_L(to_dev(B, bad)).cpu().numpy()
+    assert h.status() == B.EUNPHYSICAL
+    scale = np.max(np.abs(bad[0])) / w.dx
+    r = {W.WENO5: 3, W.WENO7: 4, W.MUSTA_FORCE: 2}[scheme]
+    near = np.zeros(Lo.shape[1:], dtype=bool)
+    near[ck - r:ck + r + 1, cj, ci] = near[ck, cj - r:cj + r + 1, ci] = near[ck, cj, ci - r:ci + r + 1] = True
+    assert np.all(np.isfinite(Lg))
+    far_err = max(np.max(np.abs((Lg[c] - Lo[c])[~near])) for c in range(5)) / scale
+    near_err = max(np.max(np.abs((Lg[c] - Lo[c])[near])) for c in range(5)) / scale
+    assert far_err <= TOL_STAGE, far_err
+    assert near_err <= 2e-9, near_err
+    # the clamp did act: without it the result would differ by far more than the tolerance
+    assert max(np.max(np.abs(Lo[c][near])) for c in range(5)) / scale > 1e-3
+    h.close()
+
+
+# ------------------------------------------------------------------ non-finite states raise the flag
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("field,value", [(0, float("nan")), (2, float("nan")), (0, float("inf")), (0, -1.0)])
+def test_non_finite_or_negative_energy_raises_the_flag(B, scheme, field, value):
+    w = small_workload(scheme, (40, 33, 24))
+    bad = w.cons.copy()
+    bad[field, 10, 20, 30] = value
+    h = B.from_workload(w)
+    h.step(1e-4, 1)
+    assert h.status() == 0
+    h.set_state(to_dev(B, bad))
+    h.step(1e-4, 1)
+    assert h.status() == B.EUNPHYSICAL, (scheme, field, value)
+    h.close()
+
+
+# ------------------------------------------------------------------ the sizes and precisions bench.py times
+@functools.lru_cache(maxsize=1)
+def _production_512():
+    return W.lumpy(n=512, hotspots=200, with_velocity=True, scheme=W.WENO5, nsteps=1, cfl=0.2)
+
+
+@pytest.mark.parametrize("scheme,prec", [(W.WENO7, 0), (W.MUSTA_FORCE, 0), (W.WENO7, 1), (W.WENO5, 1)])
+def test_bench_variants_at_512_on_sampled_cells(B, oracle, scheme, prec):
+    """BASELINE configs[4] at its full size for the variants of the bench line other than WENO5 fp64 (which
+    tests/test_gpu_parity.py::test_full_size_step_on_sampled_cells covers): one RK3 step, sampled cells recomputed
+    by the oracle from a (6 r + 1)^3 crop, plus conservation over the whole grid."""
+    import torch
+    n = 512
+    w0 = _production_512()
+    w = W.Workload(w0.name, w0.n, w0.dx, w0.origin, scheme, w0.bc, w0.cons, 0.0, cfl=0.2, nsteps=1)
+    h = B.from_workload(w, precision=prec)
+    dt = 0.2 * w.dx / h.max_signal_speed()
+    h.step(dt, 1)
+    assert h.status() == 0
+    ug_t = h.get_state()
+    r = {W.WENO5: 3, W.WENO7: 4, W.MUSTA_FORCE: 2}[scheme]
+    half = 3 * r
+    samples = [(0, 0, 0), (n - 1, n - 1, n - 1), (30, 6, 63), (31, 7, 64), (62, 127, 127), (61, 128, 128),
+               (n // 2, n // 2, n // 2), (n - 1, 0, 128), (333, 222, 111)]
+    worst = 0.0
+    scale = np.max(np.abs(w.cons[0]))
+    fmax = [np.max(np.abs(w.cons[c])) for c in range(5)]
+    for (i, j, k) in samples:
+        crop = _crop_periodic(w.cons, (i, j, k), half)
+        m = 2 * half + 1
+        wc = W.Workload("crop", (m, m, m), w.dx, (0, 0, 0), scheme, (W.BC_PERIODIC,) * 3, crop)
+        o = oracle.from_workload(wc)
+        o.step(dt, 1)
+        ref = o.get_state()[:, half, half, half]
+        got = ug_t[:, k, j, i].double().cpu().numpy()
+        for c in range(5):
+            den = max(abs(ref[c]), 1e-15 * scale) if c == 0 else max(fmax[c], 1e-15 * scale)
+            worst = max(worst, abs(got[c] - ref[c]) / den)
+    assert worst <= (3e-12 if prec == 0 else 1e-5), worst
+    tot1 = [float(torch.sum(ug_t[c].double())) for c in range(5)]
+    tot0 = [float(np.sum(w.cons[c])) for c in range(5)]
+    for a, b in zip(tot0, tot1):
+        assert abs(a - b) <= (1e-11 if prec == 0 else 2e-6) * abs(tot0[0]), (tot0, tot1)
+    del ug_t
+    h.close()

@@ -1,6 +1,7 @@
 """Slab decomposition along z.  CPU: the partition and neighbour logic, and the
 neighbour exchange / max-reduction over a 2-rank gloo group (the same code that runs over NCCL).  GPU (-m gpu):
 several slabs advanced in lockstep in one process must reproduce the undecomposed run BIT FOR BIT."""
+import math
 import os
 import sys
 
@@ -26,16 +27,6 @@ def test_split_and_neighbours():
     assert S.neighbours(0, 1, S.BC_PERIODIC) == (0, 0)
 
 
-def test_outflow_ghost_repeats_the_boundary_plane():
-    g, ny, nx = 3, 2, 4
-    planes = torch.arange(5 * g * ny * nx, dtype=torch.float64)
-    lo = S.outflow_ghost(planes, g, 0).view(5, g, ny * nx)
-    hi = S.outflow_ghost(planes, g, 1).view(5, g, ny * nx)
-    src = planes.view(5, g, ny * nx)
-    for l in range(g):
-        assert torch.equal(lo[:, l], src[:, 0]) and torch.equal(hi[:, l], src[:, g - 1])
-
-
 def test_local_comm_wiring():
     for bc in (S.BC_PERIODIC, S.BC_OUTFLOW):
         c = S.LocalComm(3, bc)
@@ -44,7 +35,7 @@ def test_local_comm_wiring():
         assert got[1] == ("hi0", "lo2")
         assert got[0] == (("hi2" if bc == S.BC_PERIODIC else None), "lo1")
         assert got[2] == ("hi1", ("lo0" if bc == S.BC_PERIODIC else None))
-        assert c.max([0.2, 0.7, 0.5]) == 0.7
+        assert float(c.max([torch.tensor([v], dtype=torch.float64) for v in (0.2, 0.7, 0.5)])) == 0.7
 
 
 def _worker(rank, world, port, bc, out):
@@ -54,7 +45,7 @@ def _worker(rank, world, port, bc, out):
     lo = torch.full((6,), 10.0 * rank + 1.0, dtype=torch.float64)     # "my lowest planes"
     hi = torch.full((6,), 10.0 * rank + 2.0, dtype=torch.float64)     # "my highest planes"
     (below, above), = comm.exchange([(lo, hi)])
-    m = comm.max([0.3 + 0.1 * rank])
+    m = float(comm.max([torch.tensor([0.3 + 0.1 * rank], dtype=torch.float64)]))
     out[rank] = (None if below is None else float(below[0]), None if above is None else float(above[0]), m)
     dist.barrier()
     dist.destroy_process_group()
@@ -74,6 +65,86 @@ def test_dist_comm_over_gloo_two_ranks(bc):
     else:
         assert res[0][0] is None and res[1][1] is None      # physical ends
     assert res[0][2] == res[1][2] == pytest.approx(0.4)
+
+
+# ------------------------------------------------------------------ the whole control flow of SlabGroup.step_cfl off-GPU
+class FakeHydro:
+    """A CPU stand-in with the slab calls of binding.Hydro: one value per z-plane, g = 2 ghost planes, and a "stage"
+    out = in + dt * (in[k-2] - 2 in[k] + in[k+2]) that needs BOTH ghost layers of the buffer it reads.  Stage s reads
+    buffer s and writes buffer (s + 1) % 3, as the library does.  It only exists to drive SlabGroup."""
+    G = 2
+
+    def __init__(self, planes):
+        self.nz = len(planes)
+        self.shape = (5, self.nz, 1, 1)
+        self.buf = [torch.zeros(self.nz + 2 * self.G, dtype=torch.float64) for _ in range(3)]
+        self.buf[0][self.G:-self.G] = torch.as_tensor(planes, dtype=torch.float64)
+        self.calls = []
+
+    def zhalo_elems(self):
+        return self.G
+
+    def get_zhalo(self, buffer, side):
+        v = self.buf[buffer][self.G:-self.G]
+        return (v[:self.G] if side == 0 else v[-self.G:]).clone()
+
+    def put_zhalo(self, buffer, side, packed):
+        b = self.buf[buffer]
+        if packed is None:      # zero-gradient
+            packed = (b[self.G] if side == 0 else b[-self.G - 1]).repeat(self.G)
+        if side == 0:
+            b[:self.G] = packed
+        else:
+            b[-self.G:] = packed
+        self.calls.append(("put", buffer, side))
+
+    def local_max_speed(self):
+        return self.buf[0][self.G:-self.G].abs().max().reshape(1).clone()
+
+    def step_stage_cfl(self, cfl, stage, a):
+        dt = cfl / float(a)
+        u = self.buf[stage]
+        G = self.G
+        self.buf[(stage + 1) % 3][G:-G] = u[G:-G] + dt * (u[:-2 * G] - 2.0 * u[G:-G] + u[2 * G:])
+        self.calls.append(("stage", stage))
+
+    def interior(self):
+        return self.buf[0][self.G:-self.G].clone()
+
+
+def _planes(nz):
+    return [math.sin(0.7 * k) + 0.05 * k for k in range(nz)]
+
+
+def _step_worker(rank, world, port, bc, nz, nsteps, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    k0, k1 = S.split_planes(nz, world)[rank]
+    h = FakeHydro(_planes(nz)[k0:k1])
+    S.SlabGroup([h], S.DistComm(dist, bc), 1.0).step_cfl(0.1, nsteps)
+    out[rank] = (h.interior().tolist(), h.calls[:9])
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("bc", [S.BC_PERIODIC, S.BC_OUTFLOW])
+def test_step_cfl_control_flow_over_gloo_two_ranks(bc):
+    """SlabGroup.step_cfl end to end with two ranks over gloo: the max-reduction of the device scalar, one exchange
+    per stage BEFORE that stage, the ring of two (periodic) or the zero-gradient ends (outflow).  The decomposed run
+    must equal, bit for bit, the same fake advanced as one domain."""
+    nz, nsteps, world = 11, 3, 2
+    one = FakeHydro(_planes(nz))
+    S.SlabGroup([one], S.LocalComm(1, bc), 1.0).step_cfl(0.1, nsteps)
+    port = 33500 + os.getpid() % 2000 + bc
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_step_worker, args=(world, port, bc, nz, nsteps, out), nprocs=world, join=True)
+        res = dict(out)
+    got = res[0][0] + res[1][0]
+    assert got == one.interior().tolist()
+    # per stage: both ghost sides of the stage's input buffer are written, then the stage runs
+    assert res[0][1] == [("put", 0, 0), ("put", 0, 1), ("stage", 0), ("put", 1, 0), ("put", 1, 1), ("stage", 1),
+                         ("put", 2, 0), ("put", 2, 1), ("stage", 2)]
 
 
 # ------------------------------------------------------------------ GPU: bit-identity with the undecomposed run
@@ -101,3 +172,27 @@ def test_slabs_reproduce_the_single_domain_run_bit_for_bit(scheme, bc_z, parts):
     assert torch.equal(got, want)
     for h in hs:
         h.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("scheme,g", [(W.WENO5, 3), (W.MUSTA_FORCE, 2)])
+def test_put_zhalo_without_a_buffer_is_the_outflow_rule(scheme, g):
+    """hydro_put_zhalo(NULL) on a slab with external z ghosts must give exactly what bc_z = outflow gives: the same
+    L(u)-driven step, bit for bit (reading Q9 applied by the library, not by the Python side)."""
+    from paper_1604_03360_b200 import binding as B
+    n = (24, 17, 15)
+    big = W.lumpy(n=max(n), hotspots=12, with_velocity=True, scheme=scheme, box=max(n) / 16.0, sigma_unit=0.12)
+    cons = np.ascontiguousarray(big.cons[:, :n[2], :n[1], :n[0]])
+    w = W.Workload("slab", n, big.dx, (0.0, 0.0, 0.0), scheme, (W.BC_PERIODIC, W.BC_OUTFLOW, W.BC_OUTFLOW), cons, 0.0)
+    ref = B.from_workload(w)
+    ref.step(1e-3, 2)
+    want = ref.get_state().cpu()
+    ref.close()
+    h = S.make_slab(B, w, 0, n[2])
+    for _ in range(2):
+        for s in range(3):
+            h.put_zhalo(s, 0, None)
+            h.put_zhalo(s, 1, None)
+            h.step_stage(1e-3, s)
+    assert torch.equal(h.get_state().cpu(), want)
+    h.close()
