@@ -40,10 +40,11 @@ struct hydro_ctx {
     size_t ws_bytes = 0;
     Ctl* ctl = nullptr;
     char* U[3] = {nullptr, nullptr, nullptr};  // u^n and two stage buffers (padded, 5 fields each)
-    char* Wb[2] = {nullptr, nullptr};           // primitives (padded, 5 arrays), two buffers: the z sweep's epilogue
-                                                // writes the next stage's while this stage's are still read
-    int wcur = 0;                               // buffer holding the primitives of the stage input
-    bool w_ready = false;                       // interior of Wb[wcur] already holds the primitives of u^n
+    char* Wb[2] = {nullptr, nullptr};           // primitives (padded, 7 arrays) for the GENERIC kernel only (grids with an
+                                                // inactive axis, "kernel" = generic): the marching kernels make their
+                                                // primitives on the fly; Wb[1] is unused (= Wb[0])
+    int wcur = 0;
+    bool w_ready = false;                       // (generic path) never true: the primitives are remade every stage
     bool max_ready = false;                     // ctl->maxspeed_bits holds the max signal speed of u^n (stage-3 epilogue)
     int stage_open = 0;                         // stages of a hydro_step_stage sequence done so far (0 = between steps)
     int device = -1;                            // CUDA device of the workspace (captured at bind)
@@ -54,8 +55,8 @@ struct hydro_ctx {
     // "profile" option: CUDA events around every stage-kernel launch (bench.py roofline)
     int profile = 0;
     std::vector<cudaEvent_t> ev;  // pairs (start, stop), recorded on the stream
-    // "graph" option: one steady-state step of hydro_step_cfl captured as a CUDA graph and replayed (N4).  A step
-    // flips the primitive buffers once (three stages), so there is one graph per (cfl, buffer parity).
+    // "graph" option: one steady-state step of hydro_step_cfl captured as a CUDA graph and replayed (N4); one graph
+    // per value of cfl.
     struct StepGraph {
         cudaGraphExec_t exec;
         double cfl;
@@ -100,6 +101,9 @@ void make_geom(hydro_ctx* c) {
 
 size_t state_bytes(const hydro_ctx* c) { return (size_t)NF * (size_t)c->G.fs * esize(c); }
 size_t prim_bytes(const hydro_ctx* c) { return (size_t)NW * (size_t)c->G.fs * esize(c); }
+bool fused_supported(const Geom& G);
+// the primitive arrays exist only where the generic kernel can be asked for
+bool needs_w(const hydro_ctx* c) { return c->kernel == HYDRO_KERNEL_GENERIC || !fused_supported(c->G); }
 
 // Every entry point that touches the device runs on the device of the workspace, whatever device is current in the
 // calling thread; the caller's current device is restored on return.
@@ -205,7 +209,6 @@ bool fused_supported(const Geom& G) { return G.g[0] > 0 && G.g[1] > 0 && G.g[2] 
 
 bool want_fused(const hydro_ctx* c) {
     if (c->kernel == HYDRO_KERNEL_GENERIC) return false;
-    if (c->kernel == HYDRO_KERNEL_AUTO && !c->fused_ready) return false;
     return fused_supported(c->G);
 }
 
@@ -236,23 +239,21 @@ struct StageTimer {
 
 // One stage: Uout = ca u^n + cb (Us + dt L(Us)), or L(Us) itself (mode 1).
 template <class T>
-int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double cb, int mode, T* Wnext = nullptr,
-             int epi_max = 0) {
+int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double cb, int mode, int epi_max = 0) {
     StageArgs A = stage_args(c, ca, cb, mode);
     A.epi_max = epi_max;
     StageTimer timer(c);
     if (want_fused(c)) {
         if (!c->fused_ready) return fail(c, HYDRO_ECUDA, "marching kernels not configured: %s", c->plan_err);
         int nl = 0, rc;
-        const T* W = (const T*)c->Wb[c->wcur];
         if (c->scheme == HYDRO_MUSTA_FORCE)
             rc = launch_musta<T>(c->G, A, Us, Un, Uout, c->ctl, c->zc > 0 ? c->zc : 64, c->yc > 0 ? c->yc : 128,
                                  c->stream, &nl, c->plan_err, sizeof c->plan_err);
         else if (c->scheme == HYDRO_WENO5)
-            rc = launch_weno<T, 3>(c->G, A, Us, W, Un, Uout, Wnext, c->ctl, c->zc > 0 ? c->zc : WENO_ZC,
+            rc = launch_weno<T, 3>(c->G, A, Us, Un, Uout, c->ctl, c->zc > 0 ? c->zc : WENO_ZC,
                                    c->yc > 0 ? c->yc : WENO_YC, c->stream, &nl, c->plan_err, sizeof c->plan_err);
         else
-            rc = launch_weno<T, 4>(c->G, A, Us, W, Un, Uout, Wnext, c->ctl, c->zc > 0 ? c->zc : WENO_ZC,
+            rc = launch_weno<T, 4>(c->G, A, Us, Un, Uout, c->ctl, c->zc > 0 ? c->zc : WENO_ZC,
                                    c->yc > 0 ? c->yc : WENO_YC, c->stream, &nl, c->plan_err, sizeof c->plan_err);
         if (rc != 0) return fail(c, HYDRO_ECUDA, "stage launch: %s", c->plan_err);
         c->launches += nl;
@@ -274,30 +275,27 @@ int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double 
 
 // One SSP-RK3 step (a9, O8):  u1 = u + dt L(u);  u2 = 3/4 u + 1/4 (u1 + dt L(u1));
 // u' = 1/3 u + 2/3 (u2 + dt L(u2)), ghosts at t, t+dt, t+dt/2.  dt_fixed > 0, or CFL mode.
-// With the marching kernels every stage leaves what the next one needs: the WENO x/z kernel's epilogue writes the
-// primitives of its output into the other W buffer, and stage 3 of either scheme reduces the max signal speed of
-// the new state.  con2prim (WENO) or the max-speed pass (MUSTA-FORCE, CFL mode) therefore run as separate kernels
-// only for the first step after hydro_set_state / hydro_eval_L; the ghost cells' primitives come from the halo kernel.
+// The marching kernels make con2prim + signal speeds (a2-a3) of every cell as it enters a stencil window, and stage 3
+// reduces the max signal speed of the new state (a4): the max-speed pass runs as a separate kernel only for the
+// first CFL step after hydro_set_state / hydro_eval_L.  Only the generic kernel reads primitive arrays (prim_kernel).
 template <class T>
 int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl, const double* ext_max = nullptr) {
     T* U[3] = {(T*)c->U[0], (T*)c->U[1], (T*)c->U[2]};
     const bool weno = c->scheme != HYDRO_MUSTA_FORCE;
     const bool cflmode = !(dt_fixed > 0.0);
     const bool marching = want_fused(c);
-    const bool epi = weno && marching;
     const double tfrac[3] = {0.0, 1.0, 0.5};
     const double ca[3] = {0.0, 0.75, 1.0 / 3.0}, cb[3] = {1.0, 0.25, 2.0 / 3.0};
     T* const in[3] = {U[0], U[1], U[2]};
     T* const out[3] = {U[1], U[2], U[0]};   // stage 3 writes u^n in place: each cell reads only its own u^n
     int rc;
-    const bool have_w = c->w_ready;   // interior primitives of in[s] already in Wb[wcur] (previous stage's epilogue)
-    if ((rc = do_halo<T>(c, in[s], tfrac[s], false, 0.0, (weno && have_w) ? (T*)c->Wb[c->wcur] : nullptr))) return rc;
+    if ((rc = do_halo<T>(c, in[s], tfrac[s], false, 0.0))) return rc;
     const bool need_max = s == 0 && cflmode && !c->max_ready && ext_max == nullptr;
     if (need_max) {   // the reduction accumulates with atomicMax: start from zero
         reset_max_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
         LAUNCHED(c, "reset_max_kernel");
     }
-    if (weno && !have_w) {
+    if (weno && !marching) {   // the generic kernel reads its primitives from arrays
         if ((rc = do_prim<T>(c, in[s], need_max ? 1 : 0))) return rc;
     } else if (need_max) {
         if ((rc = do_max_speed<T>(c, in[s]))) return rc;
@@ -308,10 +306,7 @@ int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl, const double
         LAUNCHED(c, "begin_step_kernel");
         c->max_ready = false;
     }
-    T* Wnext = epi ? (T*)c->Wb[c->wcur ^ 1] : nullptr;
-    if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, Wnext, (marching && s == 2) ? 1 : 0))) return rc;
-    if (epi) c->wcur ^= 1;
-    c->w_ready = epi;
+    if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, (marching && s == 2) ? 1 : 0))) return rc;
     if (s == 2) {
         end_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
         LAUNCHED(c, "end_step_kernel");
@@ -339,8 +334,7 @@ void drop_graphs(hydro_ctx* c) {
 // epilogues) is a fixed sequence of launches whose only step-dependent inputs live in the device control block:
 // it can be replayed from a graph.
 bool graph_ready(const hydro_ctx* c) {
-    return c->use_graph && !c->profile && c->stream != nullptr && want_fused(c) && c->max_ready &&
-           (c->scheme == HYDRO_MUSTA_FORCE || c->w_ready);
+    return c->use_graph && !c->profile && c->stream != nullptr && want_fused(c) && c->max_ready;
 }
 
 template <class T>
@@ -422,11 +416,10 @@ int eval_L_impl(hydro_ctx* c, const void* cons, double t_stage, void* L_out) {
     const dim3 b = blk2d(64, 4);
     const dim3 g = grd(c->G.n[0], c->G.n[1], c->G.n[2], b);
     int rc;
-    c->w_ready = false;   // the primitive buffer is used as scratch
     pack_kernel<T><<<g, b, 0, c->stream>>>(c->G, (const T*)cons, U1);
     LAUNCHED(c, "pack_kernel");
     if ((rc = do_halo<T>(c, U1, 0.0, true, t_stage))) return rc;
-    if (c->scheme != HYDRO_MUSTA_FORCE && (rc = do_prim<T>(c, U1, 0))) return rc;
+    if (c->scheme != HYDRO_MUSTA_FORCE && !want_fused(c) && (rc = do_prim<T>(c, U1, 0))) return rc;
     if ((rc = do_stage<T>(c, U1, U1, U2, 0.0, 1.0, 1))) return rc;
     unpack_kernel<T><<<g, b, 0, c->stream>>>(c->G, U2, (T*)L_out);
     LAUNCHED(c, "unpack_kernel");
@@ -488,6 +481,8 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
     } else if (k == "kernel") {
         const int p = (int)v;
         if (p < 0 || p > 2) return fail(c, HYDRO_EINVAL, "kernel must be 0, 1 or 2");
+        if (c->ws && p == HYDRO_KERNEL_GENERIC && c->Wb[0] == nullptr)
+            return fail(c, HYDRO_EINVAL, "kernel = generic needs its primitive arrays: set it before the workspace is bound");
         c->kernel = p;
     } else if (k == "tile_zc" || k == "sweep_zc") {
         if (v < 1) return fail(c, HYDRO_EINVAL, "%s < 1", key);
@@ -541,7 +536,7 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
 
 size_t hydro_workspace_bytes(const hydro_ctx* c) {
     if (!c) return 0;
-    return 256 + 3 * state_bytes(c) + 2 * prim_bytes(c);  // control block, U0, U1, U2, W (two buffers)
+    return 256 + 3 * state_bytes(c) + (needs_w(c) ? prim_bytes(c) : 0);  // control block, U0, U1, U2, [W]
 }
 
 int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
@@ -562,8 +557,7 @@ int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
     c->ctl = (Ctl*)base;
     const size_t sb = state_bytes(c);
     for (int i = 0; i < 3; ++i) c->U[i] = base + 256 + i * sb;
-    c->Wb[0] = base + 256 + 3 * sb;
-    c->Wb[1] = c->Wb[0] + prim_bytes(c);
+    c->Wb[0] = c->Wb[1] = needs_w(c) ? base + 256 + 3 * sb : nullptr;
     c->wcur = 0;
     c->w_ready = c->max_ready = false;
     c->stage_open = 0;
@@ -572,9 +566,9 @@ int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
     set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, c->t_host, 1, 1);
     LAUNCHED(c, "set_ctl_kernel");
     c->fused_ready = false;
-    if (fused_supported(c->G) && c->kernel != HYDRO_KERNEL_GENERIC) {
+    if (fused_supported(c->G)) {
         c->fused_ready = (c->precision == HYDRO_F64 ? configure_marching<double>(c) : configure_marching<float>(c)) == 0;
-        if (!c->fused_ready && c->kernel == HYDRO_KERNEL_FUSED)
+        if (!c->fused_ready && c->kernel != HYDRO_KERNEL_GENERIC)
             return fail(c, HYDRO_ECUDA, "marching kernels: %s", c->plan_err);
     }
     return HYDRO_OK;
