@@ -16,9 +16,14 @@
 //
 // Parity pins (tests/test_oracle_*.py, all `-m "not gpu"`): con2prim round trip; wave speeds vs
 // numerical eigenvalues of dF/dU; WENO5/7 coefficients re-derived with exact rationals, linear
-// limit, orders 5/7; LLF and MUSTA consistency and scalar closed forms; SSP-RK3 stability
-// polynomial; uniform state, conservation, symmetry; exact Sod Riemann solution; d-dimensional
-// Hubble closed forms.  No function here is "parity unpinned".
+// limit, pointwise orders 5/7; LLF and MUSTA consistency and scalar closed forms; limiters; the
+// p = const closure; SSP-RK3 stability polynomial; uniform state, conservation; exact Sod Riemann
+// solution (test_oracle_solver.py); and in test_oracle_flows.py: d = 1, 2, 3 Hubble flows with the
+// analytic ghost fill and its stage times against closed forms that are themselves checked against
+// Eq. (1) by finite differences, configs 2 and 3 at reduced size, the outflow rule against a by-hand
+// extension, the FORCE flux for unequal velocities from its definition, charge advection at measured
+// order 5 / 7 / 2, an isentropic simple wave, mirror / permutation symmetry, the active-axes rule of
+// the CFL maximum and the Q16 clamp values.  No function here is "parity unpinned".
 //
 // Build: g++ -O2 -std=c++17 -shared -fPIC -ffp-contract=off hydro_oracle.cpp -o liboracle_hydro.so
 // (-ffp-contract=off: no FMA contraction, the arithmetic is exactly what is written).

@@ -2,7 +2,8 @@
 
 Nothing here is compared with the CUDA path.  Expected values are closed forms / invariants:
 uniform state, conservation, the RK3 stability polynomial acting on a Fourier mode of the linearised
-scheme, the exact Sod Riemann solution, d-dimensional Hubble flows, advection order, symmetries."""
+scheme, the exact Sod Riemann solution.  (The Hubble flows, advection orders, the simple wave and the symmetries are
+in tests/test_oracle_flows.py.)"""
 import math
 
 import numpy as np
