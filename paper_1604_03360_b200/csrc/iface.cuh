@@ -261,19 +261,35 @@ HD void musta_force_stages(const Acc& acc, int K, T C, int lim, int eos, T p0, T
 //   floating point),   4 F* = (F_L + Q_L/tau) + (F_R - Q_R/tau) + F(2 Q_M) = (G_L - G_R)/tau + F(2 Q_M),
 //   corrector: Q_L' = G_L - (tau/4)(4 F*),  Q_R' = G_R + (tau/4)(4 F*).
 // Returns FOUR TIMES the flux: the caller folds the 1/4 into its 1/dx factor (exact).
+// Admissibility of the states the branch-free path evaluates, accumulated over an interface as ONE running minimum
+// (a register, not a chain of booleans): after all evaluations `margin >= 0` must hold.
+//   fp64 (integer pipe, high words): margin = min over the states of  hi(E) - hi(1e-300) - 1  and
+//   hi(D) - hi(t) - 2, with D = 4 E^2 - 3 M^2 and t = E^2: hi(D) >= hi(t) + 2 means D > t (1 + 2^-21), i.e.
+//   |M| < (1 - 1e-7) E, well inside the Q16 bound; a negative E or D is a negative integer.  Infinities and NaNs can
+//   pass here: they make the flux non-finite, which musta_force_fast4 tests once at its end.
+//   fp32: the same two margins as floating-point differences.
+template <class T> struct MustaMargin { T m; };
+template <> struct MustaMargin<double> { int m; };
 template <class T>
-HD bool musta_fast_ok(T E, T t, T D) { return !below_floor(E) && D >= t * (T)1.0001; }
+HD void musta_margin_init(MustaMargin<T>& g) { g.m = (T)1; }
+template <class T>
+HD void musta_margin(MustaMargin<T>& g, T E, T t, T D) {
+    g.m = tmin(g.m, tmin(E - (T)1e-30, D - t * (T)1.0001));
+    if (!(D <= (T)3e38)) g.m = (T)-1;
+}
+template <class T>
+HD bool musta_margin_bad(const MustaMargin<T>& g) { return !(g.m >= (T)0); }
 template <class T>
 HD bool musta_finite(T x) { return tabs(x) <= (T)3e38; }
 #ifdef __CUDA_ARCH__
 template <>
-__device__ __forceinline__ bool musta_fast_ok<double>(double E, double t, double D) {
-    // two signed compares of high words (integer pipe).  E above the floor (a negative E is a negative integer);
-    // D = 4 E^2 - 3 M^2 against t = E^2: hi(D) >= hi(t) + 2 means D > t (1 + 2^-21), i.e. |M| < (1 - 1e-7) E, well
-    // inside the Q16 bound, and a negative D fails.  Infinities and NaNs can pass here: they make the flux
-    // non-finite, which musta_force_fast4 tests once at its end.
-    return __double2hiint(E) > 0x01a56e1f && __double2hiint(D) > __double2hiint(t) + 1;
+__device__ __forceinline__ void musta_margin_init<double>(MustaMargin<double>& g) { g.m = 0x7fffffff; }
+template <>
+__device__ __forceinline__ void musta_margin<double>(MustaMargin<double>& g, double E, double t, double D) {
+    g.m = min(g.m, min(__double2hiint(E) - 0x01a56e20, __double2hiint(D) - __double2hiint(t) - 2));
 }
+template <>
+__device__ __forceinline__ bool musta_margin_bad<double>(const MustaMargin<double>& g) { return g.m < 0; }
 template <>
 __device__ __forceinline__ bool musta_finite<double>(double x) {
     return (unsigned)(__double2hiint(x) << 1) < 0xffe00000u;
@@ -281,12 +297,12 @@ __device__ __forceinline__ bool musta_finite<double>(double x) {
 #endif
 
 template <class T, int DIR, bool SPEED>
-HD void musta_eval_fast(const T Q[NF], T F[NF], T& a, bool& bad) {
+HD void musta_eval_fast(const T Q[NF], T F[NF], T& a, MustaMargin<T>& g) {
     const T E = Q[0], md = Q[1 + DIR];
     const T m2 = tfma(Q[1], Q[1], tfma(Q[2], Q[2], Q[3] * Q[3]));
     const T t = E * E;
     const T D = tfma((T)4, t, (T)-3 * m2);
-    bad |= !musta_fast_ok(E, t, D);
+    musta_margin(g, E, t, D);
     const T s = fast_sqrt(D);
     const T w = (T)3 * fast_rcp(tfma((T)2, E, s));   // v_i = M_i w
     const T p = (s - E) * (T)(1.0 / 3.0);            // cancellation error: an ulp of E, i.e. an ulp of the flux it enters
@@ -304,6 +320,8 @@ HD void musta_eval_fast(const T Q[NF], T F[NF], T& a, bool& bad) {
 template <class T, int DIR, int KS>
 HD void musta_force_fast4(const T QL0[NF], const T QR0[NF], T C, T invC, T fh4[NF], bool& bad) {
     T QL[NF], QR[NF];
+    MustaMargin<T> g;
+    musta_margin_init(g);
 #pragma unroll
     for (int c = 0; c < NF; ++c) {
         QL[c] = QL0[c];
@@ -312,8 +330,8 @@ HD void musta_force_fast4(const T QL0[NF], const T QR0[NF], T C, T invC, T fh4[N
 #pragma unroll
     for (int stage = 1; stage <= KS; ++stage) {
         T FL[NF], FR[NF], GL[NF], GR[NF], Q2[NF], F2[NF], aL, aR, unused;
-        musta_eval_fast<T, DIR, true>(QL, FL, aL, bad);
-        musta_eval_fast<T, DIR, true>(QR, FR, aR, bad);
+        musta_eval_fast<T, DIR, true>(QL, FL, aL, g);
+        musta_eval_fast<T, DIR, true>(QR, FR, aR, g);
         const T S = max_nonneg(aL, aR);
         const T tau = C * fast_rcp(S), itau = S * invC;
 #pragma unroll
@@ -322,7 +340,7 @@ HD void musta_force_fast4(const T QL0[NF], const T QR0[NF], T C, T invC, T fh4[N
             GR[c] = tfma(-tau, FR[c], QR[c]);
             Q2[c] = GL[c] + GR[c];
         }
-        musta_eval_fast<T, DIR, false>(Q2, F2, unused, bad);
+        musta_eval_fast<T, DIR, false>(Q2, F2, unused, g);
         // (F_L + Q_L/tau) + (F_R - Q_R/tau) = (G_L - G_R)/tau
 #pragma unroll
         for (int c = 0; c < NF; ++c) fh4[c] = tfma(itau, GL[c] - GR[c], F2[c]);
@@ -336,7 +354,7 @@ HD void musta_force_fast4(const T QL0[NF], const T QR0[NF], T C, T invC, T fh4[N
         }
     }
     // a NaN or an infinity anywhere above has reached the flux
-    bad |= !musta_finite(((fh4[0] + fh4[1]) + (fh4[2] + fh4[3])) + fh4[4]);
+    bad = musta_margin_bad(g) || !musta_finite(((fh4[0] + fh4[1]) + (fh4[2] + fh4[3])) + fh4[4]);
 }
 
 template <class T, int DIR, class Acc>

@@ -196,20 +196,16 @@ musta_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* Un, T* U
         cp_async_wait<D - 1>();   // plane k's stage has landed
         const T* st = sm + ((k - k0) % D) * S::STAGE;
         const T* src = st + tid;
-        T u2[NF], hv[NF];
+        T u2[NF];
 #pragma unroll
         for (int c = 0; c < NF; ++c) u2[c] = src[c * TH];
-        if (lane < NHL) {
-            const T* hs = st + NS * TH + (wy * NHL + lane) * NF;
-#pragma unroll
-            for (int c = 0; c < NF; ++c) hv[c] = hs[c];
-        }
         __syncwarp();             // every lane is done with the row of plane k-1
 #pragma unroll
         for (int c = 0; c < NF; ++c) row[c * RWX + lane + R - 1] = zc_.u0[c];
-        if (lane < NHL) {
+        if (lane < NHL) {         // the halo cells go from their slots straight into the row
+            const T* hs = st + NS * TH + (wy * NHL + lane) * NF;
 #pragma unroll
-            for (int c = 0; c < NF; ++c) row[c * RWX + hq] = hv[c];
+            for (int c = 0; c < NF; ++c) row[c * RWX + hq] = hs[c];
         }
         __syncwarp();
         // z: face k + 1/2

@@ -47,11 +47,13 @@ constexpr int WENO_THREADS = 32 * WENO_ROWS;
 // per cell and axis cost 120 B of DRAM traffic per cell and stage against ~50 fp64 instructions to make them again;
 // the kernels are bound by instruction issue AND run at the board's power cap, where the bytes cost more clock than
 // the flops).
-template <class T, int NDIR>
+// EOS: the closure is a compile-time constant of the kernel (0: p = e/3, 1: p = p0): a run-time branch here costs
+// ~90 register moves per cell where its two sides merge.
+template <class T, int NDIR, int EOS>
 __device__ __forceinline__ void cell_prims(const T u[NF], const EosArgs& eos, const int (&dirs)[NDIR], T v[NDIR],
                                            T a[NDIR], T& p, int& flag) {
     T winv, v2;
-    if (eos.kind == 1) {
+    if (EOS == 1) {
         con2prim_p0(u[0], u[1], u[2], u[3], (T)eos.p0, winv, p, v2, flag);
 #pragma unroll
         for (int d = 0; d < NDIR; ++d) {
@@ -144,7 +146,7 @@ struct WenoXZShape {
     }
 };
 
-template <class T, int R>
+template <class T, int R, int EOS>
 __global__ void __launch_bounds__(WENO_THREADS, (R == 4 && sizeof(T) == 8) ? 2 : WENO5_MINB)
 weno_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* Un, T* Uout, Ctl* ctl, int zc) {
     using S = WenoXZShape<T, R>;
@@ -204,7 +206,7 @@ weno_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* Un, T* Uo
     // ring slot of its plane
     auto enter = [&](const T u[NF], T cell[NV], int slot, int& fl) {
         T v[2], a[2], p;
-        cell_prims<T, 2>(u, A.eos, dirs_zx, v, a, p, fl);
+        cell_prims<T, 2, EOS>(u, A.eos, dirs_zx, v, a, p, fl);
 #pragma unroll
         for (int c = 0; c < NF; ++c) cell[c] = u[c];
         cell[NF] = v[0];
@@ -263,7 +265,7 @@ weno_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* Un, T* Uo
             T u[NF], v[1], a[1], p;
 #pragma unroll
             for (int c = 0; c < NF; ++c) u[c] = hs[c];
-            cell_prims<T, 1>(u, A.eos, dirs_x, v, a, p, flag);
+            cell_prims<T, 1, EOS>(u, A.eos, dirs_x, v, a, p, flag);
 #pragma unroll
             for (int c = 0; c < NF; ++c) row[c * RWX + hq] = u[c];
             row[(NF + 0) * RWX + hq] = v[0];
@@ -313,7 +315,7 @@ constexpr size_t weno_y_smem_bytes() {
     return sizeof(T) * ((size_t)WENO_DEPTH * (NF + NF) + NF) * WENO_THREADS;
 }
 
-template <class T, int R, bool EPI>
+template <class T, int R, bool EPI, int EOS>
 __global__ void __launch_bounds__(WENO_THREADS, (R == 4 && sizeof(T) == 8) ? 2 : WENO5_MINB)
 weno_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl, int yc) {
     using Win = WenoWindow<T, R, 1>;
@@ -352,7 +354,7 @@ weno_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl, 
 
     auto enter = [&](const T u[NF], T cell[NV]) {
         T v[1], a[1], p;
-        cell_prims<T, 1>(u, A.eos, dirs_y, v, a, p, flag);
+        cell_prims<T, 1, EOS>(u, A.eos, dirs_y, v, a, p, flag);
 #pragma unroll
         for (int c = 0; c < NF; ++c) cell[c] = u[c];
         cell[NF] = v[0];
@@ -403,7 +405,7 @@ weno_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl, 
         issue(j + D);             // refill the slot just consumed
         if (EPI) {   // stage 3 of a CFL step: a4 of the finished cell (all three axes are active here)
             T w[NW];
-            prim_of_cell(o, w, flag, A.eos);
+            prim_of_cell_t<T, EOS>(o, w, flag, (T)A.eos.p0);
             amax = fmax(amax, fmax((double)w[W_AX], fmax((double)w[W_AX + 1], (double)w[W_AX + 2])));
         }
     }
@@ -413,14 +415,14 @@ weno_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl, 
 
 template <class T, int R>
 int configure_weno(char* err, size_t errlen) {
-    cudaError_t e = cudaFuncSetAttribute(weno_xz_kernel<T, R>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)WenoXZShape<T, R>::smem_bytes());
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(weno_y_kernel<T, R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)weno_y_smem_bytes<T, R>());
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(weno_y_kernel<T, R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)weno_y_smem_bytes<T, R>());
+    const int sxz = (int)WenoXZShape<T, R>::smem_bytes(), sy = (int)weno_y_smem_bytes<T, R>();
+    const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+    cudaError_t e = cudaFuncSetAttribute(weno_xz_kernel<T, R, 0>, attr, sxz);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(weno_xz_kernel<T, R, 1>, attr, sxz);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(weno_y_kernel<T, R, false, 0>, attr, sy);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(weno_y_kernel<T, R, true, 0>, attr, sy);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(weno_y_kernel<T, R, false, 1>, attr, sy);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(weno_y_kernel<T, R, true, 1>, attr, sy);
     if (e != cudaSuccess) {
         snprintf(err, errlen, "cudaFuncSetAttribute (weno): %s", cudaGetErrorString(e));
         return -1;
@@ -429,17 +431,24 @@ int configure_weno(char* err, size_t errlen) {
 }
 
 // stage = x/z kernel (writes Uout) + y sweep (adds L_y; stage 3 of a CFL step: the max signal speed of the new state)
+template <class T, int R, int EOS>
+void launch_weno_eos(const Geom& G, const StageArgs& A, const T* Us, const T* Un, T* Uout, Ctl* ctl, int zc, int yc,
+                     cudaStream_t st) {
+    const dim3 b(32, WENO_ROWS, 1);
+    const dim3 g((G.n[0] + 30) / 31, (G.n[1] + WENO_ROWS - 1) / WENO_ROWS, (G.n[2] + zc - 1) / zc);
+    weno_xz_kernel<T, R, EOS><<<g, b, WenoXZShape<T, R>::smem_bytes(), st>>>(G, A, Us, Un, Uout, ctl, zc);
+    const dim3 gy((G.n[0] + 31) / 32, (G.n[2] + WENO_ROWS - 1) / WENO_ROWS, (G.n[1] + yc - 1) / yc);
+    if (A.epi_max && A.mode != 1)
+        weno_y_kernel<T, R, true, EOS><<<gy, b, weno_y_smem_bytes<T, R>(), st>>>(G, A, Us, Uout, ctl, yc);
+    else
+        weno_y_kernel<T, R, false, EOS><<<gy, b, weno_y_smem_bytes<T, R>(), st>>>(G, A, Us, Uout, ctl, yc);
+}
+
 template <class T, int R>
 int launch_weno(const Geom& G, const StageArgs& A, const T* Us, const T* Un, T* Uout, Ctl* ctl, int zc, int yc,
                 cudaStream_t st, int* launches, char* err, size_t errlen) {
-    const dim3 b(32, WENO_ROWS, 1);
-    const dim3 g((G.n[0] + 30) / 31, (G.n[1] + WENO_ROWS - 1) / WENO_ROWS, (G.n[2] + zc - 1) / zc);
-    weno_xz_kernel<T, R><<<g, b, WenoXZShape<T, R>::smem_bytes(), st>>>(G, A, Us, Un, Uout, ctl, zc);
-    const dim3 gy((G.n[0] + 31) / 32, (G.n[2] + WENO_ROWS - 1) / WENO_ROWS, (G.n[1] + yc - 1) / yc);
-    if (A.epi_max && A.mode != 1)
-        weno_y_kernel<T, R, true><<<gy, b, weno_y_smem_bytes<T, R>(), st>>>(G, A, Us, Uout, ctl, yc);
-    else
-        weno_y_kernel<T, R, false><<<gy, b, weno_y_smem_bytes<T, R>(), st>>>(G, A, Us, Uout, ctl, yc);
+    if (A.eos.kind == 1) launch_weno_eos<T, R, 1>(G, A, Us, Un, Uout, ctl, zc, yc, st);
+    else launch_weno_eos<T, R, 0>(G, A, Us, Un, Uout, ctl, zc, yc, st);
     *launches = 2;
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) {
