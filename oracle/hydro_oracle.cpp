@@ -49,15 +49,31 @@ enum { NF = 5 };  // E, Mx, My, Mz, R
 template <class T>
 struct Prim {
     T e, p, n, v[3];
+    T cs2 = (T)1 / (T)3;   // dp/de at this state (1/3 for p = e/3, 0 for p = p0, the table's slope for kind 2)
 };
 
 // Equation of state.  kind 0: p = e/3 (reading Q2, the default everywhere).  kind 1: p = p0, a
 // constant: the closure for which the anisotropic free-streaming flow of the paper's ref. [8]
 // is an exact solution.
+// kind 2: a TABULATED barotropic closure p(e) (SURVEY 8(f)-N1 second half; the paper's physics, needs a
+// general equation of state): n values p_i = p(e_i) at e_i = e_min + i (e_max - e_min)/(n - 1), interpolated linearly
+// in e; below e_min and above e_max the first / last segment is continued.  c_s^2 = dp/de is the segment's slope.
 struct Eos {
     int kind;
     double p0;
-    Eos() : kind(0), p0(0.0) {}
+    std::vector<double> tab;
+    double e_min, e_max;
+    Eos() : kind(0), p0(0.0), e_min(0.0), e_max(1.0) {}
+    // p and dp/de of the table at energy density e
+    void lookup(double e, double& p, double& cs2) const {
+        const int n = (int)tab.size();
+        const double de = (e_max - e_min) / (n - 1);
+        int i = (int)std::floor((e - e_min) / de);
+        if (i < 0) i = 0;
+        if (i > n - 2) i = n - 2;
+        cs2 = (tab[i + 1] - tab[i]) / de;
+        p = tab[i] + (e - (e_min + i * de)) * cs2;
+    }
 };
 
 // O1'. p = p0 constant: from E + p0 = (e + p0) gamma^2 and M = (e + p0) gamma^2 v:
@@ -86,6 +102,52 @@ Prim<T> con2prim_pconst(const T u[NF], int* flag, T p0) {
     }
     w.e = (H - p0) - Mabs * Mabs / H;
     w.p = p0;
+    w.cs2 = (T)0;
+    w.n = R * std::sqrt((T)1 - v2);
+    return w;
+}
+
+// O1''. tabulated p(e): from e = E - M.v and v = M/(E + p) the energy density solves
+//   f(e) = E - M^2/(E + p(e)) - e = 0,   f'(e) = M^2 p'(e)/(E + p(e))^2 - 1 = v^2 c_s^2 - 1 < 0,
+// by Newton's iteration from e = E (where f <= 0), until the step is below 1e-15 e (at most 60 steps); then
+// v_i = M_i/(E + p), n = R sqrt(1 - v^2).  Clamps as for p = e/3 (Q16): E >= 1e-300, |M| <= (1 - 1e-12) E, which
+// keeps e > 0 for any table with p >= 0.
+template <class T>
+Prim<T> con2prim_table(const T u[NF], int* flag, const Eos& eos) {
+    T E = u[0], M[3] = {u[1], u[2], u[3]}, R = u[4];
+    if (!(E >= (T)1e-300)) {
+        E = (T)1e-300;
+        if (flag) *flag = 1;
+    }
+    T Mabs = std::sqrt(M[0] * M[0] + M[1] * M[1] + M[2] * M[2]);
+    const T lim = ((T)1 - (T)1e-12) * E;
+    if (!(Mabs <= lim)) {
+        const T sc = lim / Mabs;
+        for (int i = 0; i < 3; ++i) M[i] *= sc;
+        Mabs = lim;
+        if (flag) *flag = 1;
+    }
+    double e = (double)E, p = 0, cs2 = 0;
+    for (int it = 0; it < 60; ++it) {
+        eos.lookup(e, p, cs2);
+        const double H = (double)E + p;
+        const double f = (double)E - (double)Mabs * (double)Mabs / H - e;
+        const double fp = (double)Mabs * (double)Mabs * cs2 / (H * H) - 1.0;
+        const double en = e - f / fp;
+        const bool done = std::fabs(en - e) <= 1e-15 * std::fabs(en);
+        e = en;
+        if (done) break;
+    }
+    eos.lookup(e, p, cs2);
+    Prim<T> w;
+    T v2 = 0;
+    for (int i = 0; i < 3; ++i) {
+        w.v[i] = M[i] / (E + (T)p);
+        v2 += w.v[i] * w.v[i];
+    }
+    w.e = (T)e;
+    w.p = (T)p;
+    w.cs2 = (T)cs2;
     w.n = R * std::sqrt((T)1 - v2);
     return w;
 }
@@ -93,6 +155,7 @@ Prim<T> con2prim_pconst(const T u[NF], int* flag, T p0) {
 template <class T>
 Prim<T> con2prim(const T u[NF], int* flag, const Eos& eos = Eos()) {
     if (eos.kind == 1) return con2prim_pconst<T>(u, flag, (T)eos.p0);
+    if (eos.kind == 2) return con2prim_table<T>(u, flag, eos);
     T E = u[0], M[3] = {u[1], u[2], u[3]}, R = u[4];
     if (!(E >= (T)1e-300)) {
         E = (T)1e-300;
@@ -132,6 +195,18 @@ T signal_speed(const T v[3], int d, const Eos& eos = Eos()) {
     const T vd = v[d];
     const T disc = ((T)1 - v2) * ((T)1 - vd * vd - (v2 - vd * vd) * cs2);
     return (std::fabs(vd) * ((T)1 - cs2) + cs * std::sqrt(disc)) / ((T)1 - v2 * cs2);
+}
+
+// The same for the state w with ITS sound speed (w.cs2 = dp/de: 1/3, 0, or the table's slope):
+//   a_d = ( |v_d|(1-cs2) + sqrt(cs2 (1-v^2)(1 - v_d^2 - (v^2 - v_d^2) cs2)) ) / (1 - v^2 cs2)
+template <class T>
+T signal_speed(const Prim<T>& w, int d, const Eos& eos) {
+    if (eos.kind != 2) return signal_speed(w.v, d, eos);
+    const T cs2 = w.cs2;
+    const T v2 = w.v[0] * w.v[0] + w.v[1] * w.v[1] + w.v[2] * w.v[2];
+    const T vd = w.v[d];
+    const T disc = cs2 * ((T)1 - v2) * ((T)1 - vd * vd - (v2 - vd * vd) * cs2);
+    return (std::fabs(vd) * ((T)1 - cs2) + std::sqrt(disc)) / ((T)1 - v2 * cs2);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -220,7 +295,7 @@ void llf_weno_flux(int r, const T cells[][NF], int d, T eps, T fhat[NF], int* fl
     for (int k = 0; k < 2 * r; ++k) {
         const Prim<T> w = con2prim(cells[k], flag, eos);
         phys_flux(cells[k], w, d, F[k]);
-        a[k] = signal_speed(w.v, d, eos);
+        a[k] = signal_speed(w, d, eos);
     }
     llf_weno_split(r, cells, F, a, eps, fhat);
 }
@@ -270,7 +345,7 @@ void musta_force_flux(const T cells[4][NF], int d, int K, T C, T fstar[NF], int*
         T FL[NF], FR[NF], QM[NF], FM[NF];
         phys_flux(QL, wl, d, FL);
         phys_flux(QR, wr, d, FR);
-        const T S = std::fmax(signal_speed(wl.v, d, eos), signal_speed(wr.v, d, eos));
+        const T S = std::fmax(signal_speed(wl, d, eos), signal_speed(wr, d, eos));
         const T tau = C / S;
         for (int c = 0; c < NF; ++c) QM[c] = (QL[c] + QR[c]) / (T)2 - tau * (FR[c] - FL[c]) / (T)2;
         const Prim<T> wm = con2prim(QM, flag, eos);
@@ -403,7 +478,7 @@ struct Solver {
                 load(pad, jx[0], jx[1], jx[2], cells[m]);
                 const Prim<T>& w = prim[pidx(jx[0], jx[1], jx[2])];
                 phys_flux(cells[m], w, a, F[m]);
-                sp[m] = signal_speed(w.v, a, eos);
+                sp[m] = signal_speed(w, a, eos);
             }
             llf_weno_split<T>(r, cells, F, sp, (T)eps, fh);
         }
@@ -522,7 +597,7 @@ struct Solver {
                     load(u, i, j, k, c);
                     const Prim<T> w = con2prim(c, &flag, eos);
                     for (int a = 0; a < 3; ++a)
-                        if (g[a] > 0) m = std::fmax(m, (double)signal_speed(w.v, a, eos));
+                        if (g[a] > 0) m = std::fmax(m, (double)signal_speed(w, a, eos));
                 }
         return m;
     }
@@ -597,7 +672,9 @@ int oracle_set_option(oracle_ctx* c, const char* key, double v) {
             if (b < 0 || b > 2) rc = EINVAL_; else S->bc[k[3] - 'x'] = b;
         } else if (k == "musta_stages") { if (v < 1) rc = EINVAL_; else S->musta_stages = (int)v; }
         else if (k == "musta_cfl") { if (!(v > 0)) rc = EINVAL_; else S->musta_cfl = v; }
-        else if (k == "eos") { if (v != 0 && v != 1) rc = EINVAL_; else S->eos.kind = (int)v; }
+        else if (k == "eos") {
+            if (v != 0 && v != 1 && !(v == 2 && S->eos.tab.size() >= 2)) rc = EINVAL_; else S->eos.kind = (int)v;
+        }
         else if (k == "eos_p0") { if (!(v >= 0)) rc = EINVAL_; else S->eos.p0 = v; }
         else if (k == "limiter") { if (v < 0 || v > 3) rc = EINVAL_; else S->limiter = (int)v; }
         else if (k == "weno_eps") { if (!(v > 0)) rc = EINVAL_; else S->eps = v; }
@@ -708,6 +785,28 @@ int oracle_con2prim_eos(const double u[5], int eos, double p0, double prim_out[6
 double oracle_signal_speed_eos(const double v[3], int d, int eos, double p0) {
     Eos q; q.kind = eos; q.p0 = p0;
     return signal_speed<double>(v, d, q);
+}
+// tabulated closure: n >= 2 values p(e_i) on the uniform grid e_min .. e_max (host pointer); selects kind 2
+int oracle_set_eos_table(oracle_ctx* c, const double* p, int n, double e_min, double e_max) {
+    if (!c || !p || n < 2 || !(e_max > e_min)) return EINVAL_;
+    BOTH(c, {
+        S->eos.tab.assign(p, p + n);
+        S->eos.e_min = e_min;
+        S->eos.e_max = e_max;
+        S->eos.kind = 2;
+    });
+    return OK;
+}
+// pointwise pieces with a table: prim_out = e, p, n, vx, vy, vz, cs2; speeds of that state along x, y, z
+int oracle_con2prim_table(const double u[5], const double* p, int n, double e_min, double e_max, double prim_out[7],
+                          double speeds_out[3]) {
+    Eos q; q.kind = 2; q.tab.assign(p, p + n); q.e_min = e_min; q.e_max = e_max;
+    int flag = 0;
+    const Prim<double> w = con2prim<double>(u, &flag, q);
+    prim_out[0] = w.e; prim_out[1] = w.p; prim_out[2] = w.n;
+    prim_out[3] = w.v[0]; prim_out[4] = w.v[1]; prim_out[5] = w.v[2]; prim_out[6] = w.cs2;
+    for (int d = 0; d < 3; ++d) speeds_out[d] = signal_speed<double>(w, d, q);
+    return flag;
 }
 double oracle_limited_slope(int lim, double a, double b) { return limited_slope<double>(lim, a, b); }
 int oracle_musta_force_flux_lim(const double* cells, int d, int K, double C, int lim, double fstar[5]) {

@@ -48,6 +48,8 @@ def lib():
         L.oracle_get_time.argtypes = [vp, pd]
         L.oracle_eval_L.argtypes = [vp, vp, dbl, vp]
         L.oracle_eval_L_extended.argtypes = [vp, vp, dbl, vp]
+        L.oracle_set_eos_table.argtypes = [vp, pd, i32, dbl, dbl]
+        L.oracle_con2prim_table.argtypes = [pd, pd, i32, dbl, dbl, pd, pd]
         L.oracle_con2prim.argtypes = [pd, pd]
         L.oracle_signal_speed.argtypes = [pd, i32]
         L.oracle_signal_speed.restype = dbl
@@ -104,6 +106,14 @@ def con2prim_eos(u, eos, p0):
     out = np.empty(6)
     flag = lib().oracle_con2prim_eos(_pd(u), int(eos), float(p0), _pd(out))
     return out, flag
+
+
+def con2prim_table(u, p, e_min, e_max):
+    """(e, p, n, vx, vy, vz, cs2), (a_x, a_y, a_z), flag for the tabulated closure."""
+    a = np.ascontiguousarray(p, dtype=np.float64)
+    prim, sp = np.zeros(7), np.zeros(3)
+    flag = lib().oracle_con2prim_table(_pd(_arr(u, 5)), _pd(a), len(a), float(e_min), float(e_max), _pd(prim), _pd(sp))
+    return prim, sp, flag
 
 
 def phys_flux(u, d):
@@ -202,6 +212,12 @@ class Oracle:
         lib().oracle_eval_L(self._h, a.ctypes.data, float(t_stage), out.ctypes.data)
         return out
 
+    def set_eos_table(self, p, e_min, e_max):
+        """Tabulated closure p(e): values on the uniform grid e_min .. e_max; selects eos kind 2."""
+        a = np.ascontiguousarray(p, dtype=np.float64)
+        rc = lib().oracle_set_eos_table(self._h, _pd(a), len(a), float(e_min), float(e_max))
+        assert rc == 0
+
     def eval_L_extended(self, cons, t_stage=0.0):
         """L(u) by the same code in long double, rounded to double (a referee for the fp64 oracle's own rounding)."""
         assert self.dtype == np.float64
@@ -234,6 +250,8 @@ def from_workload(w, precision=0):
     o.set_option("t", w.t0)
     for k, v in w.options.items():
         o.set_option(k, v)
+    if getattr(w, "eos_table", None) is not None:
+        o.set_eos_table(*w.eos_table)
     if precision:
         o.set_option("precision", precision)
     o.set_state(w.cons)

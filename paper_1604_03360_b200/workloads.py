@@ -36,6 +36,7 @@ class Workload:
     dt: float | None = None      # fixed dt (config 2)
     nsteps: int = 0
     options: dict = dataclasses.field(default_factory=dict)
+    eos_table: tuple | None = None   # (p values on a uniform e grid, e_min, e_max): tabulated closure p(e), eos kind 2
 
 
 def prim_to_cons(e, n, vx, vy, vz):
@@ -67,6 +68,14 @@ def prim_to_cons_p0(e, n, vx, vy, vz, p0):
     out[3] = w * vz
     out[4] = n * np.sqrt(g2)
     return out
+
+
+def crossover_eos_table(n=4096, e_max=64.0, a=0.18, e_c=1.0):
+    """A smooth 'crossover' equation of state as a table (input data for the tabulated closure):
+    c_s^2(e) = 1/3 - a/(1 + (e/e_c)^2) rises from 1/3 - a at low energy density to 1/3 (the p = e/3 gas) at high,
+    p(e) = e/3 - a e_c atan(e/e_c).  Returns (p values at n uniform points of [0, e_max], 0.0, e_max)."""
+    e = np.linspace(0.0, e_max, n)
+    return e / 3.0 - a * e_c * np.arctan(e / e_c), 0.0, float(e_max)
 
 
 def cell_centres(n, dx, origin):
