@@ -132,6 +132,15 @@ int hydro_step(hydro_ctx *ctx, double dt, int nsteps);
  * Asynchronous. */
 int hydro_step_cfl(hydro_ctx *ctx, double cfl, int nsteps);
 
+/* Tabulated barotropic equation of state p(e) (the quark-gluon-plasma physics the solver
+ * is for needs a general equation of state): n >= 2 values p(e_i) at e_i = e_min + i (e_max - e_min)/(n - 1) in
+ * DEVICE memory, ALWAYS doubles, owned by the caller and kept alive while the context uses them.  p is interpolated
+ * linearly in e (the first and last segments are continued beyond the table), c_s^2 = dp/de is the segment's slope;
+ * conserved -> primitive solves E - M^2/(E + p(e)) - e = 0 by Newton's iteration, the characteristic speeds use the
+ * state's own c_s^2.  Selects option "eos" = 2 ("eos" = 0 / 1 switches back; "eos" = 2 re-selects the table).
+ * EINVAL: null or non-device pointer, n < 2, e_max <= e_min. */
+int hydro_set_eos_table(hydro_ctx *ctx, const void *p_device, int n, double e_min, double e_max);
+
 /* Event-by-event batches ("event-by-event simulations"): advance nctx independent
  * contexts by nsteps CFL steps each.  The steps are issued round-robin over the batch, every context on its own
  * stream (hydro_set_stream), so that the kernels of small grids run side by side on the GPU.  Asynchronous; the

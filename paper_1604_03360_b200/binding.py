@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libhydro_b200.so")
 SYMBOLS = [
     "hydro_create", "hydro_set_option", "hydro_set_stream", "hydro_workspace_bytes", "hydro_bind_workspace",
     "hydro_set_state", "hydro_get_state", "hydro_set_state_host", "hydro_get_state_host", "hydro_step",
-    "hydro_step_cfl", "hydro_step_cfl_batch", "hydro_max_signal_speed", "hydro_eval_L", "hydro_get_time", "hydro_status",
+    "hydro_step_cfl", "hydro_step_cfl_batch", "hydro_set_eos_table", "hydro_max_signal_speed", "hydro_eval_L", "hydro_get_time", "hydro_status",
     "hydro_launch_count", "hydro_stage_kernel_time", "hydro_last_error",
     "hydro_zhalo_elems", "hydro_get_zhalo", "hydro_put_zhalo", "hydro_step_stage", "hydro_local_max_speed",
     "hydro_step_stage_cfl", "hydro_destroy",
@@ -56,6 +56,7 @@ def _load():
     L.hydro_step.argtypes = [vp, dbl, i32]
     L.hydro_step_cfl.argtypes = [vp, dbl, i32]
     L.hydro_step_cfl_batch.argtypes = [ctypes.POINTER(vp), i32, dbl, i32]
+    L.hydro_set_eos_table.argtypes = [vp, vp, i32, dbl, dbl]
     L.hydro_max_signal_speed.argtypes = [vp, pd]
     L.hydro_eval_L.argtypes = [vp, vp, dbl, vp]
     L.hydro_get_time.argtypes = [vp, pd]
@@ -103,6 +104,13 @@ class Hydro:
 
     def set_option(self, key, value):
         self._check(lib.hydro_set_option(self._h, key.encode(), float(value)))
+
+    def set_eos_table(self, p, e_min, e_max):
+        """Tabulated closure p(e): `p` = values on the uniform grid e_min .. e_max (any array-like; uploaded as a
+        float64 device tensor that this object keeps alive)."""
+        self._eos_table = torch.as_tensor(p, dtype=torch.float64).to(self.device).contiguous()
+        self._check(lib.hydro_set_eos_table(self._h, self._eos_table.data_ptr(), self._eos_table.numel(),
+                                            float(e_min), float(e_max)))
 
     def workspace_bytes(self):
         return lib.hydro_workspace_bytes(self._h)
@@ -249,6 +257,8 @@ def from_workload(w, precision=F64, kernel=KERNEL_AUTO, device="cuda"):
     h.set_option("kernel", kernel)
     for k, v in w.options.items():
         h.set_option(k, v)
+    if getattr(w, "eos_table", None) is not None:
+        h.set_eos_table(*w.eos_table)
     h.bind()
     h.set_state(torch.from_numpy(w.cons).to(device=device, dtype=h.dtype).contiguous())
     return h

@@ -170,6 +170,80 @@ HD void con2prim_p0(T E, T M0, T M1, T M2, T p0, T& winv, T& p, T& v2, int& flag
     winv = w * sc;
 }
 
+// Equation of state of a context.  kind 0: p = e/3 (reading Q2); 1: p = p0 (reading Q14);
+// 2: tabulated barotropic p(e) (second half of N1): n values on the uniform grid e_min + i de in the caller's DEVICE
+// memory (always doubles), interpolated linearly, the end segments continued; c_s^2 = dp/de is the segment's slope.
+struct EosArgs {
+    int kind;
+    double p0;
+    const double* tab;
+    int n;
+    double e_min, de;
+};
+
+// p and dp/de of the table at energy density e.  The segment index and the slope use true divisions, so that the
+// choice of segment is the one any IEEE evaluation of floor((e - e_min)/de) makes.
+HD void eos_table_lookup(const EosArgs& eos, double e, double& p, double& cs2) {
+    int i = (int)floor((e - eos.e_min) / eos.de);
+    i = i < 0 ? 0 : (i > eos.n - 2 ? eos.n - 2 : i);
+#ifdef __CUDA_ARCH__
+    const double pa = __ldg(eos.tab + i), pb = __ldg(eos.tab + i + 1);
+#else
+    const double pa = eos.tab[i], pb = eos.tab[i + 1];
+#endif
+    cs2 = (pb - pa) / eos.de;
+    p = pa + (e - (eos.e_min + i * eos.de)) * cs2;
+}
+
+// con2prim for the tabulated closure: the energy density solves f(e) = E - M^2/(E + p(e)) - e = 0 with
+// f' = v^2 c_s^2 - 1 < 0; Newton's iteration from e = E until the step falls below 1e-15 e (at most 60 steps), in
+// double whatever T is.  Same outputs and clamp policy (E >= 1e-300, |M| <= (1 - 1e-12) E) as con2prim, plus cs2.
+template <class T>
+HD void con2prim_tab(T E_, T M0, T M1, T M2, const EosArgs& eos, T& winv, T& p, T& v2, T& cs2, int& flag) {
+    double E = (double)E_;
+    if (below_floor(E_)) {
+        E = 1e-300;
+        flag = 1;
+    }
+    double m2 = (double)M0 * M0 + (double)M1 * M1 + (double)M2 * M2;
+    double sc = 1.0;
+    const double lim = (1.0 - 1e-12) * E;
+    if (!(m2 <= lim * lim)) {
+        const double mabs = sqrt(m2);
+        if (!(mabs <= lim)) {
+            sc = lim / mabs;
+            m2 = lim * lim;
+            flag = 1;
+        }
+    }
+    double e = E, pe = 0.0, c2 = 0.0;
+    for (int it = 0; it < 60; ++it) {
+        eos_table_lookup(eos, e, pe, c2);
+        const double H = E + pe;
+        const double f = E - m2 / H - e;
+        const double fp = m2 * c2 / (H * H) - 1.0;
+        const double en = e - f / fp;
+        const bool done = fabs(en - e) <= 1e-15 * fabs(en);
+        e = en;
+        if (done) break;
+    }
+    eos_table_lookup(eos, e, pe, c2);
+    const double w = 1.0 / (E + pe);
+    p = (T)pe;
+    cs2 = (T)c2;
+    v2 = (T)(m2 * w * w);
+    winv = (T)(w * sc);
+}
+
+// a3 for a state with its own sound speed (tabulated closure):
+//   a_d = ( |v_d| (1-cs2) + sqrt(cs2 (1-v^2)(1 - v_d^2 - (v^2 - v_d^2) cs2)) ) / (1 - v^2 cs2)
+template <class T>
+HD T signal_speed_cs(T vd, T v2, T cs2) {
+    const T vd2 = vd * vd;
+    const T disc = max_nonneg(cs2 * ((T)1 - v2) * ((T)1 - vd2 - (v2 - vd2) * cs2), (T)0);
+    return (tabs(vd) * ((T)1 - cs2) + tsqrt(disc)) / ((T)1 - v2 * cs2);
+}
+
 // a3. directional characteristic speeds, c_s^2 = 1/3 (a3):
 //   a_d = ( |v_d| (1-cs2) + cs sqrt((1-v^2)(1 - v_d^2 - (v^2 - v_d^2) cs2)) ) / (1 - v^2 cs2)
 // FLOOR = false: for states known to be well inside |v| < 1 (the branch-free MUSTA path), where disc > 0 holds with

@@ -30,7 +30,7 @@ struct hydro_ctx {
     double eps = 1e-6, musta_cfl = 0.9;
     int musta_stages = 2;
     int limiter = 0;
-    EosArgs eos = {0, 0.0};
+    EosArgs eos = {0, 0.0, nullptr, 0, 0.0, 1.0};
     double t_host = 0.0;  // value to push into the control block at bind / set_option("t")
     HubbleParams H;
     cudaStream_t stream = nullptr;
@@ -497,7 +497,8 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
         if (v < 1) return fail(c, HYDRO_EINVAL, "musta_stages < 1");
         c->musta_stages = (int)v;
     } else if (k == "eos") {
-        if (v != 0.0 && v != 1.0) return fail(c, HYDRO_EINVAL, "eos must be 0 (p = e/3) or 1 (p = p0)");
+        if (v != 0.0 && v != 1.0 && !(v == 2.0 && c->eos.tab != nullptr))
+            return fail(c, HYDRO_EINVAL, "eos must be 0 (p = e/3), 1 (p = p0) or 2 (after hydro_set_eos_table)");
         c->eos.kind = (int)v;
         c->w_ready = c->max_ready = false;   // cached primitives and max signal speed belong to the old closure
     } else if (k == "eos_p0") {
@@ -656,6 +657,24 @@ int hydro_step_cfl(hydro_ctx* c, double cfl, int nsteps) {
         else rc = c->precision == HYDRO_F64 ? do_step<double>(c, -1.0, cfl) : do_step<float>(c, -1.0, cfl);
         if (rc) return rc;
     }
+    return HYDRO_OK;
+}
+
+int hydro_set_eos_table(hydro_ctx* c, const void* p_device, int n, double e_min, double e_max) {
+    if (!c) return HYDRO_EINVAL;
+    if (!p_device || n < 2 || !(e_max > e_min)) return fail(c, HYDRO_EINVAL, "hydro_set_eos_table: null table, n < 2 or e_max <= e_min");
+    cudaPointerAttributes attr;
+    if (cudaPointerGetAttributes(&attr, p_device) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+        cudaGetLastError();
+        return fail(c, HYDRO_EINVAL, "hydro_set_eos_table: the table is not CUDA device memory");
+    }
+    drop_graphs(c);
+    c->eos.tab = (const double*)p_device;
+    c->eos.n = n;
+    c->eos.e_min = e_min;
+    c->eos.de = (e_max - e_min) / (n - 1);
+    c->eos.kind = 2;
+    c->w_ready = c->max_ready = false;
     return HYDRO_OK;
 }
 

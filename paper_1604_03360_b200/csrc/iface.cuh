@@ -133,22 +133,25 @@ HD T limited_slope(int lim, T a, T b) {
 // con2prim, O7).  Q is modified only if the Q16 clamp fires.  EOSRT: the equation of state is the run-time
 // (eos, p0); otherwise the default p = e/3 at compile time.
 template <class T, int DIR, bool EOSRT>
-HD void flux_and_speed(const T Q[NF], T F[NF], T& a, int& flag, int eos, T p0) {
-    T winv, p, v2;
-    if (EOSRT && eos == 1) con2prim_p0(Q[0], Q[1], Q[2], Q[3], p0, winv, p, v2, flag);
+HD void flux_and_speed(const T Q[NF], T F[NF], T& a, int& flag, const EosArgs& eos) {
+    T winv, p, v2, cs2 = (T)0;
+    if (EOSRT && eos.kind == 1) con2prim_p0(Q[0], Q[1], Q[2], Q[3], (T)eos.p0, winv, p, v2, flag);
+    else if (EOSRT && eos.kind == 2) con2prim_tab(Q[0], Q[1], Q[2], Q[3], eos, winv, p, v2, cs2, flag);
     else con2prim(Q[0], Q[1], Q[2], Q[3], winv, p, v2, flag);
     const T vd = Q[1 + DIR] * winv;
     F[0] = Q[1 + DIR];
 #pragma unroll
     for (int j = 0; j < 3; ++j) F[1 + j] = (j == DIR) ? tfma(Q[1 + j], vd, p) : Q[1 + j] * vd;
     F[4] = Q[4] * vd;
-    if (EOSRT && eos == 1) a = tabs(vd);
+    if (EOSRT && eos.kind == 1) a = tabs(vd);
+    else if (EOSRT && eos.kind == 2) a = signal_speed_cs(vd, v2, cs2);
     else a = signal_speed(vd, v2, speed_inv_den(v2));
 }
 template <class T, int DIR, bool EOSRT>
-HD void flux_only(const T Q[NF], T F[NF], int& flag, int eos, T p0) {
-    T winv, p, v2;
-    if (EOSRT && eos == 1) con2prim_p0(Q[0], Q[1], Q[2], Q[3], p0, winv, p, v2, flag);
+HD void flux_only(const T Q[NF], T F[NF], int& flag, const EosArgs& eos) {
+    T winv, p, v2, cs2;
+    if (EOSRT && eos.kind == 1) con2prim_p0(Q[0], Q[1], Q[2], Q[3], (T)eos.p0, winv, p, v2, flag);
+    else if (EOSRT && eos.kind == 2) con2prim_tab(Q[0], Q[1], Q[2], Q[3], eos, winv, p, v2, cs2, flag);
     else con2prim(Q[0], Q[1], Q[2], Q[3], winv, p, v2, flag);
     const T vd = Q[1 + DIR] * winv;
     F[0] = Q[1 + DIR];
@@ -168,8 +171,9 @@ HD void musta_flux(const T Q[NF], T F[NF], T& a, int& flag) {
     const T t = E * E;
     const T c2 = ((T)1 - (T)1e-12) * ((T)1 - (T)1e-12);
     if (below_floor(E) || !(m2 <= c2 * t)) {   // rare (kept inline: out of line, Q and F would live in local memory)
-        if (SPEED) flux_and_speed<T, DIR, false>(Q, F, a, flag, 0, (T)0);
-        else flux_only<T, DIR, false>(Q, F, flag, 0, (T)0);
+        const EosArgs gas = {0, 0.0, nullptr, 0, 0.0, 1.0};
+        if (SPEED) flux_and_speed<T, DIR, false>(Q, F, a, flag, gas);
+        else flux_only<T, DIR, false>(Q, F, flag, gas);
         return;
     }
     const T s = fast_sqrt(tfma((T)4, t, (T)-3 * m2));
@@ -194,15 +198,15 @@ HD T musta_slope(int lim, T dm, T dp) { return LIMS == 0 ? minmod(dm, dp) : limi
 // the Q16 clamp, K and the closure may be run-time values.  QL, QR are overwritten by the corrected states.
 // KS > 0: the number of stages is the compile-time constant KS; KS = 0: run-time K.
 template <class T, int DIR, int KS, bool EOSRT>
-HD void musta_force_core(T QL[NF], T QR[NF], int K, T C, int eos, T p0, T fh[NF], int& flag) {
+HD void musta_force_core(T QL[NF], T QR[NF], int K, T C, const EosArgs& eos, T fh[NF], int& flag) {
     const T invC = fast_rcp(C);   // (one MUFU-seeded reciprocal per interface; a true division costs a subroutine)
     const int nst = KS > 0 ? KS : K;
 #pragma unroll
     for (int stage = 1; stage <= nst; ++stage) {
         T FL[NF], FR[NF], QM[NF], FM[NF], aL, aR;
         if (EOSRT) {
-            flux_and_speed<T, DIR, true>(QL, FL, aL, flag, eos, p0);
-            flux_and_speed<T, DIR, true>(QR, FR, aR, flag, eos, p0);
+            flux_and_speed<T, DIR, true>(QL, FL, aL, flag, eos);
+            flux_and_speed<T, DIR, true>(QR, FR, aR, flag, eos);
         } else {
             musta_flux<T, DIR, true>(QL, FL, aL, flag);
             musta_flux<T, DIR, true>(QR, FR, aR, flag);
@@ -214,7 +218,7 @@ HD void musta_force_core(T QL[NF], T QR[NF], int K, T C, int eos, T p0, T fh[NF]
         const T tau = C * fast_rcp(S), itau = S * invC;
 #pragma unroll
         for (int c = 0; c < NF; ++c) QM[c] = (T)0.5 * ((QL[c] + QR[c]) - tau * (FR[c] - FL[c]));
-        if (EOSRT) flux_only<T, DIR, true>(QM, FM, flag, eos, p0);
+        if (EOSRT) flux_only<T, DIR, true>(QM, FM, flag, eos);
         else {
             T unused;
             musta_flux<T, DIR, false>(QM, FM, unused, flag);
@@ -236,7 +240,7 @@ HD void musta_force_core(T QL[NF], T QR[NF], int K, T C, int eos, T p0, T fh[NF]
 // LIMS >= 0: the limiter is the compile-time constant LIMS and the closure the default one; LIMS < 0: run-time
 // limiter and closure.
 template <class T, int DIR, int KS, int LIMS, class Acc>
-HD void musta_force_stages(const Acc& acc, int K, T C, int lim, int eos, T p0, T fh[NF], int& flag) {
+HD void musta_force_stages(const Acc& acc, int K, T C, int lim, const EosArgs& eos, T fh[NF], int& flag) {
     constexpr bool EOSRT = LIMS < 0;
     T QL[NF], QR[NF];
 #pragma unroll
@@ -246,7 +250,7 @@ HD void musta_force_stages(const Acc& acc, int K, T C, int lim, int eos, T p0, T
         QL[c] = tfma((T)0.5, musta_slope<T, LIMS>(lim, dm, d0), u1);
         QR[c] = tfma((T)-0.5, musta_slope<T, LIMS>(lim, d0, dp), u2);
     }
-    musta_force_core<T, DIR, KS, EOSRT>(QL, QR, K, C, eos, p0, fh, flag);
+    musta_force_core<T, DIR, KS, EOSRT>(QL, QR, K, C, eos, fh, flag);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -358,9 +362,9 @@ HD void musta_force_fast4(const T QL0[NF], const T QR0[NF], T C, T invC, T fh4[N
 }
 
 template <class T, int DIR, class Acc>
-HD void musta_force_iface(const Acc& acc, int K, T C, int lim, int eos, T p0, T fh[NF], int& flag) {
-    if (K == 2 && lim == 0 && eos == 0) musta_force_stages<T, DIR, 2, 0>(acc, K, C, lim, eos, p0, fh, flag);
-    else musta_force_stages<T, DIR, 0, -1>(acc, K, C, lim, eos, p0, fh, flag);
+HD void musta_force_iface(const Acc& acc, int K, T C, int lim, const EosArgs& eos, T fh[NF], int& flag) {
+    if (K == 2 && lim == 0 && eos.kind == 0) musta_force_stages<T, DIR, 2, 0>(acc, K, C, lim, eos, fh, flag);
+    else musta_force_stages<T, DIR, 0, -1>(acc, K, C, lim, eos, fh, flag);
 }
 
 }  // namespace hydro

@@ -29,7 +29,7 @@ struct StageArgs {
     int musta_K;        // Q8
     double musta_C;     // Q7
     int limiter;        // MUSCL slope limiter: 0 minmod (Q6), 1 van Leer, 2 MC, 3 superbee
-    EosArgs eos;        // equation of state: kind 0 p = e/3 (Q2), 1 p = p0
+    EosArgs eos;        // equation of state: kind 0 p = e/3 (Q2), 1 p = p0, 2 tabulated p(e)
     int epi_max;        // z-sweep epilogue: also reduce the max signal speed of the new state (stage 3)
 };
 
@@ -40,7 +40,7 @@ __device__ __forceinline__ void iface_generic(const Geom& G, const StageArgs& A,
     const long long stride = DIR == 0 ? 1 : (DIR == 1 ? G.sx : G.sxy);
     constexpr int R = SCHEME == 0 ? 3 : (SCHEME == 1 ? 4 : 2);
     GlobalAcc<T> acc{U + p - (R - 1) * stride, W + p - (R - 1) * stride, G.fs, stride};
-    if constexpr (SCHEME == 2) musta_force_iface<T, DIR>(acc, A.musta_K, (T)A.musta_C, A.limiter, A.eos.kind, (T)A.eos.p0, fh, flag);
+    if constexpr (SCHEME == 2) musta_force_iface<T, DIR>(acc, A.musta_K, (T)A.musta_C, A.limiter, A.eos, fh, flag);
     else {
         llf_weno_iface2<T, R, DIR>(acc, (T)A.eps, fh);   // twice the flux
 #pragma unroll

@@ -85,8 +85,8 @@ __device__ __forceinline__ void musta_general4(const T QL[NF], const T QR[NF], c
         a[c] = QL[c];
         b[c] = QR[c];
     }
-    if (FAST) musta_force_core<T, DIR, 2, false>(a, b, 2, C, 0, (T)0, f4, flag);
-    else musta_force_core<T, DIR, 0, true>(a, b, A.musta_K, C, A.eos.kind, (T)A.eos.p0, f4, flag);
+    if (FAST) musta_force_core<T, DIR, 2, false>(a, b, 2, C, A.eos, f4, flag);
+    else musta_force_core<T, DIR, 0, true>(a, b, A.musta_K, C, A.eos, f4, flag);
 #pragma unroll
     for (int c = 0; c < NF; ++c) f4[c] *= (T)4;
 }

@@ -47,7 +47,7 @@ constexpr int WENO_THREADS = 32 * WENO_ROWS;
 // per cell and axis cost 120 B of DRAM traffic per cell and stage against ~50 fp64 instructions to make them again;
 // the kernels are bound by instruction issue AND run at the board's power cap, where the bytes cost more clock than
 // the flops).
-// EOS: the closure is a compile-time constant of the kernel (0: p = e/3, 1: p = p0): a run-time branch here costs
+// EOS: the closure is a compile-time constant of the kernel (0: p = e/3, 1: p = p0, 2: tabulated): a run-time branch here costs
 // ~90 register moves per cell where its two sides merge.
 template <class T, int NDIR, int EOS>
 __device__ __forceinline__ void cell_prims(const T u[NF], const EosArgs& eos, const int (&dirs)[NDIR], T v[NDIR],
@@ -59,6 +59,14 @@ __device__ __forceinline__ void cell_prims(const T u[NF], const EosArgs& eos, co
         for (int d = 0; d < NDIR; ++d) {
             v[d] = u[1 + dirs[d]] * winv;
             a[d] = tabs(v[d]);
+        }
+    } else if (EOS == 2) {
+        T cs2;
+        con2prim_tab(u[0], u[1], u[2], u[3], eos, winv, p, v2, cs2, flag);
+#pragma unroll
+        for (int d = 0; d < NDIR; ++d) {
+            v[d] = u[1 + dirs[d]] * winv;
+            a[d] = signal_speed_cs(v[d], v2, cs2);
         }
     } else {
         con2prim(u[0], u[1], u[2], u[3], winv, p, v2, flag);
@@ -405,7 +413,7 @@ weno_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl, 
         issue(j + D);             // refill the slot just consumed
         if (EPI) {   // stage 3 of a CFL step: a4 of the finished cell (all three axes are active here)
             T w[NW];
-            prim_of_cell_t<T, EOS>(o, w, flag, (T)A.eos.p0);
+            prim_of_cell_t<T, EOS>(o, w, flag, A.eos);
             amax = fmax(amax, fmax((double)w[W_AX], fmax((double)w[W_AX + 1], (double)w[W_AX + 2])));
         }
     }
@@ -423,6 +431,9 @@ int configure_weno(char* err, size_t errlen) {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(weno_y_kernel<T, R, true, 0>, attr, sy);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(weno_y_kernel<T, R, false, 1>, attr, sy);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(weno_y_kernel<T, R, true, 1>, attr, sy);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(weno_xz_kernel<T, R, 2>, attr, sxz);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(weno_y_kernel<T, R, false, 2>, attr, sy);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(weno_y_kernel<T, R, true, 2>, attr, sy);
     if (e != cudaSuccess) {
         snprintf(err, errlen, "cudaFuncSetAttribute (weno): %s", cudaGetErrorString(e));
         return -1;
@@ -448,6 +459,7 @@ template <class T, int R>
 int launch_weno(const Geom& G, const StageArgs& A, const T* Us, const T* Un, T* Uout, Ctl* ctl, int zc, int yc,
                 cudaStream_t st, int* launches, char* err, size_t errlen) {
     if (A.eos.kind == 1) launch_weno_eos<T, R, 1>(G, A, Us, Un, Uout, ctl, zc, yc, st);
+    else if (A.eos.kind == 2) launch_weno_eos<T, R, 2>(G, A, Us, Un, Uout, ctl, zc, yc, st);
     else launch_weno_eos<T, R, 0>(G, A, Us, Un, Uout, ctl, zc, yc, st);
     *launches = 2;
     const cudaError_t e = cudaGetLastError();

@@ -37,31 +37,32 @@ __global__ void end_step_kernel(Ctl* ctl) {
 __global__ void reset_max_kernel(Ctl* ctl) { ctl->maxspeed_bits = 0ull; }
 
 // W = (v_x, v_y, v_z, p, a_x, a_y, a_z) of one cell from its conserved values (a2-a3).  EOS 0: p = e/3; EOS 1:
-// p = p0, whose characteristic speeds are all v_d, so a_d = |v_d|.
+// p = p0, whose characteristic speeds are all v_d, so a_d = |v_d|; EOS 2: the tabulated closure.
 template <class T, int EOS>
-__device__ __forceinline__ void prim_of_cell_t(const T u[NF], T w[NW], int& flag, T p0) {
-    T v2, winv;
-    if (EOS == 1) con2prim_p0(u[0], u[1], u[2], u[3], p0, winv, w[W_P], v2, flag);
+__device__ __forceinline__ void prim_of_cell_t(const T u[NF], T w[NW], int& flag, const EosArgs& eos) {
+    T v2, winv, cs2;
+    if (EOS == 1) con2prim_p0(u[0], u[1], u[2], u[3], (T)eos.p0, winv, w[W_P], v2, flag);
+    else if (EOS == 2) con2prim_tab(u[0], u[1], u[2], u[3], eos, winv, w[W_P], v2, cs2, flag);
     else con2prim(u[0], u[1], u[2], u[3], winv, w[W_P], v2, flag);
 #pragma unroll
     for (int d = 0; d < 3; ++d) w[W_V + d] = u[1 + d] * winv;
     if (EOS == 1) {
 #pragma unroll
         for (int d = 0; d < 3; ++d) w[W_AX + d] = tabs(w[W_V + d]);
+    } else if (EOS == 2) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) w[W_AX + d] = signal_speed_cs(w[W_V + d], v2, cs2);
     } else {
         const T id = speed_inv_den(v2);
 #pragma unroll
         for (int d = 0; d < 3; ++d) w[W_AX + d] = signal_speed(w[W_V + d], v2, id);
     }
 }
-struct EosArgs {
-    int kind;     // 0: p = e/3, 1: p = p0
-    double p0;
-};
 template <class T>
 __device__ __forceinline__ void prim_of_cell(const T u[NF], T w[NW], int& flag, const EosArgs& eos) {
-    if (eos.kind == 1) prim_of_cell_t<T, 1>(u, w, flag, (T)eos.p0);
-    else prim_of_cell_t<T, 0>(u, w, flag, (T)0);
+    if (eos.kind == 1) prim_of_cell_t<T, 1>(u, w, flag, eos);
+    else if (eos.kind == 2) prim_of_cell_t<T, 2>(u, w, flag, eos);
+    else prim_of_cell_t<T, 0>(u, w, flag, eos);
 }
 
 // ------------------------------------------------------------------------------------------------

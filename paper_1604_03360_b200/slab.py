@@ -136,6 +136,8 @@ def make_slab(binding, w, k0, k1, precision=0, device="cuda"):
     h.set_option("bc_z", binding.BC_EXTERNAL)
     for k, v in w.options.items():
         h.set_option(k, v)
+    if getattr(w, "eos_table", None) is not None:
+        h.set_eos_table(*w.eos_table)
     h.set_option("t", w.t0)
     h.bind()
     h.set_state(torch.from_numpy(np.ascontiguousarray(w.cons[:, k0:k1])).to(device=device, dtype=h.dtype).contiguous())

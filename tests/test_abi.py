@@ -67,7 +67,12 @@ def test_workspace_size_follows_the_padded_layout(L, scheme, g):
         sx = -(-(n[0] + 2 * g) // (16 // es)) * (16 // es)
         vol = sx * (n[1] + 2 * g) * (n[2] + 2 * g)
         fs = -(-vol // (256 // es)) * (256 // es)
-        assert L.hydro_workspace_bytes(h) == 256 + (3 * 5 + 2 * 7) * fs * es   # three states, two primitive sets
+        # three states: the marching kernels keep no primitive arrays ...
+        assert L.hydro_set_option(h, b"kernel", 0.0) == 0
+        assert L.hydro_workspace_bytes(h) == 256 + 3 * 5 * fs * es
+        # ... the generic kernel keeps one set of seven
+        assert L.hydro_set_option(h, b"kernel", 1.0) == 0
+        assert L.hydro_workspace_bytes(h) == 256 + (3 * 5 + 7) * fs * es
     L.hydro_destroy(h)
 
 

@@ -167,3 +167,65 @@ def test_bench_variants_at_512_on_sampled_cells(B, oracle, scheme, prec):
         assert abs(a - b) <= (1e-11 if prec == 0 else 2e-6) * abs(tot0[0]), (tot0, tot1)
     del ug_t
     h.close()
+
+
+# ------------------------------------------------------------------ tabulated equation of state (N1, second half)
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("kernel", ["fused", "generic"])
+def test_tabulated_eos_matches_the_oracle(B, oracle, scheme, kernel):
+    """The crossover table p(e) (c_s^2 from 0.15 to 1/3): L(u), one step and ten steps against the oracle on a ragged
+    grid through the marching kernels and the generic kernel; and with the linear p = e/3 table the result must be the
+    closed-form gas's."""
+    n = (45, 23, 38)
+    w0 = small_workload(scheme, n)
+    tab = W.crossover_eos_table(n=2048, e_max=float(np.max(w0.cons[0])) * 1.5)
+    w = W.Workload("xover", n, w0.dx, (0, 0, 0), scheme, (W.BC_PERIODIC, W.BC_OUTFLOW, W.BC_PERIODIC), w0.cons, 0.0,
+                   cfl=0.2, nsteps=10, eos_table=tab)
+    kern = B.KERNEL_FUSED if kernel == "fused" else B.KERNEL_GENERIC
+    o = oracle.from_workload(w)
+    h = B.from_workload(w, kernel=kern)
+    scale = np.max(np.abs(w.cons[0])) / w.dx
+    Lo = o.eval_L(w.cons)
+    Lg = h.eval_L(to_dev(B, w.cons)).cpu().numpy()
+    assert reldiff(Lg, Lo, scale=scale) <= TOL_STAGE
+    assert abs(h.max_signal_speed() - o.max_signal_speed()) <= 1e-14
+    dts = oracle.run(o, w)
+    o1 = oracle.from_workload(w)
+    o1.step(dts[0], 1)
+    h.step(dts[0], 1)
+    assert reldiff(h.get_state().cpu().numpy(), o1.get_state()) <= 3 * TOL_STAGE
+    for dt in dts[1:]:
+        h.step(dt, 1)
+    assert reldiff(h.get_state().cpu().numpy(), o.get_state()) <= 1e-11
+    assert h.status() == 0
+    h.close()
+    # it is not the gas: the operator differs
+    og = oracle.from_workload(w0)
+    assert np.max(np.abs(og.eval_L(w0.cons) - Lo)) > 1e-3 * scale
+    # the linear table is the gas
+    wl = W.Workload("lin", n, w0.dx, (0, 0, 0), scheme, (W.BC_PERIODIC,) * 3, w0.cons, 0.0,
+                    eos_table=(np.linspace(0.0, 80.0, 401) / 3.0, 0.0, 80.0))
+    wg = W.Workload("gas", n, w0.dx, (0, 0, 0), scheme, (W.BC_PERIODIC,) * 3, w0.cons, 0.0)
+    hl, hg = B.from_workload(wl, kernel=kern), B.from_workload(wg, kernel=kern)
+    Ll = hl.eval_L(to_dev(B, w0.cons)).cpu().numpy()
+    Lgas = hg.eval_L(to_dev(B, w0.cons)).cpu().numpy()
+    assert reldiff(Ll, Lgas, scale=scale) <= TOL_STAGE
+    hl.close()
+    hg.close()
+
+
+def test_eos_table_arguments_are_checked(B):
+    import torch
+    h = B.Hydro(16, 16, 16, 0.1, W.WENO5)
+    with pytest.raises(B.HydroError):
+        h.set_option("eos", 2)                                   # no table yet
+    t = torch.linspace(0, 10, 11, dtype=torch.float64, device="cuda")
+    assert B.lib.hydro_set_eos_table(h._h, t.data_ptr(), 1, 0.0, 1.0) == B.EINVAL
+    assert B.lib.hydro_set_eos_table(h._h, t.data_ptr(), 11, 1.0, 1.0) == B.EINVAL
+    assert B.lib.hydro_set_eos_table(h._h, None, 11, 0.0, 1.0) == B.EINVAL
+    host = np.zeros(11)
+    assert B.lib.hydro_set_eos_table(h._h, host.ctypes.data, 11, 0.0, 1.0) == B.EINVAL
+    assert B.lib.hydro_set_eos_table(h._h, t.data_ptr(), 11, 0.0, 30.0) == B.OK
+    h.set_option("eos", 0)
+    h.set_option("eos", 2)
+    h.close()
