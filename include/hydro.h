@@ -188,6 +188,17 @@ int hydro_step_stage(hydro_ctx *ctx, double dt, int stage);
 int hydro_local_max_speed(hydro_ctx *ctx, void *maxspeed_device_out);
 int hydro_step_stage_cfl(hydro_ctx *ctx, double cfl, int stage, const void *maxspeed_device);
 
+/* One stage with the halo exchange hidden behind the interior ("fully hidden by computing the boundary
+ * planes first" -- here the INTERIOR planes first, while the planes travel).  On the context's stream: x/y ghost fill,
+ * the x/z kernel over the planes whose z stencils stay inside the slab, cudaStreamWaitEvent(ready_event) (a
+ * cudaEvent_t the caller records on its communication stream once the neighbours' planes have arrived; NULL: no
+ * wait), the ghost planes written from the packed DEVICE buffers ghosts_lo / ghosts_hi (layout of hydro_get_zhalo;
+ * NULL: zero-gradient copies of the slab's own boundary plane), the x/z kernel over the g..8 outermost planes on
+ * each side, the y sweep.  Results are bit-identical to hydro_put_zhalo x 2 + hydro_step_stage_cfl.  The packed
+ * buffers must stay untouched until the stream has passed this call.  EINVAL unless bc_z = HYDRO_BC_EXTERNAL. */
+int hydro_step_stage_overlap(hydro_ctx *ctx, double cfl, int stage, const void *maxspeed_device,
+                             const void *ghosts_lo_device, const void *ghosts_hi_device, void *ready_event);
+
 /* With the "profile" option on: total device time in milliseconds of the stage kernels (the L(u) +
  * Runge-Kutta kernel, the dominant one) launched since the last call, and their number, written to HOST
  * pointers.  Synchronises the stream and clears the record. */

@@ -26,7 +26,7 @@ SYMBOLS = [
     "hydro_step_cfl", "hydro_step_cfl_batch", "hydro_set_eos_table", "hydro_max_signal_speed", "hydro_eval_L", "hydro_get_time", "hydro_status",
     "hydro_launch_count", "hydro_stage_kernel_time", "hydro_last_error",
     "hydro_zhalo_elems", "hydro_get_zhalo", "hydro_put_zhalo", "hydro_step_stage", "hydro_local_max_speed",
-    "hydro_step_stage_cfl", "hydro_destroy",
+    "hydro_step_stage_cfl", "hydro_step_stage_overlap", "hydro_destroy",
 ]
 
 
@@ -71,6 +71,7 @@ def _load():
     L.hydro_step_stage.argtypes = [vp, dbl, i32]
     L.hydro_local_max_speed.argtypes = [vp, vp]
     L.hydro_step_stage_cfl.argtypes = [vp, dbl, i32, vp]
+    L.hydro_step_stage_overlap.argtypes = [vp, dbl, i32, vp, vp, vp, vp]
     L.hydro_last_error.argtypes = [vp]
     L.hydro_last_error.restype = ctypes.c_char_p
     L.hydro_destroy.argtypes = [vp]
@@ -214,6 +215,17 @@ class Hydro:
 
     def step_stage(self, dt, stage):
         self._check(lib.hydro_step_stage(self._h, float(dt), int(stage)))
+
+    def step_stage_overlap(self, cfl, stage, maxspeed, ghosts_lo, ghosts_hi, ready_event=None):
+        """hydro_step_stage_overlap; ghosts_* = packed device tensors or None (zero-gradient); ready_event = a
+        torch.cuda.Event recorded on the communication stream, or None."""
+        assert maxspeed.is_cuda and maxspeed.dtype == torch.float64 and maxspeed.numel() == 1
+        for t in (ghosts_lo, ghosts_hi):
+            assert t is None or (t.is_cuda and t.is_contiguous() and t.dtype == self.dtype and t.numel() == self.zhalo_elems())
+        ev = None if ready_event is None else ctypes.c_void_p(ready_event.cuda_event)
+        self._check(lib.hydro_step_stage_overlap(self._h, float(cfl), int(stage), maxspeed.data_ptr(),
+                                                 None if ghosts_lo is None else ghosts_lo.data_ptr(),
+                                                 None if ghosts_hi is None else ghosts_hi.data_ptr(), ev))
 
     def stage_kernel_time(self):
         """(total ms, launches) of the stage kernels since the last call ("profile" option)."""

@@ -201,6 +201,8 @@ StageArgs stage_args(const hydro_ctx* c, double ca, double cb, int mode) {
     A.limiter = c->limiter;
     A.eos = c->eos;
     A.epi_max = 0;
+    A.kbeg = 0;
+    A.kend = c->G.n[2];
     return A;
 }
 
@@ -238,23 +240,27 @@ struct StageTimer {
 };
 
 // One stage: Uout = ca u^n + cb (Us + dt L(Us)), or L(Us) itself (mode 1).
+// parts / kbeg / kend (marching kernels only): bit 0 the x/z kernel over the planes [kbeg, kend), bit 1 the y sweep.
 template <class T>
-int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double cb, int mode, int epi_max = 0) {
+int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double cb, int mode, int epi_max = 0,
+             int parts = 3, int kbeg = 0, int kend = -1) {
     StageArgs A = stage_args(c, ca, cb, mode);
     A.epi_max = epi_max;
+    A.kbeg = kbeg;
+    A.kend = kend < 0 ? c->G.n[2] : kend;
     StageTimer timer(c);
     if (want_fused(c)) {
         if (!c->fused_ready) return fail(c, HYDRO_ECUDA, "marching kernels not configured: %s", c->plan_err);
         int nl = 0, rc;
         if (c->scheme == HYDRO_MUSTA_FORCE)
             rc = launch_musta<T>(c->G, A, Us, Un, Uout, c->ctl, c->zc > 0 ? c->zc : 64, c->yc > 0 ? c->yc : 128,
-                                 c->stream, &nl, c->plan_err, sizeof c->plan_err);
+                                 c->stream, parts, &nl, c->plan_err, sizeof c->plan_err);
         else if (c->scheme == HYDRO_WENO5)
             rc = launch_weno<T, 3>(c->G, A, Us, Un, Uout, c->ctl, c->zc > 0 ? c->zc : WENO_ZC,
-                                   c->yc > 0 ? c->yc : WENO_YC, c->stream, &nl, c->plan_err, sizeof c->plan_err);
+                                   c->yc > 0 ? c->yc : WENO_YC, c->stream, parts, &nl, c->plan_err, sizeof c->plan_err);
         else
             rc = launch_weno<T, 4>(c->G, A, Us, Un, Uout, c->ctl, c->zc > 0 ? c->zc : WENO_ZC,
-                                   c->yc > 0 ? c->yc : WENO_YC, c->stream, &nl, c->plan_err, sizeof c->plan_err);
+                                   c->yc > 0 ? c->yc : WENO_YC, c->stream, parts, &nl, c->plan_err, sizeof c->plan_err);
         if (rc != 0) return fail(c, HYDRO_ECUDA, "stage launch: %s", c->plan_err);
         c->launches += nl;
         return HYDRO_OK;
@@ -278,8 +284,22 @@ int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double 
 // The marching kernels make con2prim + signal speeds (a2-a3) of every cell as it enters a stencil window, and stage 3
 // reduces the max signal speed of the new state (a4): the max-speed pass runs as a separate kernel only for the
 // first CFL step after hydro_set_state / hydro_eval_L.  Only the generic kernel reads primitive arrays (prim_kernel).
+// z-halo planes of a slab (defined below)
+int zhalo_impl(hydro_ctx* c, int buffer, int side, void* packed, int put);
+
+// Overlap (slab decomposition): the planes whose z stencils stay inside the slab are launched
+// first; the stream then waits for the caller's event (the neighbours' planes have arrived), the ghost planes are
+// written, and the two boundary chunks and the y sweep follow.
+struct Overlap {
+    bool on = false;
+    const void* lo = nullptr;   // packed ghost planes below / above (null: zero-gradient from the slab's own plane)
+    const void* hi = nullptr;
+    cudaEvent_t ready = nullptr;
+};
+
 template <class T>
-int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl, const double* ext_max = nullptr) {
+int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl, const double* ext_max = nullptr,
+                  const Overlap& ov = Overlap()) {
     T* U[3] = {(T*)c->U[0], (T*)c->U[1], (T*)c->U[2]};
     const bool weno = c->scheme != HYDRO_MUSTA_FORCE;
     const bool cflmode = !(dt_fixed > 0.0);
@@ -306,7 +326,27 @@ int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl, const double
         LAUNCHED(c, "begin_step_kernel");
         c->max_ready = false;
     }
-    if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, (marching && s == 2) ? 1 : 0))) return rc;
+    const int epi = (marching && s == 2) ? 1 : 0;
+    if (ov.on && marching) {
+        const int nz = c->G.n[2], g = c->G.g[2];
+        const int b = nz >= 4 * g ? (g > 8 ? g : 8) < nz / 2 ? (g > 8 ? g : 8) : g : 0;   // planes per boundary chunk
+        if (b > 0 && (rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, epi, 1, b, nz - b))) return rc;
+        if (ov.ready != nullptr) CUDA_OK(c, cudaStreamWaitEvent(c->stream, ov.ready, 0));
+        if ((rc = zhalo_impl(c, s, 0, const_cast<void*>(ov.lo), ov.lo ? 1 : 2))) return rc;
+        if ((rc = zhalo_impl(c, s, 1, const_cast<void*>(ov.hi), ov.hi ? 1 : 2))) return rc;
+        if (b > 0) {
+            if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, epi, 1, 0, b))) return rc;
+            if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, epi, 1, nz - b, nz))) return rc;
+            if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, epi, 2))) return rc;
+        } else if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, epi))) return rc;
+    } else {
+        if (ov.on) {   // generic kernel: no split, the ghosts first
+            if (ov.ready != nullptr) CUDA_OK(c, cudaStreamWaitEvent(c->stream, ov.ready, 0));
+            if ((rc = zhalo_impl(c, s, 0, const_cast<void*>(ov.lo), ov.lo ? 1 : 2))) return rc;
+            if ((rc = zhalo_impl(c, s, 1, const_cast<void*>(ov.hi), ov.hi ? 1 : 2))) return rc;
+        }
+        if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, epi))) return rc;
+    }
     if (s == 2) {
         end_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
         LAUNCHED(c, "end_step_kernel");
@@ -734,7 +774,9 @@ size_t hydro_zhalo_elems(const hydro_ctx* c) {
     return (size_t)NF * c->G.g[2] * c->G.n[1] * c->G.n[0];
 }
 
-static int zhalo_impl(hydro_ctx* c, int buffer, int side, void* packed, int put) {
+}  // extern "C"
+namespace {
+int zhalo_impl(hydro_ctx* c, int buffer, int side, void* packed, int put) {
     int rc = need_ws(c);
     if (rc) return rc;
     DeviceGuard dg(c);
@@ -748,6 +790,8 @@ static int zhalo_impl(hydro_ctx* c, int buffer, int side, void* packed, int put)
     LAUNCHED(c, "zhalo_kernel");
     return HYDRO_OK;
 }
+}  // namespace
+extern "C" {
 int hydro_get_zhalo(hydro_ctx* c, int buffer, int side, void* packed_out) { return zhalo_impl(c, buffer, side, packed_out, 0); }
 int hydro_put_zhalo(hydro_ctx* c, int buffer, int side, const void* packed_in) {
     return zhalo_impl(c, buffer, side, const_cast<void*>(packed_in), packed_in ? 1 : 2);
@@ -771,6 +815,26 @@ int hydro_step_stage_cfl(hydro_ctx* c, double cfl, int stage, const void* maxspe
     if (stage != c->stage_open) return fail(c, HYDRO_EINVAL, "hydro_step_stage_cfl: stage %d out of order (expected %d)", stage, c->stage_open);
     const double* m = (const double*)maxspeed_dev;
     return c->precision == HYDRO_F64 ? do_step_stage<double>(c, stage, -1.0, cfl, m) : do_step_stage<float>(c, stage, -1.0, cfl, m);
+}
+
+int hydro_step_stage_overlap(hydro_ctx* c, double cfl, int stage, const void* maxspeed_dev, const void* ghosts_lo_dev,
+                             const void* ghosts_hi_dev, void* ready_event) {
+    int rc = need_ws(c);
+    if (rc) return rc;
+    DeviceGuard dg(c);
+    if (!(cfl > 0) || stage < 0 || stage > 2 || !maxspeed_dev)
+        return fail(c, HYDRO_EINVAL, "hydro_step_stage_overlap: cfl <= 0, stage not in 0..2 or null pointer");
+    if (c->bc[2] != HYDRO_BC_EXTERNAL || c->G.g[2] == 0)
+        return fail(c, HYDRO_EINVAL, "hydro_step_stage_overlap needs bc_z = HYDRO_BC_EXTERNAL on an active z axis");
+    if (stage != c->stage_open) return fail(c, HYDRO_EINVAL, "hydro_step_stage_overlap: stage %d out of order (expected %d)", stage, c->stage_open);
+    Overlap ov;
+    ov.on = true;
+    ov.lo = ghosts_lo_dev;
+    ov.hi = ghosts_hi_dev;
+    ov.ready = (cudaEvent_t)ready_event;
+    const double* m = (const double*)maxspeed_dev;
+    return c->precision == HYDRO_F64 ? do_step_stage<double>(c, stage, -1.0, cfl, m, ov)
+                                     : do_step_stage<float>(c, stage, -1.0, cfl, m, ov);
 }
 
 int hydro_local_max_speed(hydro_ctx* c, void* maxspeed_dev_out) {

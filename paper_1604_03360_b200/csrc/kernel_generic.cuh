@@ -31,6 +31,8 @@ struct StageArgs {
     int limiter;        // MUSCL slope limiter: 0 minmod (Q6), 1 van Leer, 2 MC, 3 superbee
     EosArgs eos;        // equation of state: kind 0 p = e/3 (Q2), 1 p = p0, 2 tabulated p(e)
     int epi_max;        // z-sweep epilogue: also reduce the max signal speed of the new state (stage 3)
+    int kbeg, kend;     // marching x/z kernels: the planes [kbeg, kend) this launch covers (the whole grid by default;
+                        // the slab path launches the planes that need no z ghost first)
 };
 
 // flux at interface (cell p) + 1/2 along DIR; p = padded index of the cell on the low side

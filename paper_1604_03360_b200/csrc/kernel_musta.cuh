@@ -132,8 +132,8 @@ musta_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* Un, T* U
     const int il = min(i, imax);                           // column this lane loads (idle lanes: clamped)
     const int hcell = lane < R - 1 ? i0 - (R - 1) + lane : i0 + 32 + (lane - (R - 1));   // halo lanes' column
     const int hq = lane < R - 1 ? lane : 32 + lane;        // and its position in the row
-    const int k0 = (int)blockIdx.z * zc;
-    const int k1 = min(k0 + zc, G.n[2]);
+    const int k0 = A.kbeg + (int)blockIdx.z * zc;
+    const int k1 = min(k0 + zc, A.kend);
     const long long p0 = G.pidx(il, j, k0);
     const long long ph = G.pidx(min(hcell, imax), j, k0);
     const bool use_un = A.mode != 1 && A.ca != 0.0;
@@ -427,25 +427,32 @@ int configure_musta(char* err, size_t errlen) {
     return 0;
 }
 
-// stage = x/z kernel (writes Uout) + y sweep (adds L_y; stage 3 of a CFL step: the max signal speed of the new state)
+// stage = x/z kernel over the planes [A.kbeg, A.kend) (writes Uout) + y sweep (adds L_y; stage 3 of a CFL step: the
+// max signal speed of the new state).  parts: bit 0 the x/z kernel, bit 1 the y sweep.
 template <class T>
 int launch_musta(const Geom& G, const StageArgs& A, const T* Us, const T* Un, T* Uout, Ctl* ctl, int zc, int yc,
-                 cudaStream_t st, int* launches, char* err, size_t errlen) {
+                 cudaStream_t st, int parts, int* launches, char* err, size_t errlen) {
     const dim3 b(32, MUSTA_ROWS, 1);
-    const dim3 g((G.n[0] + 30) / 31, (G.n[1] + MUSTA_ROWS - 1) / MUSTA_ROWS, (G.n[2] + zc - 1) / zc);
-    const dim3 gy((G.n[0] + 31) / 32, (G.n[2] + MUSTA_ROWS - 1) / MUSTA_ROWS, (G.n[1] + yc - 1) / yc);
     const size_t sxz = MustaXZShape<T>::smem_bytes(), sy = musta_y_smem_bytes<T>();
     const bool epi = A.epi_max && A.mode != 1;
-    if (musta_fast(A)) {
-        musta_xz_kernel<T, true><<<g, b, sxz, st>>>(G, A, Us, Un, Uout, ctl, zc);
-        if (epi) musta_y_kernel<T, true, true><<<gy, b, sy, st>>>(G, A, Us, Uout, ctl, yc);
-        else musta_y_kernel<T, false, true><<<gy, b, sy, st>>>(G, A, Us, Uout, ctl, yc);
-    } else {
-        musta_xz_kernel<T, false><<<g, b, sxz, st>>>(G, A, Us, Un, Uout, ctl, zc);
-        if (epi) musta_y_kernel<T, true, false><<<gy, b, sy, st>>>(G, A, Us, Uout, ctl, yc);
-        else musta_y_kernel<T, false, false><<<gy, b, sy, st>>>(G, A, Us, Uout, ctl, yc);
+    *launches = 0;
+    if ((parts & 1) && A.kend > A.kbeg) {
+        const dim3 g((G.n[0] + 30) / 31, (G.n[1] + MUSTA_ROWS - 1) / MUSTA_ROWS, (A.kend - A.kbeg + zc - 1) / zc);
+        if (musta_fast(A)) musta_xz_kernel<T, true><<<g, b, sxz, st>>>(G, A, Us, Un, Uout, ctl, zc);
+        else musta_xz_kernel<T, false><<<g, b, sxz, st>>>(G, A, Us, Un, Uout, ctl, zc);
+        ++*launches;
     }
-    *launches = 2;
+    if (parts & 2) {
+        const dim3 gy((G.n[0] + 31) / 32, (G.n[2] + MUSTA_ROWS - 1) / MUSTA_ROWS, (G.n[1] + yc - 1) / yc);
+        if (musta_fast(A)) {
+            if (epi) musta_y_kernel<T, true, true><<<gy, b, sy, st>>>(G, A, Us, Uout, ctl, yc);
+            else musta_y_kernel<T, false, true><<<gy, b, sy, st>>>(G, A, Us, Uout, ctl, yc);
+        } else {
+            if (epi) musta_y_kernel<T, true, false><<<gy, b, sy, st>>>(G, A, Us, Uout, ctl, yc);
+            else musta_y_kernel<T, false, false><<<gy, b, sy, st>>>(G, A, Us, Uout, ctl, yc);
+        }
+        ++*launches;
+    }
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) {
         snprintf(err, errlen, "%s", cudaGetErrorString(e));

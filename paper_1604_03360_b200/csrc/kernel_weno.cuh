@@ -176,8 +176,8 @@ weno_xz_kernel(Geom G, StageArgs A, const T* __restrict__ Us, const T* Un, T* Uo
     const int il = min(i, imax);                           // column this lane loads (idle lanes: clamped)
     const int hcell = lane < R - 1 ? i0 - (R - 1) + lane : i0 + 32 + (lane - (R - 1));   // halo lanes' column
     const int hq = lane < R - 1 ? lane : 32 + lane;        // and its position in the row
-    const int k0 = (int)blockIdx.z * zc;
-    const int k1 = min(k0 + zc, G.n[2]);
+    const int k0 = A.kbeg + (int)blockIdx.z * zc;
+    const int k1 = min(k0 + zc, A.kend);
     const long long p0 = G.pidx(il, j, k0);
     const long long ph = G.pidx(min(hcell, imax), j, k0);
     const bool use_un = A.mode != 1 && A.ca != 0.0;
@@ -441,27 +441,34 @@ int configure_weno(char* err, size_t errlen) {
     return 0;
 }
 
-// stage = x/z kernel (writes Uout) + y sweep (adds L_y; stage 3 of a CFL step: the max signal speed of the new state)
+// stage = x/z kernel over the planes [A.kbeg, A.kend) (writes Uout) + y sweep (adds L_y; stage 3 of a CFL step: the
+// max signal speed of the new state).  parts: bit 0 the x/z kernel, bit 1 the y sweep.
 template <class T, int R, int EOS>
 void launch_weno_eos(const Geom& G, const StageArgs& A, const T* Us, const T* Un, T* Uout, Ctl* ctl, int zc, int yc,
-                     cudaStream_t st) {
+                     cudaStream_t st, int parts, int* launches) {
     const dim3 b(32, WENO_ROWS, 1);
-    const dim3 g((G.n[0] + 30) / 31, (G.n[1] + WENO_ROWS - 1) / WENO_ROWS, (G.n[2] + zc - 1) / zc);
-    weno_xz_kernel<T, R, EOS><<<g, b, WenoXZShape<T, R>::smem_bytes(), st>>>(G, A, Us, Un, Uout, ctl, zc);
-    const dim3 gy((G.n[0] + 31) / 32, (G.n[2] + WENO_ROWS - 1) / WENO_ROWS, (G.n[1] + yc - 1) / yc);
-    if (A.epi_max && A.mode != 1)
-        weno_y_kernel<T, R, true, EOS><<<gy, b, weno_y_smem_bytes<T, R>(), st>>>(G, A, Us, Uout, ctl, yc);
-    else
-        weno_y_kernel<T, R, false, EOS><<<gy, b, weno_y_smem_bytes<T, R>(), st>>>(G, A, Us, Uout, ctl, yc);
+    if ((parts & 1) && A.kend > A.kbeg) {
+        const dim3 g((G.n[0] + 30) / 31, (G.n[1] + WENO_ROWS - 1) / WENO_ROWS, (A.kend - A.kbeg + zc - 1) / zc);
+        weno_xz_kernel<T, R, EOS><<<g, b, WenoXZShape<T, R>::smem_bytes(), st>>>(G, A, Us, Un, Uout, ctl, zc);
+        ++*launches;
+    }
+    if (parts & 2) {
+        const dim3 gy((G.n[0] + 31) / 32, (G.n[2] + WENO_ROWS - 1) / WENO_ROWS, (G.n[1] + yc - 1) / yc);
+        if (A.epi_max && A.mode != 1)
+            weno_y_kernel<T, R, true, EOS><<<gy, b, weno_y_smem_bytes<T, R>(), st>>>(G, A, Us, Uout, ctl, yc);
+        else
+            weno_y_kernel<T, R, false, EOS><<<gy, b, weno_y_smem_bytes<T, R>(), st>>>(G, A, Us, Uout, ctl, yc);
+        ++*launches;
+    }
 }
 
 template <class T, int R>
 int launch_weno(const Geom& G, const StageArgs& A, const T* Us, const T* Un, T* Uout, Ctl* ctl, int zc, int yc,
-                cudaStream_t st, int* launches, char* err, size_t errlen) {
-    if (A.eos.kind == 1) launch_weno_eos<T, R, 1>(G, A, Us, Un, Uout, ctl, zc, yc, st);
-    else if (A.eos.kind == 2) launch_weno_eos<T, R, 2>(G, A, Us, Un, Uout, ctl, zc, yc, st);
-    else launch_weno_eos<T, R, 0>(G, A, Us, Un, Uout, ctl, zc, yc, st);
-    *launches = 2;
+                cudaStream_t st, int parts, int* launches, char* err, size_t errlen) {
+    *launches = 0;
+    if (A.eos.kind == 1) launch_weno_eos<T, R, 1>(G, A, Us, Un, Uout, ctl, zc, yc, st, parts, launches);
+    else if (A.eos.kind == 2) launch_weno_eos<T, R, 2>(G, A, Us, Un, Uout, ctl, zc, yc, st, parts, launches);
+    else launch_weno_eos<T, R, 0>(G, A, Us, Un, Uout, ctl, zc, yc, st, parts, launches);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) {
         snprintf(err, errlen, "%s", cudaGetErrorString(e));

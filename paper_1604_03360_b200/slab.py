@@ -71,6 +71,29 @@ class DistComm:
             req.wait()
         return [(recv_lo, recv_hi)]
 
+    def exchange_async(self, pairs):
+        """The same exchange issued on a side stream (CUDA tensors), so that the caller's stream is free to compute
+        while the planes travel: returns (ghosts, event) with the event recorded on the side stream behind the
+        receives; hydro_step_stage_overlap makes the compute stream wait for it only where the ghosts are needed.
+        CPU tensors (gloo): a plain exchange, event None."""
+        (send_lo, send_hi), = pairs
+        if not send_lo.is_cuda:
+            return self.exchange(pairs), None
+        cur = torch.cuda.current_stream(send_lo.device)
+        if getattr(self, "side", None) is None:
+            self.side = torch.cuda.Stream(send_lo.device)
+        self.side.wait_stream(cur)                       # the packing kernels have run
+        with torch.cuda.stream(self.side):
+            got = self.exchange(pairs)
+            ready = torch.cuda.Event()
+            ready.record(self.side)
+        for t in (send_lo, send_hi):
+            t.record_stream(self.side)                   # allocator: these buffers are in use on the side stream
+        for t in got[0]:
+            if t is not None:
+                t.record_stream(cur)
+        return got, ready
+
     def max(self, values):
         """values = [one 1-element float64 tensor] (this rank's slab): all-reduced in place with MAX over the ranks,
         on the tensor's device (NCCL on the GPU, gloo on the CPU); nothing comes to the host."""
@@ -92,6 +115,9 @@ class LocalComm:
             lo, hi = neighbours(r, self.n, self.bc_z)
             out.append((pairs[lo][1] if lo is not None else None, pairs[hi][0] if hi is not None else None))
         return out
+
+    def exchange_async(self, pairs):
+        return self.exchange(pairs), None
 
     def max(self, values):
         """Element-wise maximum of the slabs' 1-element tensors (what the all-reduce does between ranks)."""
@@ -116,15 +142,23 @@ class SlabGroup:
             x.put_zhalo(buffer, 0, below)      # None at a physical end: the library's zero-gradient rule
             x.put_zhalo(buffer, 1, above)
 
-    def step_cfl(self, cfl, nsteps=1):
-        """Per step: the slabs' max signal speeds are max-reduced on the device, then three stages, each after a
-        halo exchange; dt = cfl dx / max is taken inside the library (hydro_step_stage_cfl).  No host sync."""
+    def step_cfl(self, cfl, nsteps=1, overlap=True):
+        """Per step: the slabs' max signal speeds are max-reduced on the device, then three stages, each with a halo
+        exchange; dt = cfl dx / max is taken inside the library.  No host sync.
+        overlap: the exchange runs on a side stream while hydro_step_stage_overlap computes the planes that need no
+        ghost; otherwise exchange -> hydro_put_zhalo -> hydro_step_stage_cfl one after the other.  Same results."""
         for _ in range(nsteps):
             a = self.comm.max([x.local_max_speed() for x in self.h])
             for s in range(3):
-                self._fill_z_ghosts(s)
-                for x in self.h:
-                    x.step_stage_cfl(cfl, s, a)
+                if not overlap:
+                    self._fill_z_ghosts(s)
+                    for x in self.h:
+                        x.step_stage_cfl(cfl, s, a)
+                    continue
+                pairs = [(x.get_zhalo(s, 0), x.get_zhalo(s, 1)) for x in self.h]
+                got, ready = self.comm.exchange_async(pairs)
+                for x, (below, above) in zip(self.h, got):
+                    x.step_stage_overlap(cfl, s, a, below, above, ready)
 
 
 def make_slab(binding, w, k0, k1, precision=0, device="cuda"):

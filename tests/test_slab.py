@@ -108,6 +108,12 @@ class FakeHydro:
         self.buf[(stage + 1) % 3][G:-G] = u[G:-G] + dt * (u[:-2 * G] - 2.0 * u[G:-G] + u[2 * G:])
         self.calls.append(("stage", stage))
 
+    def step_stage_overlap(self, cfl, stage, a, lo, hi, ready):
+        assert ready is None                      # CPU tensors: no stream to wait on
+        self.put_zhalo(stage, 0, lo)
+        self.put_zhalo(stage, 1, hi)
+        self.step_stage_cfl(cfl, stage, a)
+
     def interior(self):
         return self.buf[0][self.G:-self.G].clone()
 
@@ -116,29 +122,30 @@ def _planes(nz):
     return [math.sin(0.7 * k) + 0.05 * k for k in range(nz)]
 
 
-def _step_worker(rank, world, port, bc, nz, nsteps, out):
+def _step_worker(rank, world, port, bc, nz, nsteps, overlap, out):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     k0, k1 = S.split_planes(nz, world)[rank]
     h = FakeHydro(_planes(nz)[k0:k1])
-    S.SlabGroup([h], S.DistComm(dist, bc), 1.0).step_cfl(0.1, nsteps)
+    S.SlabGroup([h], S.DistComm(dist, bc), 1.0).step_cfl(0.1, nsteps, overlap=overlap)
     out[rank] = (h.interior().tolist(), h.calls[:9])
     dist.barrier()
     dist.destroy_process_group()
 
 
+@pytest.mark.parametrize("overlap", [False, True])
 @pytest.mark.parametrize("bc", [S.BC_PERIODIC, S.BC_OUTFLOW])
-def test_step_cfl_control_flow_over_gloo_two_ranks(bc):
+def test_step_cfl_control_flow_over_gloo_two_ranks(bc, overlap):
     """SlabGroup.step_cfl end to end with two ranks over gloo: the max-reduction of the device scalar, one exchange
     per stage BEFORE that stage, the ring of two (periodic) or the zero-gradient ends (outflow).  The decomposed run
     must equal, bit for bit, the same fake advanced as one domain."""
     nz, nsteps, world = 11, 3, 2
     one = FakeHydro(_planes(nz))
-    S.SlabGroup([one], S.LocalComm(1, bc), 1.0).step_cfl(0.1, nsteps)
-    port = 33500 + os.getpid() % 2000 + bc
+    S.SlabGroup([one], S.LocalComm(1, bc), 1.0).step_cfl(0.1, nsteps, overlap=overlap)
+    port = 33500 + os.getpid() % 2000 + bc + 2 * int(overlap)
     with mp.Manager() as m:
         out = m.dict()
-        mp.spawn(_step_worker, args=(world, port, bc, nz, nsteps, out), nprocs=world, join=True)
+        mp.spawn(_step_worker, args=(world, port, bc, nz, nsteps, overlap, out), nprocs=world, join=True)
         res = dict(out)
     got = res[0][0] + res[1][0]
     assert got == one.interior().tolist()
@@ -149,9 +156,10 @@ def test_step_cfl_control_flow_over_gloo_two_ranks(bc):
 
 # ------------------------------------------------------------------ GPU: bit-identity with the undecomposed run
 @pytest.mark.gpu
+@pytest.mark.parametrize("overlap", [False, True])
 @pytest.mark.parametrize("scheme", [W.WENO5, W.WENO7, W.MUSTA_FORCE])
 @pytest.mark.parametrize("bc_z,parts", [(W.BC_PERIODIC, 2), (W.BC_OUTFLOW, 3), (W.BC_PERIODIC, 1)])
-def test_slabs_reproduce_the_single_domain_run_bit_for_bit(scheme, bc_z, parts):
+def test_slabs_reproduce_the_single_domain_run_bit_for_bit(scheme, bc_z, parts, overlap):
     from paper_1604_03360_b200 import binding as B
     n = (40, 33, 70)
     big = W.lumpy(n=max(n), hotspots=12, with_velocity=True, scheme=scheme, box=max(n) / 16.0, sigma_unit=0.12)
@@ -165,7 +173,7 @@ def test_slabs_reproduce_the_single_domain_run_bit_for_bit(scheme, bc_z, parts):
     ranges = S.split_planes(n[2], parts)
     hs = [S.make_slab(B, w, k0, k1) for k0, k1 in ranges]
     group = S.SlabGroup(hs, S.LocalComm(parts, bc_z), w.dx)
-    group.step_cfl(0.2, 3)
+    group.step_cfl(0.2, 3, overlap=overlap)
     got = torch.cat([h.get_state().cpu() for h in hs], dim=1)
     assert all(h.status() == 0 for h in hs)
     assert abs(hs[0].time - t_ref) == 0.0
@@ -196,3 +204,35 @@ def test_put_zhalo_without_a_buffer_is_the_outflow_rule(scheme, g):
             h.step_stage(1e-3, s)
     assert torch.equal(h.get_state().cpu(), want)
     h.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("scheme", [W.WENO5, W.MUSTA_FORCE])
+def test_dist_comm_side_stream_path_on_one_gpu(scheme):
+    """DistComm over a one-rank NCCL group (a periodic ring of one): the exchange is issued on the side stream, the
+    stage waits for its event only before the boundary planes; the result must equal the undecomposed run bit for
+    bit, and the serial (no overlap) path too."""
+    from paper_1604_03360_b200 import binding as B
+    dist.init_process_group("nccl", init_method="tcp://127.0.0.1:%d" % (36500 + os.getpid() % 2000 + scheme), rank=0,
+                            world_size=1)
+    try:
+        _ring_of_one(B, scheme)
+    finally:
+        dist.destroy_process_group()
+
+
+def _ring_of_one(B, scheme):
+    n = (40, 33, 70)
+    big = W.lumpy(n=max(n), hotspots=12, with_velocity=True, scheme=scheme, box=max(n) / 16.0, sigma_unit=0.12)
+    cons = np.ascontiguousarray(big.cons[:, :n[2], :n[1], :n[0]])
+    w = W.Workload("ring1", n, big.dx, (0.0, 0.0, 0.0), scheme, (W.BC_PERIODIC,) * 3, cons, 0.0, cfl=0.2)
+    ref = B.from_workload(w)
+    ref.step_cfl(0.2, 4)
+    want = ref.get_state()
+    ref.close()
+    for overlap in (True, False):
+        h = S.make_slab(B, w, 0, n[2])
+        S.SlabGroup([h], S.DistComm(dist, W.BC_PERIODIC), w.dx).step_cfl(0.2, 4, overlap=overlap)
+        assert torch.equal(h.get_state(), want)
+        assert h.status() == 0
+        h.close()
