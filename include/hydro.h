@@ -80,7 +80,7 @@ int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme)
  *   "hubble_t0|hubble_e0|hubble_n0|hubble_bx|hubble_by|hubble_bz"  parameters of the closed-form
  *                   Hubble flow used by HYDRO_BC_HUBBLE (readings Q13, Q14)
  *   "tile_zc", "sweep_zc"  cells a block of the x/z kernel marches through along z / of the y sweep along y
- *                   (defaults 128 / 128 for the WENO kernels, 64 / 128 for MUSTA-FORCE; tuning knobs: a longer
+ *                   (defaults 64 / 128 for all kernels, doubled for the WENO kernels on axes of 256 / 512 cells or more; tuning knobs: a longer
  *                   march amortises the one redundant flux and the pipeline fill of a chunk)
  *   "profile"       0 (default) | 1: record a CUDA event pair on the stream around every stage-kernel
  *                   launch, read back with hydro_stage_kernel_time
