@@ -229,3 +229,25 @@ def test_eos_table_arguments_are_checked(B):
     h.set_option("eos", 0)
     h.set_option("eos", 2)
     h.close()
+
+
+# ------------------------------------------------------------------ fp32: the cross-multiplied WENO weights at any data scale
+@pytest.mark.parametrize("scheme", [W.WENO5, W.WENO7])
+@pytest.mark.parametrize("scale,eps", [(1e4, 1e-6), (1e3, 1e-6), (1e-3, 1e-14), (1.0, 1e-13)])
+def test_fp32_weno_weights_survive_any_data_scale(B, oracle, scheme, scale, eps):
+    """The fp32 kernels multiply the weights through (products of squared smoothness indicators: the 6th power for
+    WENO7).  Flux jumps of 1e4..1e5 would overflow them and a tiny epsilon on flat data underflow them; the kernels
+    rescale the indicators by a power of two first.  L(u) of scaled data against the fp64 oracle with the same
+    epsilon (the equations are homogeneous of degree one in (E, M, R), so the data stay admissible)."""
+    w = small_workload(scheme, (45, 23, 38))
+    cons = w.cons * scale
+    ws = W.Workload("scaled", w.n, w.dx, (0, 0, 0), scheme, (W.BC_PERIODIC,) * 3, cons, 0.0,
+                    options={"weno_eps": eps})
+    o = oracle.from_workload(ws)
+    h = B.from_workload(ws, precision=1)
+    Lo = o.eval_L(cons)
+    Lg = h.eval_L(to_dev(B, cons, h.dtype)).cpu().numpy()
+    assert np.all(np.isfinite(Lg))
+    assert reldiff(Lg, Lo, scale=np.max(np.abs(cons[0])) / w.dx) <= 3e-5
+    assert h.status() == 0
+    h.close()
