@@ -44,7 +44,7 @@ BYTES_PER_CELL_STEP = {"f64": 320.0, "f32": 160.0}
 # DRAM bytes of one stage (x/z kernel + y sweep), dram__bytes_read.sum + dram__bytes_write.sum of one
 # `ncu --set full` capture of each kernel at 512^3 (profiles/r02_*_ncu.txt); algorithmic bytes of one stage at that
 # size: 320/3 B x 512^3 = 1.43e10
-TRAFFIC_BYTES_PER_STAGE = {("musta", "f64", 512): 27.62e9, ("weno5", "f64", 512): 27.94e9, ("weno7", "f64", 512): 28.09e9}
+TRAFFIC_BYTES_PER_STAGE = {("musta", "f64", 512): 27.61e9, ("weno5", "f64", 512): 27.6e9, ("weno7", "f64", 512): 27.6e9}
 # (the captured launches are the first stage of a step, which does not read u^n: stages 2 and 3 add 5.4e9 each)
 KERNEL_NAMES = {"weno5": "weno_xz_kernel<T,3> + weno_y_kernel<T,3,EPI>", "weno7": "weno_xz_kernel<T,4> + weno_y_kernel<T,4,EPI>",
                 "musta": "musta_xz_kernel<T,FAST> + musta_y_kernel<T,EPI,FAST>"}
