@@ -49,7 +49,8 @@ enum { NF = 5 };  // E, Mx, My, Mz, R
 template <class T>
 struct Prim {
     T e, p, n, v[3];
-    T cs2 = (T)1 / (T)3;   // dp/de at this state (1/3 for p = e/3, 0 for p = p0, the table's slope for kind 2)
+    T cs2 = (T)0.33333333333333331;   // dp/de at this state (1/3 for p = e/3, 0 for p = p0, the table's slope for kind 2);
+                                      // a literal: the default must not add an operation to con2prim's count
 };
 
 // Equation of state.  kind 0: p = e/3 (reading Q2, the default everywhere).  kind 1: p = p0, a
