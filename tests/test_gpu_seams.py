@@ -251,3 +251,91 @@ def test_fp32_weno_weights_survive_any_data_scale(B, oracle, scheme, scale, eps)
     assert reldiff(Lg, Lo, scale=np.max(np.abs(cons[0])) / w.dx) <= 3e-5
     assert h.status() == 0
     h.close()
+
+
+# ------------------------------------------------------------------ maximum sizes: index arithmetic beyond 2^31 elements
+def test_large_noncubic_grid_beyond_2_31_elements(B, oracle):
+    """1100 x 700 x 600 = 4.6e8 cells: one padded field has 4.7e8 elements, a state 2.4e9 (> 2^31) and 1.9e10 bytes
+    (> 2^32), the workspace 57 GB.  The state is generated on the GPU (seeded torch generator; smooth hotspots with
+    blended velocities like config 5), advanced by one WENO5 step, and checked on sampled cells against the oracle
+    (19^3 crops, including cells in the last planes, rows and columns, whose offsets are the largest) and for
+    conservation."""
+    import torch
+    nx, ny, nz = 1100, 700, 600
+    free, _ = torch.cuda.mem_get_info()
+    if free < 110e9:
+        pytest.skip("needs about 110 GB of free device memory")
+    dev, dt_ = "cuda", torch.float64
+    g = torch.Generator(device=dev)
+    g.manual_seed(1604)
+    box = (nx / 32.0, ny / 32.0, nz / 32.0)
+    dx = 1.0 / 32.0
+    ax = [(torch.arange(n, device=dev, dtype=dt_) + 0.5) * dx for n in (nx, ny, nz)]
+    X, Y, Z = ax[0].view(1, 1, nx), ax[1].view(1, ny, 1), ax[2].view(nz, 1, 1)
+    e = torch.full((nz, ny, nx), 0.1, device=dev, dtype=dt_)
+    mv = [torch.zeros_like(e) for _ in range(3)]
+    nh = 24
+    c = torch.rand(nh, 3, generator=g, device=dev, dtype=dt_) * torch.tensor(box, device=dev, dtype=dt_)
+    sg = 0.6 + 1.0 * torch.rand(nh, generator=g, device=dev, dtype=dt_)
+    A = torch.exp(0.5 * torch.randn(nh, generator=g, device=dev, dtype=dt_))
+    vv = torch.randn(nh, 3, generator=g, device=dev, dtype=dt_)
+    vv = vv / vv.norm(dim=1, keepdim=True) * (0.5 * torch.rand(nh, 1, generator=g, device=dev, dtype=dt_))
+    for k in range(nh):
+        def dist(a, cc, L):
+            t = (a - cc).abs()
+            return torch.minimum(t, L - t)
+        gk = A[k] * (torch.exp(-dist(X, c[k, 0], box[0]) ** 2 / (2 * sg[k] ** 2)) *
+                     torch.exp(-dist(Y, c[k, 1], box[1]) ** 2 / (2 * sg[k] ** 2)) *
+                     torch.exp(-dist(Z, c[k, 2], box[2]) ** 2 / (2 * sg[k] ** 2)))
+        e += gk
+        for a in range(3):
+            mv[a] += gk * vv[k, a]
+        del gk
+    cons = torch.empty((5, nz, ny, nx), device=dev, dtype=dt_)
+    v2 = torch.zeros_like(e)
+    for a in range(3):
+        mv[a] /= e                      # blended velocity, |v| < 0.5
+        v2 += mv[a] * mv[a]
+    g2 = 1.0 / (1.0 - v2)
+    del v2
+    w = (4.0 / 3.0) * e * g2
+    cons[0] = w - e / 3.0
+    for a in range(3):
+        cons[1 + a] = w * mv[a]
+    cons[4] = 0.2 * e ** 0.75 * g2.sqrt()
+    del w, g2, e, mv
+    h = B.Hydro(nx, ny, nz, dx, W.WENO5)
+    for axn in "xyz":
+        h.set_option("bc_" + axn, W.BC_PERIODIC)
+    h.bind()
+    h.set_state(cons)
+    dt = 0.2 * dx / h.max_signal_speed()
+    tot0 = [float(cons[cc].sum()) for cc in range(5)]
+    h.step(dt, 1)
+    assert h.status() == 0
+    out = h.get_state()
+    tot1 = [float(out[cc].sum()) for cc in range(5)]
+    for a, b in zip(tot0, tot1):
+        assert abs(a - b) <= 1e-11 * abs(tot0[0]), (tot0, tot1)
+    half = 9
+    samples = [(0, 0, 0), (nx - 1, ny - 1, nz - 1), (nx - 2, 3, nz - 1), (30, ny - 1, 63), (31, 7, 64), (620, 127, 599),
+               (nx // 2, ny // 2, nz // 2), (1099, 0, 128), (333, 699, 111)]
+    scale = float(cons[0].abs().max())
+    fmax = [float(cons[cc].abs().max()) for cc in range(5)]
+    worst = 0.0
+    for (i, j, k) in samples:
+        ix = torch.arange(i - half, i + half + 1, device=dev) % nx
+        iy = torch.arange(j - half, j + half + 1, device=dev) % ny
+        iz = torch.arange(k - half, k + half + 1, device=dev) % nz
+        crop = cons[:, iz][:, :, iy][:, :, :, ix].cpu().numpy()
+        m = 2 * half + 1
+        wc = W.Workload("crop", (m, m, m), dx, (0, 0, 0), W.WENO5, (W.BC_PERIODIC,) * 3, np.ascontiguousarray(crop))
+        o = oracle.from_workload(wc)
+        o.step(dt, 1)
+        ref = o.get_state()[:, half, half, half]
+        got = out[:, k, j, i].cpu().numpy()
+        for cc in range(5):
+            den = max(abs(ref[cc]), 1e-15 * scale) if cc == 0 else max(fmax[cc], 1e-15 * scale)
+            worst = max(worst, abs(got[cc] - ref[cc]) / den)
+    assert worst <= 3e-12, worst
+    h.close()
