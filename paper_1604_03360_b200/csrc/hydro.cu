@@ -40,11 +40,9 @@ struct hydro_ctx {
     size_t ws_bytes = 0;
     Ctl* ctl = nullptr;
     char* U[3] = {nullptr, nullptr, nullptr};  // u^n and two stage buffers (padded, 5 fields each)
-    char* Wb[2] = {nullptr, nullptr};           // primitives (padded, 7 arrays) for the GENERIC kernel only (grids with an
-                                                // inactive axis, "kernel" = generic): the marching kernels make their
-                                                // primitives on the fly; Wb[1] is unused (= Wb[0])
-    int wcur = 0;
-    bool w_ready = false;                       // (generic path) never true: the primitives are remade every stage
+    char* Wb = nullptr;                         // primitives (padded, 7 arrays) for the GENERIC kernel only (grids with an
+                                                // inactive axis, "kernel" = generic), remade every stage; the marching
+                                                // kernels make their primitives on the fly
     bool max_ready = false;                     // ctl->maxspeed_bits holds the max signal speed of u^n (stage-3 epilogue)
     int stage_open = 0;                         // stages of a hydro_step_stage sequence done so far (0 = between steps)
     int device = -1;                            // CUDA device of the workspace (captured at bind)
@@ -60,7 +58,6 @@ struct hydro_ctx {
     struct StepGraph {
         cudaGraphExec_t exec;
         double cfl;
-        int wcur_before, wcur_after;
         long long launches;
     };
     int use_graph = 0;
@@ -152,7 +149,7 @@ int need_ws(hydro_ctx* c) {
 }
 
 template <class T>
-int do_halo(hydro_ctx* c, T* pad, double tfrac, bool use_abs, double t_abs, T* Wghost = nullptr) {
+int do_halo(hydro_ctx* c, T* pad, double tfrac, bool use_abs, double t_abs) {
     HaloArgs A;
     long long total = 0;
     for (int a = 0; a < 3; ++a) {
@@ -167,7 +164,7 @@ int do_halo(hydro_ctx* c, T* pad, double tfrac, bool use_abs, double t_abs, T* W
     if (total == 0) return HYDRO_OK;
     const int tb = 256;
     halo_fill_kernel<T><<<(unsigned)((total + tb - 1) / tb), tb, 0, c->stream>>>(c->G, A, c->ctl, tfrac, t_abs,
-                                                                                   use_abs ? 1 : 0, pad, Wghost);
+                                                                                   use_abs ? 1 : 0, pad);
     LAUNCHED(c, "halo_fill_kernel");
     return HYDRO_OK;
 }
@@ -175,7 +172,7 @@ int do_halo(hydro_ctx* c, T* pad, double tfrac, bool use_abs, double t_abs, T* W
 template <class T>
 int do_prim(hydro_ctx* c, const T* pad, int do_max) {
     const dim3 b = blk2d(64, 4);
-    prim_kernel<T><<<grd(c->G.np[0], c->G.np[1], c->G.np[2], b), b, 0, c->stream>>>(c->G, pad, (T*)c->Wb[c->wcur], c->ctl,
+    prim_kernel<T><<<grd(c->G.np[0], c->G.np[1], c->G.np[2], b), b, 0, c->stream>>>(c->G, pad, (T*)c->Wb, c->ctl,
                                                                                       do_max, c->eos);
     LAUNCHED(c, "prim_kernel");
     return HYDRO_OK;
@@ -275,7 +272,7 @@ int do_stage(hydro_ctx* c, const T* Us, const T* Un, T* Uout, double ca, double 
         return fail(c, HYDRO_EINVAL, "kernel=fused requested but the grid does not allow it (an axis is inactive)");
     const dim3 b = blk2d(32, 4);
     const dim3 g = grd(c->G.n[0], c->G.n[1], c->G.n[2], b);
-    const T* W = (const T*)c->Wb[c->wcur];
+    const T* W = (const T*)c->Wb;
     switch (c->scheme) {
         case HYDRO_WENO5: stage_generic_kernel<T, 0><<<g, b, 0, c->stream>>>(c->G, A, Us, W, Un, Uout, c->ctl); break;
         case HYDRO_WENO7: stage_generic_kernel<T, 1><<<g, b, 0, c->stream>>>(c->G, A, Us, W, Un, Uout, c->ctl); break;
@@ -316,6 +313,11 @@ int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl, const double
     T* const out[3] = {U[1], U[2], U[0]};   // stage 3 writes u^n in place: each cell reads only its own u^n
     int rc;
     if ((rc = do_halo<T>(c, in[s], tfrac[s], false, 0.0))) return rc;
+    if (ov.on && !marching) {   // generic kernel: no split; the ghost planes first (its con2prim pass reads them)
+        if (ov.ready != nullptr) CUDA_OK(c, cudaStreamWaitEvent(c->stream, ov.ready, 0));
+        if ((rc = zhalo_impl(c, s, 0, const_cast<void*>(ov.lo), ov.lo ? 1 : 2))) return rc;
+        if ((rc = zhalo_impl(c, s, 1, const_cast<void*>(ov.hi), ov.hi ? 1 : 2))) return rc;
+    }
     const bool need_max = s == 0 && cflmode && !c->max_ready && ext_max == nullptr;
     if (need_max) {   // the reduction accumulates with atomicMax: start from zero
         reset_max_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
@@ -345,14 +347,7 @@ int do_step_stage(hydro_ctx* c, int s, double dt_fixed, double cfl, const double
             if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, epi, 1, nz - b, nz))) return rc;
             if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, epi, 2))) return rc;
         } else if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, epi))) return rc;
-    } else {
-        if (ov.on) {   // generic kernel: no split, the ghosts first
-            if (ov.ready != nullptr) CUDA_OK(c, cudaStreamWaitEvent(c->stream, ov.ready, 0));
-            if ((rc = zhalo_impl(c, s, 0, const_cast<void*>(ov.lo), ov.lo ? 1 : 2))) return rc;
-            if ((rc = zhalo_impl(c, s, 1, const_cast<void*>(ov.hi), ov.hi ? 1 : 2))) return rc;
-        }
-        if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, epi))) return rc;
-    }
+    } else if ((rc = do_stage<T>(c, in[s], U[0], out[s], ca[s], cb[s], 0, epi))) return rc;
     if (s == 2) {
         end_step_kernel<<<1, 1, 0, c->stream>>>(c->ctl);
         LAUNCHED(c, "end_step_kernel");
@@ -386,14 +381,12 @@ bool graph_ready(const hydro_ctx* c) {
 template <class T>
 int graph_step(hydro_ctx* c, double cfl) {
     for (const auto& g : c->graphs)
-        if (g.cfl == cfl && g.wcur_before == c->wcur) {
+        if (g.cfl == cfl) {
             CUDA_OK(c, cudaGraphLaunch(g.exec, c->stream));
-            c->wcur = g.wcur_after;
             c->launches += g.launches;
             return HYDRO_OK;
         }
     // capture: nothing executes, the host-side bookkeeping of do_step is rolled back afterwards
-    const int wcur0 = c->wcur;
     const long long l0 = c->launches;
     if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
         cudaGetLastError();
@@ -405,10 +398,7 @@ int graph_step(hydro_ctx* c, double cfl) {
     const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
     hydro_ctx::StepGraph g;
     g.cfl = cfl;
-    g.wcur_before = wcur0;
-    g.wcur_after = c->wcur;
     g.launches = c->launches - l0;
-    c->wcur = wcur0;
     c->launches = l0;
     if (rc != HYDRO_OK || e != cudaSuccess || graph == nullptr) {
         if (graph) cudaGraphDestroy(graph);
@@ -527,7 +517,7 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
     } else if (k == "kernel") {
         const int p = (int)v;
         if (p < 0 || p > 2) return fail(c, HYDRO_EINVAL, "kernel must be 0, 1 or 2");
-        if (c->ws && p == HYDRO_KERNEL_GENERIC && c->Wb[0] == nullptr)
+        if (c->ws && p == HYDRO_KERNEL_GENERIC && c->Wb == nullptr)
             return fail(c, HYDRO_EINVAL, "kernel = generic needs its primitive arrays: set it before the workspace is bound");
         c->kernel = p;
     } else if (k == "tile_zc" || k == "sweep_zc") {
@@ -546,11 +536,11 @@ int hydro_set_option(hydro_ctx* c, const char* key, double v) {
         if (v != 0.0 && v != 1.0 && !(v == 2.0 && c->eos.tab != nullptr))
             return fail(c, HYDRO_EINVAL, "eos must be 0 (p = e/3), 1 (p = p0) or 2 (after hydro_set_eos_table)");
         c->eos.kind = (int)v;
-        c->w_ready = c->max_ready = false;   // cached primitives and max signal speed belong to the old closure
+        c->max_ready = false;   // the cached max signal speed belongs to the old closure
     } else if (k == "eos_p0") {
         if (!(v >= 0)) return fail(c, HYDRO_EINVAL, "eos_p0 < 0");
         c->eos.p0 = v;
-        c->w_ready = c->max_ready = false;
+        c->max_ready = false;
     } else if (k == "limiter") {
         if (v < 0 || v > 3) return fail(c, HYDRO_EINVAL, "limiter must be 0..3");
         c->limiter = (int)v;
@@ -604,9 +594,8 @@ int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
     c->ctl = (Ctl*)base;
     const size_t sb = state_bytes(c);
     for (int i = 0; i < 3; ++i) c->U[i] = base + 256 + i * sb;
-    c->Wb[0] = c->Wb[1] = needs_w(c) ? base + 256 + 3 * sb : nullptr;
-    c->wcur = 0;
-    c->w_ready = c->max_ready = false;
+    c->Wb = needs_w(c) ? base + 256 + 3 * sb : nullptr;
+    c->max_ready = false;
     c->stage_open = 0;
     drop_graphs(c);
     CUDA_OK(c, cudaMemsetAsync(p, 0, hydro_workspace_bytes(c), c->stream));
@@ -631,7 +620,7 @@ int hydro_set_state(hydro_ctx* c, const void* cons) {
     if (c->precision == HYDRO_F64) pack_kernel<double><<<g, b, 0, c->stream>>>(c->G, (const double*)cons, (double*)c->U[0]);
     else pack_kernel<float><<<g, b, 0, c->stream>>>(c->G, (const float*)cons, (float*)c->U[0]);
     LAUNCHED(c, "pack_kernel");
-    c->w_ready = c->max_ready = false;
+    c->max_ready = false;
     c->stage_open = 0;
     set_ctl_kernel<<<1, 1, 0, c->stream>>>(c->ctl, 0.0, 0, 1);   // the time is the caller's ("t" option): kept
     LAUNCHED(c, "set_ctl_kernel");
@@ -720,7 +709,7 @@ int hydro_set_eos_table(hydro_ctx* c, const void* p_device, int n, double e_min,
     c->eos.e_min = e_min;
     c->eos.de = (e_max - e_min) / (n - 1);
     c->eos.kind = 2;
-    c->w_ready = c->max_ready = false;
+    c->max_ready = false;
     return HYDRO_OK;
 }
 

@@ -139,7 +139,7 @@ struct HaloArgs {
 
 template <class T>
 __global__ void halo_fill_kernel(Geom G, HaloArgs A, Ctl* ctl, double tfrac, double t_abs,
-                                 int use_abs, T* __restrict__ pad, T* __restrict__ Wghost) {
+                                 int use_abs, T* __restrict__ pad) {
     long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     int a = 0;
     for (; a < 3; ++a) {
@@ -162,35 +162,20 @@ __global__ void halo_fill_kernel(Geom G, HaloArgs A, Ctl* ctl, double tfrac, dou
     cell[a2] = q2;
     cell[a] = m < g ? m - g : n + (m - g);
     const long long p = G.pidx(cell[0], cell[1], cell[2]);
+    if (A.bc[a] == 3) return;   // external ghosts (slab decomposition): the caller's business (hydro_put_zhalo)
     T val[NF];
-    if (A.bc[a] == 3) {
-        // external ghosts (slab decomposition): only their primitives may have to be made below
-        if (Wghost == nullptr) return;
-#pragma unroll
-        for (int c = 0; c < NF; ++c) val[c] = pad[c * G.fs + p];
+    if (A.bc[a] == 2) {
+        const double tt = use_abs ? t_abs : ctl->t + tfrac * ctl->dt;
+        hubble_state<T>(A.H, A.bc, cell, tt, val);
     } else {
-        if (A.bc[a] == 2) {
-            const double tt = use_abs ? t_abs : ctl->t + tfrac * ctl->dt;
-            hubble_state<T>(A.H, A.bc, cell, tt, val);
-        } else {
-            int from[3] = {cell[0], cell[1], cell[2]};
-            from[a] = A.bc[a] == 1 ? ((cell[a] % n) + n) % n : min(max(cell[a], 0), n - 1);
-            const long long ps = G.pidx(from[0], from[1], from[2]);
+        int from[3] = {cell[0], cell[1], cell[2]};
+        from[a] = A.bc[a] == 1 ? ((cell[a] % n) + n) % n : min(max(cell[a], 0), n - 1);
+        const long long ps = G.pidx(from[0], from[1], from[2]);
 #pragma unroll
-            for (int c = 0; c < NF; ++c) val[c] = pad[c * G.fs + ps];
-        }
-#pragma unroll
-        for (int c = 0; c < NF; ++c) pad[c * G.fs + p] = val[c];
+        for (int c = 0; c < NF; ++c) val[c] = pad[c * G.fs + ps];
     }
-    // when the interior primitives came from the previous stage's epilogue, the ghost cells' are made here
-    if (Wghost != nullptr) {
-        T w[NW];
-        int flag = 0;
-        prim_of_cell(val, w, flag, A.eos);
 #pragma unroll
-        for (int q = 0; q < NW; ++q) Wghost[q * G.fs + p] = w[q];
-        if (flag) ctl->flag = 1;
-    }
+    for (int c = 0; c < NF; ++c) pad[c * G.fs + p] = val[c];
 }
 
 // ------------------------------------------------------------------------------------------------

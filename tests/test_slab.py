@@ -183,6 +183,29 @@ def test_slabs_reproduce_the_single_domain_run_bit_for_bit(scheme, bc_z, parts, 
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("scheme", [W.WENO5, W.WENO7, W.MUSTA_FORCE])
+@pytest.mark.parametrize("n", [(1, 24, 30), (40, 33, 24)])
+def test_generic_kernel_slabs_with_overlap_call(scheme, n):
+    """The slab calls on the generic kernel (a grid with an inactive axis, or "kernel" = generic): the overlap call
+    has nothing to split there, but must still give the undecomposed result bit for bit."""
+    from paper_1604_03360_b200 import binding as B
+    cons = W.random_state((n[2], n[1], n[0]), seed=9, vmax=0.4)
+    w = W.Workload("g", n, 0.05, (0.0, 0.0, 0.0), scheme, (W.BC_PERIODIC, W.BC_OUTFLOW, W.BC_PERIODIC), cons, 0.0, cfl=0.2,
+                   options={"kernel": 1})
+    ref = B.from_workload(w, kernel=B.KERNEL_GENERIC)
+    ref.step_cfl(0.2, 3)
+    want = ref.get_state().cpu()
+    ref.close()
+    for overlap in (True, False):
+        hs = [S.make_slab(B, w, k0, k1) for k0, k1 in S.split_planes(n[2], 2)]
+        S.SlabGroup(hs, S.LocalComm(2, W.BC_PERIODIC), w.dx).step_cfl(0.2, 3, overlap=overlap)
+        got = torch.cat([h.get_state().cpu() for h in hs], dim=1)
+        assert torch.equal(got, want)
+        for h in hs:
+            h.close()
+
+
+@pytest.mark.gpu
 @pytest.mark.parametrize("scheme,g", [(W.WENO5, 3), (W.MUSTA_FORCE, 2)])
 def test_put_zhalo_without_a_buffer_is_the_outflow_rule(scheme, g):
     """hydro_put_zhalo(NULL) on a slab with external z ghosts must give exactly what bc_z = outflow gives: the same
