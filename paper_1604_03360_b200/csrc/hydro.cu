@@ -1,7 +1,8 @@
 // hydro.cu -- C ABI of libhydro_b200 (include/hydro.h): context, options, workspace carving and the
 // launch sequence of one SSP-RK3 step:
-//   per stage:  halo fill (a1) -> [con2prim + speeds + max (a2-a4), first step only] -> stage kernels (a5-a9, and
-//   a2-a4 of the cells they finish)
+//   per stage:  halo fill (a1) -> [max signal speed (a4), first CFL step only] -> stage kernels (a2-a3 of the cells
+//   they read, a5-a9, and a4 of the cells stage 3 finishes); optionally replayed from a CUDA graph, or split around a
+//   halo exchange for the slab decomposition
 // No CPU arithmetic of the method happens here: the host only orders kernels on the caller's stream.
 #include <cuda_runtime.h>
 

@@ -2,20 +2,23 @@
 // the SSP-RK3 combination (a9), every interface flux computed once.
 //
 // The predictor-corrector flux runs con2prim on face states that mix all five fields, so one thread carries all
-// five fields of its stencil.
-//   musta_xz_kernel<T>     x and z fluxes in ONE marching kernel without block barriers.  A warp is a row of 32
+// five fields of its stencil.  The MUSCL slope belongs to a cell and is made once per cell.
+//   musta_xz_kernel<T, FAST>  x and z fluxes in ONE marching kernel without block barriers.  A warp is a row of 32
 //       consecutive x positions (lane 0 is the helper column one cell below the 31 cells the warp owns), a block is
 //       four such rows, and every thread marches along z through a chunk of planes:
-//         z: the 4-cell stencil of the thread's column lives in a register window;
-//         x: the plane-k cells of the window are exactly the row the x-stencil needs, so every lane writes its cell
-//            into a per-WARP shared-memory row, 3 halo lanes add the cells beyond the row's ends, and after a
-//            __syncwarp each lane reads its 4-cell x-stencil from that row.  The lower-face flux comes from lane-1
-//            by shuffle.
+//         z: the column state (MustaColumn: u_k, u_{k+1}, their difference, Q_L of face k+1/2) lives in registers;
+//         x: every lane writes its plane-k cell into a per-WARP shared-memory row, 3 halo lanes add the cells beyond
+//            the row's ends; after a __syncwarp each lane reads its two neighbours, makes the slope of ITS cell,
+//            keeps Q_L of its upper face and hands Q_R of its lower face to the lane below by shuffle (the last
+//            lane also makes the one slope beyond the row).  The lower-face flux comes from lane-1 by shuffle.
+//         The x and the z interface of a plane are evaluated in one basic block (four independent con2prim chains).
 //       Writes Uout = ca u^n + cb (u_s + dt (L_x + L_z)).
-//   musta_y_kernel<T, EPI> the marching sweep along y: thread per (x, z) column, threads of a warp along x (so every
-//       access is coalesced), adds cb dt L_y to Uout.  EPI (stage 3 of a CFL step): the thread holds the finished
-//       cell, so it also reduces the max signal speed of the new state (a4) for the next step's dt.
-// Every global read of the marching loops is a cp.async into the thread's own slots, DEPTH cells ahead (pipeline.cuh).
+//   musta_y_kernel<T, EPI, FAST>  the marching sweep along y: thread per (x, z) column, threads of a warp along x (so
+//       every access is coalesced), two cells per iteration, adds cb dt L_y to Uout.  EPI (stage 3 of a CFL step):
+//       the thread holds the finished cells, so it also reduces the max signal speed of the new state (a4).
+// FAST = the default configuration (K = 2, minmod, p = e/3): the branch-free core of iface.cuh with the general,
+// clamped core as the rare repair; otherwise the general core with run-time K, limiter and closure.
+// Every global read of the marching loops is a cp.async into the thread's own slots, a few cells ahead (pipeline.cuh).
 #pragma once
 #include <cstdio>
 

@@ -1,7 +1,8 @@
 // kernels_aux.cuh -- the small kernels around the stage kernel:
 //   (d) halo_fill_kernel    a1: outflow / periodic / analytic Hubble ghost fill, face ghosts only
 //   (a) prim_kernel         a2-a4: con2prim + three signal speeds per padded cell, fused with the
-//                           warp-shuffle / block / atomic max reduction for the CFL time step
+//                           warp-shuffle / block / atomic max reduction for the CFL time step (the GENERIC
+//                           kernel's primitives; the marching kernels make theirs on the fly)
 //       max_speed_kernel    a4 alone (interior cells, no stores): hydro_max_signal_speed
 //       pack / unpack       interior <-> padded copies for hydro_set_state / hydro_get_state
 //       begin_step / end_step  device-resident dt and t
