@@ -2,10 +2,10 @@
 //
 // Layout: every field is one padded 3-D array [npz][npy][sx], x fastest;
 // np = n + 2g on active axes (g = 3 / 4 / 2), np = n on inactive ones; the row pitch sx rounds npx up
-// to 16 bytes and the field stride fs rounds sx*npy*npz up to 256 bytes, so that every row start is a
-// legal TMA / 128-bit address.  A state is five such arrays (E, Mx, My, Mz, R), the primitives another
-// five (winv, p, a_x, a_y, a_z).  Only face ghosts are ever filled or read: the sweeps are
-// dimension-by-dimension, so edge and corner ghosts stay zero and are never touched.
+// to 16 bytes and the field stride fs rounds sx*npy*npz up to 256 bytes, so that every row start is
+// 16-byte aligned.  A state is five such arrays (E, Mx, My, Mz, R); the generic kernel keeps another seven
+// (v_x, v_y, v_z, p, a_x, a_y, a_z).  Only face ghosts are ever filled or read: the sweeps are
+// dimension-by-dimension, so edge and corner ghosts stay zero and are never used.
 #pragma once
 #include <cuda_runtime.h>
 
