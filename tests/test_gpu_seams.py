@@ -339,3 +339,21 @@ def test_large_noncubic_grid_beyond_2_31_elements(B, oracle):
             worst = max(worst, abs(got[cc] - ref[cc]) / den)
     assert worst <= 3e-12, worst
     h.close()
+
+
+def test_generic_kernel_must_be_chosen_before_the_workspace_is_bound(B):
+    """The marching kernels keep no primitive arrays, so a workspace bound for them has none: asking for the generic
+    kernel afterwards is refused (and leaves the context usable); asked for before the bind, it gets them."""
+    w = small_workload(W.WENO5, (40, 33, 24))
+    h = B.from_workload(w)
+    n_fused = h.workspace_bytes()
+    with pytest.raises(B.HydroError):
+        h.set_option("kernel", B.KERNEL_GENERIC)
+    h.step(1e-3, 1)
+    assert h.status() == 0
+    h.close()
+    h2 = B.from_workload(w, kernel=B.KERNEL_GENERIC)
+    assert h2.workspace_bytes() > n_fused
+    h2.step(1e-3, 1)
+    assert h2.status() == 0
+    h2.close()
