@@ -400,13 +400,8 @@ musta_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl,
         }
         issue(g + NG);            // refill the slots just consumed
         if (EPI) {   // a4 of the finished cells (all three axes are active whenever this kernel runs)
-            T w[NW];
-            prim_of_cell(oa, w, flag, A.eos);
-            amax = fmax(amax, fmax((double)w[W_AX], fmax((double)w[W_AX + 1], (double)w[W_AX + 2])));
-            if (second) {
-                prim_of_cell(ob, w, flag, A.eos);
-                amax = fmax(amax, fmax((double)w[W_AX], fmax((double)w[W_AX + 1], (double)w[W_AX + 2])));
-            }
+            amax = fmax(amax, (double)max_speed_of_cell(oa, A.eos, true, true, true, flag));
+            if (second) amax = fmax(amax, (double)max_speed_of_cell(ob, A.eos, true, true, true, flag));
         }
     }
     if (EPI) warp_max_to(amax, &ctl->maxspeed_next_bits, wmask);

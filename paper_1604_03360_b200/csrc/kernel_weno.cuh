@@ -412,9 +412,7 @@ weno_y_kernel(Geom G, StageArgs A, const T* __restrict__ Us, T* Uout, Ctl* ctl, 
         }
         issue(j + D);             // refill the slot just consumed
         if (EPI) {   // stage 3 of a CFL step: a4 of the finished cell (all three axes are active here)
-            T w[NW];
-            prim_of_cell_t<T, EOS>(o, w, flag, A.eos);
-            amax = fmax(amax, fmax((double)w[W_AX], fmax((double)w[W_AX + 1], (double)w[W_AX + 2])));
+            amax = fmax(amax, (double)max_speed_of_cell_t<T, EOS>(o, A.eos, true, true, true, flag));   // (fmax drops a NaN)
         }
     }
     if (EPI) warp_max_to(amax, &ctl->maxspeed_next_bits, wmask);

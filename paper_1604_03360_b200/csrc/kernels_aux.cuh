@@ -59,6 +59,33 @@ __device__ __forceinline__ void prim_of_cell_t(const T u[NF], T w[NW], int& flag
         for (int d = 0; d < 3; ++d) w[W_AX + d] = signal_speed(w[W_V + d], v2, id);
     }
 }
+// a4 of one cell: the largest a_d over the axes flagged active.  For a given state a_d increases with |v_d|
+// (d a_d / d|v_d| = (1 - cs2)(1 - cs (1 - v^2)|v_d| / sqrt(disc)) > 0, because cs2 (1 - v^2) v_d^2 < disc reduces to
+// (1 - v_d^2)(1 - v^2 cs2) > 0), so it is the speed of the axis with the largest |M_d|: one speed, not three.
+template <class T, int EOS>
+__device__ __forceinline__ T max_speed_of_cell_t(const T u[NF], const EosArgs& eos, bool ax, bool ay, bool az,
+                                                 int& flag) {
+    T v2, winv, p, cs2;
+    if (EOS == 1) con2prim_p0(u[0], u[1], u[2], u[3], (T)eos.p0, winv, p, v2, flag);
+    else if (EOS == 2) con2prim_tab(u[0], u[1], u[2], u[3], eos, winv, p, v2, cs2, flag);
+    else con2prim(u[0], u[1], u[2], u[3], winv, p, v2, flag);
+    T m = (T)0;
+    if (ax) m = max_nonneg(m, tabs(u[1]));
+    if (ay) m = max_nonneg(m, tabs(u[2]));
+    if (az) m = max_nonneg(m, tabs(u[3]));
+    if (!(ax || ay || az)) return (T)0;   // no active axis: nothing enters the maximum (a4)
+    const T vd = m * winv;
+    if (EOS == 1) return vd;
+    if (EOS == 2) return signal_speed_cs(vd, v2, cs2);
+    return signal_speed(vd, v2, speed_inv_den(v2));
+}
+template <class T>
+__device__ __forceinline__ T max_speed_of_cell(const T u[NF], const EosArgs& eos, bool ax, bool ay, bool az, int& flag) {
+    if (eos.kind == 1) return max_speed_of_cell_t<T, 1>(u, eos, ax, ay, az, flag);
+    if (eos.kind == 2) return max_speed_of_cell_t<T, 2>(u, eos, ax, ay, az, flag);
+    return max_speed_of_cell_t<T, 0>(u, eos, ax, ay, az, flag);
+}
+
 template <class T>
 __device__ __forceinline__ void prim_of_cell(const T u[NF], T w[NW], int& flag, const EosArgs& eos) {
     if (eos.kind == 1) prim_of_cell_t<T, 1>(u, w, flag, eos);
@@ -241,11 +268,7 @@ __global__ void __launch_bounds__(256) max_speed_kernel(Geom G, const T* __restr
     if (i < G.n[0] && j < G.n[1]) {
         const long long p = G.pidx(i, j, k);
         const T u[NF] = {U[p], U[G.fs + p], U[2 * G.fs + p], U[3 * G.fs + p], (T)0};
-        T w[NW];
-        prim_of_cell(u, w, flag, eos);
-        if (G.g[0]) m = fmax(m, (double)w[W_AX]);
-        if (G.g[1]) m = fmax(m, (double)w[W_AX + 1]);
-        if (G.g[2]) m = fmax(m, (double)w[W_AX + 2]);
+        m = (double)max_speed_of_cell(u, eos, G.g[0] > 0, G.g[1] > 0, G.g[2] > 0, flag);
     }
     if (flag) ctl->flag = 1;
     block_max_to_ctl(m, ctl);
