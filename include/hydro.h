@@ -151,6 +151,31 @@ int hydro_step_cfl_batch(hydro_ctx **ctxs, int nctx, double cfl, int nsteps);
  * Writes one double to a HOST pointer; synchronises the stream. */
 int hydro_max_signal_speed(hydro_ctx *ctx, double *out_host);
 
+/* The same maximum for callers that cannot give the library any device memory.  Every other compute call works in the
+ * workspace of hydro_bind_workspace, which somebody had to allocate.  That is not always possible: a time-step or
+ * monitoring hook called from inside another code's event loop with a state it does not own; a process in which a
+ * framework's memory pool holds all of the device memory and is at its cap; a latency-bound loop where cudaMalloc is
+ * ruled out because it synchronises the whole device (every other event's stream would stall).  This call needs NO
+ * workspace (the context may be unbound; only its grid size, "precision", equation-of-state options and stream are
+ * used) and calls no cudaMalloc, cudaFree or other allocating routine: the reduction's scratch is an array built into
+ * the library image, 512.25 KiB, which every GPU that loads the library holds until the process exits.
+ *   cons_device          the INTERIOR state [5][nz][ny][nx] in device memory, element type per "precision" (read only)
+ *   maxspeed_device_out  ONE double in device memory on the same GPU; written asynchronously on the context's stream
+ *                        (a grid with no active axis gives 0)
+ * Limit: the array holds one double per tile of 64 x 4 x 1 cells, at most 65536 tiles, i.e.
+ * ceil(nx/64) * ceil(ny/4) * nz <= 65536 (256^3 is the largest cube).  Larger grids are refused with EINVAL and a text
+ * that says so; they need hydro_max_signal_speed and a workspace.
+ * Sharing: there is ONE such array per GPU and every call uses it.  Calls on the same GPU must therefore not overlap
+ * in time on the device: issue them on one stream, or order the streams with events; two calls in flight at once
+ * race on the array and both results are undefined.  Nothing the array held before a call is used: each call
+ * zeroes the ticket counter on the stream before its kernel and overwrites the tile values it reads.
+ * First call on a GPU: looks the array's device address up (cudaGetSymbolAddress, once per GPU, which also makes the
+ * runtime load the library's kernels there).  Make that first call during set-up, outside any stream capture.
+ * Clamped (unphysical) cells enter with their clamped speed; this call raises no flag (it has no control block).
+ * EINVAL: null pointer, grid beyond the limit, pointers that are not device memory of one GPU.  ECUDA: a runtime call
+ * or the launch failed.  (a3-a4 of DESIGN.md section 2; reading Q10.) */
+int hydro_max_signal_speed_static(hydro_ctx *ctx, const void *cons_device, void *maxspeed_device_out);
+
 /* L(u) of Eq. (2) for a caller-supplied interior state (DEVICE pointers, same layout as the state)
  * with ghosts filled at time t_stage: one Runge-Kutta stage's spatial operator, for per-stage parity.
  * Uses the RK stage buffers as scratch; the context's own state u^n is left untouched. */

@@ -23,7 +23,8 @@ LIB_PATH = os.path.join(_HERE, "libhydro_b200.so")
 SYMBOLS = [
     "hydro_create", "hydro_set_option", "hydro_set_stream", "hydro_workspace_bytes", "hydro_bind_workspace",
     "hydro_set_state", "hydro_get_state", "hydro_set_state_host", "hydro_get_state_host", "hydro_step",
-    "hydro_step_cfl", "hydro_step_cfl_batch", "hydro_set_eos_table", "hydro_max_signal_speed", "hydro_eval_L", "hydro_get_time", "hydro_status",
+    "hydro_step_cfl", "hydro_step_cfl_batch", "hydro_set_eos_table", "hydro_max_signal_speed",
+    "hydro_max_signal_speed_static", "hydro_eval_L", "hydro_get_time", "hydro_status",
     "hydro_launch_count", "hydro_stage_kernel_time", "hydro_last_error",
     "hydro_zhalo_elems", "hydro_get_zhalo", "hydro_put_zhalo", "hydro_step_stage", "hydro_local_max_speed",
     "hydro_step_stage_cfl", "hydro_step_stage_overlap", "hydro_destroy",
@@ -58,6 +59,7 @@ def _load():
     L.hydro_step_cfl_batch.argtypes = [ctypes.POINTER(vp), i32, dbl, i32]
     L.hydro_set_eos_table.argtypes = [vp, vp, i32, dbl, dbl]
     L.hydro_max_signal_speed.argtypes = [vp, pd]
+    L.hydro_max_signal_speed_static.argtypes = [vp, vp, vp]
     L.hydro_eval_L.argtypes = [vp, vp, dbl, vp]
     L.hydro_get_time.argtypes = [vp, pd]
     L.hydro_status.argtypes = [vp]
@@ -163,6 +165,15 @@ class Hydro:
         v = ctypes.c_double()
         self._check(lib.hydro_max_signal_speed(self._h, ctypes.byref(v)))
         return v.value
+
+    def max_signal_speed_static(self, cons, out):
+        """hydro_max_signal_speed_static: max signal speed of the interior state `cons` into the 1-element float64
+        device tensor `out`, asynchronously, with no workspace (the context need not be bound) and no allocation here
+        or in the library: for callers that cannot allocate device memory (see include/hydro.h).  Grids up to
+        ceil(nx/64) * ceil(ny/4) * nz = 65536 tiles; calls on one GPU must not overlap."""
+        assert out.is_cuda and out.dtype == torch.float64 and out.numel() == 1 and out.device == cons.device
+        self._check(lib.hydro_max_signal_speed_static(self._h, self._dev(cons), out.data_ptr()))
+        return out
 
     def eval_L(self, cons, t_stage=0.0, out=None):
         if out is None:

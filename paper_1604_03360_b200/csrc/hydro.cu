@@ -9,6 +9,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -893,3 +894,150 @@ int hydro_status(hydro_ctx* c) {
 }
 
 }  // extern "C"
+
+// ================================================================================================
+// hydro_max_signal_speed_static -- the max signal speed (a3-a4) for callers that may not allocate device memory.
+//
+// Everything above works in memory the caller hands over (hydro_bind_workspace); the reduction of
+// hydro_max_signal_speed keeps its accumulator in that workspace.  Some callers have no workspace to give and cannot
+// get one: a monitoring or time-step hook that runs inside someone else's event loop and is handed a state it does
+// not own, a process whose device memory is wholly owned by a framework's pool that is already at its cap, or a
+// latency-bound loop in which cudaMalloc is off limits because it synchronises the whole device and would stall the
+// other events' streams.  For them this entry point reduces in a fixed array that is part of the library's own
+// image: `static_scratch` below, 256 B of header + one double per tile of 64 x 4 x 1 cells, 512.25 KiB in all.
+// Every GPU that loads the library holds that array until the process exits, which is why it is kept small; the price
+// is the size limit STATIC_MAX_TILES (256^3 is the largest cube).
+//
+// Variant of max_speed_kernel: the same per-cell function, but every block stores the maximum of its tile in the
+// scratch array and takes a ticket; the block that draws the last ticket reduces the tiles' values, writes the
+// caller's output and puts the ticket counter back to zero.  No atomics on doubles, no workspace, no control block.
+namespace {
+
+constexpr unsigned STATIC_TILE_X = 64, STATIC_TILE_Y = 4;
+constexpr unsigned STATIC_MAX_TILES = 65536;
+constexpr size_t STATIC_HEAD = 256;   // [0] ticket counter (unsigned), rest unused
+constexpr size_t STATIC_BYTES = STATIC_HEAD + (size_t)STATIC_MAX_TILES * sizeof(double);
+
+// In host code this name is only a handle for cudaGetSymbolAddress (a kernel given `static_scratch` itself would be
+// given a host address); static_scratch_on() below turns it into the array's address on one device.
+static __device__ __align__(256) unsigned char static_scratch[STATIC_BYTES];
+
+// block-wide max of a non-negative value; the result is valid in thread 0
+__device__ __forceinline__ double block_max_static(double m, double* smax) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    const int tid = threadIdx.x;
+    __syncthreads();   // smax may still be read from a previous use
+    if ((tid & 31) == 0) smax[tid >> 5] = m;
+    __syncthreads();
+    if (tid < 32) {
+        m = tid < (int)(blockDim.x >> 5) ? smax[tid] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    }
+    return m;
+}
+
+// cons: the caller's INTERIOR state [5][nz][ny][nx] (no ghosts, no padding).  One block of 256 threads per tile;
+// tiles numbered x fastest, then y, then z.
+template <class T>
+__global__ void __launch_bounds__(256) max_speed_static_kernel(int nx, int ny, int nz, unsigned tiles_x, unsigned tiles_y,
+                                                               const T* __restrict__ cons, EosArgs eos,
+                                                               unsigned char* scratch, double* __restrict__ out) {
+    __shared__ double smax[8];
+    __shared__ bool last;
+    unsigned* ticket = reinterpret_cast<unsigned*>(scratch);
+    double* tile_max = reinterpret_cast<double*>(scratch + STATIC_HEAD);
+    const unsigned tile = blockIdx.x, ntiles = gridDim.x;
+    const unsigned bx = tile % tiles_x, by = (tile / tiles_x) % tiles_y;
+    const int k = (int)(tile / (tiles_x * tiles_y));
+    const int i = (int)(bx * STATIC_TILE_X + (threadIdx.x % STATIC_TILE_X));
+    const int j = (int)(by * STATIC_TILE_Y + (threadIdx.x / STATIC_TILE_X));
+    double m = 0.0;
+    if (i < nx && j < ny) {
+        const long long N = (long long)nx * ny * nz;
+        const long long q = ((long long)k * ny + j) * nx + i;
+        const T u[NF] = {cons[q], cons[N + q], cons[2 * N + q], cons[3 * N + q], (T)0};
+        int flag = 0;   // a clamped cell enters with its clamped speed; this call has no status word to raise
+        m = (double)max_speed_of_cell(u, eos, nx > 1, ny > 1, nz > 1, flag);
+    }
+    m = block_max_static(m, smax);
+    if (threadIdx.x == 0) {
+        tile_max[tile] = m;
+        __threadfence();   // the tile's value is visible before the ticket is
+        last = atomicAdd(ticket, 1u) == ntiles - 1;
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    double r = 0.0;
+    for (unsigned b = threadIdx.x; b < ntiles; b += blockDim.x) r = fmax(r, __ldcg(tile_max + b));
+    r = block_max_static(r, smax);
+    if (threadIdx.x == 0) {
+        *out = r;
+        *ticket = 0u;   // the next call on this device starts from zero again
+    }
+}
+
+// Address of static_scratch on `device`, which must be the current device.  Looked up once per device.
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex static_mu;
+unsigned char* static_ptr[STATIC_MAX_DEVICES] = {};
+
+cudaError_t static_scratch_on(int device, unsigned char** p) {
+    std::lock_guard<std::mutex> lock(static_mu);
+    if (static_ptr[device] == nullptr) {
+        void* a = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&a, static_scratch);
+        if (e != cudaSuccess) return e;
+        static_ptr[device] = static_cast<unsigned char*>(a);
+    }
+    *p = static_ptr[device];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int hydro_max_signal_speed_static(hydro_ctx* c, const void* cons_device, void* maxspeed_device_out) {
+    if (!c) return HYDRO_EINVAL;
+    if (!cons_device || !maxspeed_device_out) return fail(c, HYDRO_EINVAL, "hydro_max_signal_speed_static: null pointer");
+    const unsigned long long tx = ((unsigned)c->n[0] + STATIC_TILE_X - 1) / STATIC_TILE_X;
+    const unsigned long long ty = ((unsigned)c->n[1] + STATIC_TILE_Y - 1) / STATIC_TILE_Y;
+    const unsigned long long tiles = tx * ty * (unsigned long long)c->n[2];
+    if (tiles > STATIC_MAX_TILES)
+        return fail(c, HYDRO_EINVAL,
+                    "hydro_max_signal_speed_static: a %d x %d x %d grid is %llu tiles of %u x %u x 1 cells, the built-in "
+                    "scratch array holds %u (e.g. 256^3); use hydro_max_signal_speed with a workspace",
+                    c->n[0], c->n[1], c->n[2], tiles, STATIC_TILE_X, STATIC_TILE_Y, STATIC_MAX_TILES);
+    cudaPointerAttributes ai, ao;
+    if (cudaPointerGetAttributes(&ai, cons_device) != cudaSuccess || ai.type != cudaMemoryTypeDevice ||
+        cudaPointerGetAttributes(&ao, maxspeed_device_out) != cudaSuccess || ao.type != cudaMemoryTypeDevice ||
+        ai.device != ao.device) {
+        cudaGetLastError();
+        return fail(c, HYDRO_EINVAL, "hydro_max_signal_speed_static: state and output must be CUDA device memory of one GPU");
+    }
+    const int dev = ai.device;
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return fail(c, HYDRO_EINVAL, "hydro_max_signal_speed_static: device %d", dev);
+    // run on the device that holds the state; the caller's current device is put back on return
+    int prev = -1;
+    CUDA_OK(c, cudaGetDevice(&prev));
+    struct Back {
+        int prev, dev;
+        ~Back() { if (prev != dev) cudaSetDevice(prev); }
+    } back{prev, dev};
+    if (prev != dev) CUDA_OK(c, cudaSetDevice(dev));
+    unsigned char* scratch = nullptr;
+    CUDA_OK(c, static_scratch_on(dev, &scratch));
+    // the ticket counter must start at zero even if an earlier call on this device never finished
+    CUDA_OK(c, cudaMemsetAsync(scratch, 0, STATIC_HEAD, c->stream));
+    if (c->precision == HYDRO_F64)
+        max_speed_static_kernel<double><<<(unsigned)tiles, 256, 0, c->stream>>>(
+            c->n[0], c->n[1], c->n[2], (unsigned)tx, (unsigned)ty, (const double*)cons_device, c->eos, scratch,
+            (double*)maxspeed_device_out);
+    else
+        max_speed_static_kernel<float><<<(unsigned)tiles, 256, 0, c->stream>>>(
+            c->n[0], c->n[1], c->n[2], (unsigned)tx, (unsigned)ty, (const float*)cons_device, c->eos, scratch,
+            (double*)maxspeed_device_out);
+    LAUNCHED(c, "max_speed_static_kernel");
+    return HYDRO_OK;
+}
