@@ -164,6 +164,10 @@ class SlabGroup:
 def make_slab(binding, w, k0, k1, precision=0, device="cuda"):
     """Context for the z-range [k0, k1) of a workloads.Workload, bc_z = BC_EXTERNAL, state uploaded."""
     import numpy as np
+    if binding.BC_HUBBLE in tuple(w.bc):
+        # the closed-form ghosts need every Hubble axis and the slab's z position; the library refuses the
+        # combination with bc_z = BC_EXTERNAL at step time, this says so before anything is uploaded
+        raise ValueError("the slab decomposition does not support BC_HUBBLE (analytic ghost fill): %r" % (w.bc,))
     h = binding.Hydro(w.n[0], w.n[1], k1 - k0, w.dx, w.scheme, precision=precision, device=device)
     h.set_option("bc_x", w.bc[0])
     h.set_option("bc_y", w.bc[1])

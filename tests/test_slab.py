@@ -259,3 +259,40 @@ def _ring_of_one(B, scheme):
         assert torch.equal(h.get_state(), want)
         assert h.status() == 0
         h.close()
+
+
+def test_make_slab_refuses_the_analytic_ghost_fill():
+    """BC_HUBBLE needs all its axes and the slab's z position; a slab would get silently wrong ghosts."""
+    class FakeBinding:
+        BC_HUBBLE, BC_EXTERNAL = 2, 3
+
+        def Hydro(self, *a, **k):
+            raise AssertionError("the check comes before the context is made")
+    w = W.hubble(n=8)
+    assert W.BC_HUBBLE in w.bc
+    with pytest.raises(ValueError, match="BC_HUBBLE"):
+        S.make_slab(FakeBinding(), w, 0, 4)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("scheme", [W.WENO5, W.MUSTA_FORCE])
+def test_library_refuses_hubble_ghosts_on_a_slab(scheme):
+    """The same rule inside the library: every stepping call of a context with bc_z = EXTERNAL and a Hubble axis
+    returns EINVAL, and the plain combination still runs."""
+    import torch
+    from paper_1604_03360_b200 import binding as B
+    h = B.Hydro(16, 16, 16, 0.1, scheme, bc_x=B.BC_HUBBLE, bc_y=B.BC_OUTFLOW, bc_z=B.BC_EXTERNAL).bind()
+    cons = torch.from_numpy(W.random_state((16, 16, 16), seed=3)).cuda().contiguous()
+    h.set_state(cons)
+    a = torch.ones(1, dtype=torch.float64, device="cuda")
+    for call in (lambda: h.step_stage(0.01, 0), lambda: h.step_stage_cfl(0.2, 0, a),
+                 lambda: h.step_stage_overlap(0.2, 0, a, None, None), lambda: h.step(0.01), lambda: h.eval_L(cons)):
+        with pytest.raises(B.HydroError) as e:
+            call()
+        assert e.value.code == B.EINVAL and "HYDRO_BC_HUBBLE" in str(e.value)
+    h.set_option("bc_x", B.BC_PERIODIC)
+    h.put_zhalo(0, 0, None)
+    h.put_zhalo(0, 1, None)
+    h.step_stage(0.01, 0)          # accepted (the rough random state may raise the clamp flag: not the point here)
+    torch.cuda.synchronize()
+    h.close()
