@@ -6,8 +6,9 @@ BASELINE.json configs[4]: the 512^3 periodic lumpy state with 200 hotspots and b
                     [--grid 512] [--no-variants] [--no-cpu-baseline] [--impl reference]
 
 One "step" is one SSP-RK3 step of the whole grid with dt = CFL dx / max signal speed taken on the device
-(hydro_step_cfl, reading Q10): per stage the ghost fill, the x/z marching kernel and the y sweep, whose epilogue
-also does con2prim + signal speeds + the CFL max for the next stage.
+(hydro_step_cfl, reading Q10): per stage the ghost fill, the x/z marching kernel and the y sweep; both make con2prim
+and the signal speeds of the cells they read on the fly, and the stage-3 y sweep's epilogue reduces the CFL maximum
+of the new state for the next step.
 Prints ONE JSON line (rank 0).  N > 1 (torchrun): ONE 512^3 event decomposed into z-slabs with a halo exchange per
 Runge-Kutta stage (`--decomp slab`, the default for N > 1: SURVEY 8(e), strong scaling), time = max over ranks; the
 throughput of N independent events (`--decomp events`, weak scaling, no data-path collective) is printed beside it

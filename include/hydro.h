@@ -62,7 +62,8 @@ enum {
  * active axis shorter than the ghost width. */
 int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme);
 
-/* Set an option.  Must precede hydro_bind_workspace for "precision" (it changes the workspace size).
+/* Set an option.  "precision" and "kernel" = HYDRO_KERNEL_GENERIC must precede hydro_bind_workspace (both change the
+ * workspace size; EINVAL afterwards).
  *   "precision"     HYDRO_F64 (default) | HYDRO_F32: arithmetic and storage type of the whole path
  *   "bc_x|bc_y|bc_z" boundary rule per axis (default outflow = copy the nearest interior cell)
  *   "weno_eps"      epsilon of the WENO weights (default 1e-6, reading Q5; EINVAL below 1e-40: the weights are
@@ -86,10 +87,11 @@ int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme)
  *                   launch, read back with hydro_stage_kernel_time
  *   "graph"         0 (default) | 1: hydro_step_cfl replays one steady-state step from a CUDA graph (one
  *                   cudaGraphLaunch instead of 11 kernel launches per step; every step-dependent value, dt included,
- *                   lives in the device control block).  Needs a non-default stream (hydro_set_stream); on the
- *                   legacy default stream, with "profile" on, or before the first plain step has left the
- *                   primitives and the max signal speed behind, the plain launches run instead.  The graphs are
- *                   dropped whenever an option, the stream or the workspace changes.
+ *                   lives in the device control block).  Needs a non-default stream (hydro_set_stream) and the
+ *                   marching kernels; on the legacy default stream, with "profile" on, or while the control block
+ *                   does not yet hold the max signal speed of u^n (i.e. before the stage-3 epilogue of a first plain
+ *                   step, or hydro_max_signal_speed, has left it there) the plain launches run instead.  The
+ *                   graphs are dropped whenever an option, the stream or the workspace changes.
  *   "kernel"        HYDRO_KERNEL_AUTO (default: the marching stage kernels where all three axes are active,
  *                   else the generic one-thread-per-cell kernel) | HYDRO_KERNEL_GENERIC | HYDRO_KERNEL_FUSED
  *                   (= marching; EINVAL at step time if the grid does not allow it)
@@ -100,9 +102,10 @@ int hydro_set_option(hydro_ctx *ctx, const char *key, double value);
  * legacy default stream. */
 int hydro_set_stream(hydro_ctx *ctx, void *cuda_stream);
 
-/* Bytes of device memory the context needs for its padded state copies (three: u^n and two RK stage
- * buffers, five arrays each), two copies of the seven per-cell primitive arrays (v_x, v_y, v_z, p, a_x, a_y, a_z)
- * and a 256-byte control block. */
+/* Bytes of device memory the context needs: a 256-byte control block and three padded states (u^n and two RK stage
+ * buffers, five arrays each).  The marching kernels make their primitives on the fly and keep none in memory; only
+ * where the generic kernel can run ("kernel" = HYDRO_KERNEL_GENERIC, or a grid with an inactive axis) ONE set of the
+ * seven per-cell primitive arrays (v_x, v_y, v_z, p, a_x, a_y, a_z) is added.  Depends on "precision" and "kernel". */
 size_t hydro_workspace_bytes(const hydro_ctx *ctx);
 
 /* Hand the context its device memory (256-byte aligned, at least hydro_workspace_bytes()).  The caller
@@ -127,9 +130,9 @@ int hydro_get_state_host(hydro_ctx *ctx, void *cons_host_out);
  * signal speeds, L(u) of Eq. (2) fused with the Runge-Kutta combination).  Asynchronous. */
 int hydro_step(hydro_ctx *ctx, double dt, int nsteps);
 
-/* The same with dt = cfl * dx / (max signal speed of the state at the start of each step), the
- * maximum taken on the device by the stage-1 con2prim kernel: no host synchronisation (reading Q10).
- * Asynchronous. */
+/* The same with dt = cfl * dx / (max signal speed of the state at the start of each step), the maximum taken on the
+ * device: by the stage-3 epilogue of the previous step's y sweep (marching kernels), else by a reduction pass before
+ * stage 1 (first step after hydro_set_state, generic kernel).  No host synchronisation (reading Q10).  Asynchronous. */
 int hydro_step_cfl(hydro_ctx *ctx, double cfl, int nsteps);
 
 /* Tabulated barotropic equation of state p(e) (the quark-gluon-plasma physics the solver
@@ -138,7 +141,8 @@ int hydro_step_cfl(hydro_ctx *ctx, double cfl, int nsteps);
  * linearly in e (the first and last segments are continued beyond the table), c_s^2 = dp/de is the segment's slope;
  * conserved -> primitive solves E - M^2/(E + p(e)) - e = 0 by Newton's iteration, the characteristic speeds use the
  * state's own c_s^2.  Selects option "eos" = 2 ("eos" = 0 / 1 switches back; "eos" = 2 re-selects the table).
- * EINVAL: null or non-device pointer, n < 2, e_max <= e_min. */
+ * EINVAL: null or non-device pointer, n < 2, e_max <= e_min, or a table on another GPU than the bound workspace
+ * (checked here if the workspace is bound already, else by hydro_bind_workspace). */
 int hydro_set_eos_table(hydro_ctx *ctx, const void *p_device, int n, double e_min, double e_max);
 
 /* Event-by-event batches ("event-by-event simulations"): advance nctx independent
@@ -195,7 +199,9 @@ long long hydro_launch_count(const hydro_ctx *ctx);
  * such a buffer into the g GHOST planes of `side`.  hydro_step_stage runs ONE stage (0, 1, 2, in this order)
  * of a step of size dt: x/y ghost fill, the stage kernels; stage 2 also advances the time.  A driver advances
  * a slab as: for s in 0..2 { get both halos of buffer s, exchange with the neighbours, put, step_stage(dt, s) }.
- * All asynchronous on the stream. */
+ * All asynchronous on the stream.  The analytic ghost fill is not carried by the decomposition: with bc_z =
+ * HYDRO_BC_EXTERNAL and HYDRO_BC_HUBBLE on x or y every stepping call returns EINVAL (the closed form needs all
+ * Hubble axes and the slab's position along z). */
 size_t hydro_zhalo_elems(const hydro_ctx *ctx);
 int hydro_get_zhalo(hydro_ctx *ctx, int buffer, int side, void *packed_device_out);
 int hydro_put_zhalo(hydro_ctx *ctx, int buffer, int side, const void *packed_device_in);

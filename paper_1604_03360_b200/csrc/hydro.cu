@@ -48,6 +48,7 @@ struct hydro_ctx {
     bool max_ready = false;                     // ctl->maxspeed_bits holds the max signal speed of u^n (stage-3 epilogue)
     int stage_open = 0;                         // stages of a hydro_step_stage sequence done so far (0 = between steps)
     int device = -1;                            // CUDA device of the workspace (captured at bind)
+    int eos_device = -1;                        // CUDA device of the tabulated closure's table (hydro_set_eos_table)
     int zc = 0, yc = 0;                         // chunk lengths of the z / y march ("tile_zc", "sweep_zc"; 0 = default)
     bool fused_ready = false;                   // the marching kernels' shared-memory attributes are set
     char plan_err[256] = {0};
@@ -163,6 +164,12 @@ int do_halo(hydro_ctx* c, T* pad, double tfrac, bool use_abs, double t_abs) {
     A.H = c->H;
     A.H.dx = c->dx;
     A.eos = c->eos;
+    // The closed-form Hubble ghosts are a function of ALL the Hubble axes and of the slab's own position.  Under
+    // bc_z = EXTERNAL the z axis would drop out of the closed form (wrong exponent, z^2 missing from tau^2, M_z = 0),
+    // the slab's z origin is not shifted, and the physical z ends would get zero-gradient planes: refused.
+    if (c->bc[2] == HYDRO_BC_EXTERNAL && (c->bc[0] == HYDRO_BC_HUBBLE || c->bc[1] == HYDRO_BC_HUBBLE))
+        return fail(c, HYDRO_EINVAL, "HYDRO_BC_HUBBLE on x or y cannot be combined with bc_z = HYDRO_BC_EXTERNAL "
+                                     "(the slab decomposition does not carry the analytic ghost fill)");
     if (total == 0) return HYDRO_OK;
     const int tb = 256;
     halo_fill_kernel<T><<<(unsigned)((total + tb - 1) / tb), tb, 0, c->stream>>>(c->G, A, c->ctl, tfrac, t_abs,
@@ -588,6 +595,8 @@ int hydro_bind_workspace(hydro_ctx* c, void* p, size_t bytes) {
         cudaGetLastError();
         return fail(c, HYDRO_EINVAL, "workspace is not CUDA device memory");
     }
+    if (c->eos.tab != nullptr && c->eos_device != attr.device)
+        return fail(c, HYDRO_EINVAL, "workspace on GPU %d, equation-of-state table on GPU %d", attr.device, c->eos_device);
     c->device = attr.device;
     DeviceGuard dg(c);
     c->ws = p;
@@ -705,7 +714,10 @@ int hydro_set_eos_table(hydro_ctx* c, const void* p_device, int n, double e_min,
         cudaGetLastError();
         return fail(c, HYDRO_EINVAL, "hydro_set_eos_table: the table is not CUDA device memory");
     }
+    if (c->ws != nullptr && attr.device != c->device)
+        return fail(c, HYDRO_EINVAL, "hydro_set_eos_table: the table is on GPU %d, the workspace on GPU %d", attr.device, c->device);
     drop_graphs(c);
+    c->eos_device = attr.device;
     c->eos.tab = (const double*)p_device;
     c->eos.n = n;
     c->eos.e_min = e_min;

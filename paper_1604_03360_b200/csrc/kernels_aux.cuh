@@ -226,7 +226,7 @@ __device__ __forceinline__ void block_max_to_ctl(double m, Ctl* ctl) {
 
 // (a) con2prim + signal speeds over the padded array (face ghosts included, edge/corner ghosts
 // skipped), a2-a3; the max over INTERIOR cells and ACTIVE axes (a4) is reduced when do_max != 0.
-// Writes W = (winv, p, a_x, a_y, a_z).
+// Writes the seven arrays W = (v_x, v_y, v_z, p, a_x, a_y, a_z) that the generic kernel reads.
 template <class T>
 __global__ void __launch_bounds__(256) prim_kernel(Geom G, const T* __restrict__ U, T* __restrict__ W,
                                                    Ctl* ctl, int do_max, EosArgs eos) {
