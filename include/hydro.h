@@ -68,7 +68,10 @@ int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme)
  *   "bc_x|bc_y|bc_z" boundary rule per axis (default outflow = copy the nearest interior cell)
  *   "weno_eps"      epsilon of the WENO weights (default 1e-6, reading Q5; EINVAL below 1e-40: the weights are
  *                   evaluated cross-multiplied, which takes epsilon to the 6th power.  For the same reason fp64
- *                   data must stay below about 1e25 in magnitude; the fp32 path rescales and has no such limit)
+ *                   data must stay below about 1e25 in magnitude.  The fp32 path rescales its indicators by a power of
+ *                   two, so its bound is the plain overflow of the indicators themselves (squares of flux
+ *                   differences, with coefficients of order 1e4 in WENO7): fp32 conserved values must stay below
+ *                   about 1e16 for WENO5 and 1e13 for WENO7; beyond that L(u) is not finite)
  *   "musta_stages"  K of MUSTA-FORCE (default 2, reading Q8);  "musta_cfl" its local Courant number
  *                   (default 0.9, reading Q7)
  *   "eos", "eos_p0" equation of state: 0 (default) p = e/3 (reading Q2); 1 p = eos_p0, a constant (the closure for

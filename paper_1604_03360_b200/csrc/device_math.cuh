@@ -181,23 +181,19 @@ struct EosArgs {
     double e_min, de;
 };
 
-// p and dp/de of the table at energy density e.  The segment index and the slope use true divisions, so that the
-// choice of segment is the one any IEEE evaluation of floor((e - e_min)/de) makes.
-HD void eos_table_lookup(const EosArgs& eos, double e, double& p, double& cs2) {
-    int i = (int)floor((e - eos.e_min) / eos.de);
-    i = i < 0 ? 0 : (i > eos.n - 2 ? eos.n - 2 : i);
-#ifdef __CUDA_ARCH__
-    const double pa = __ldg(eos.tab + i), pb = __ldg(eos.tab + i + 1);
-#else
-    const double pa = eos.tab[i], pb = eos.tab[i + 1];
-#endif
-    cs2 = (pb - pa) / eos.de;
-    p = pa + (e - (eos.e_min + i * eos.de)) * cs2;
-}
-
-// con2prim for the tabulated closure: the energy density solves f(e) = E - M^2/(E + p(e)) - e = 0 with
-// f' = v^2 c_s^2 - 1 < 0; Newton's iteration from e = E until the step falls below 1e-15 e (at most 60 steps), in
-// double whatever T is.  Same outputs and clamp policy (E >= 1e-300, |M| <= (1 - 1e-12) E) as con2prim, plus cs2.
+// con2prim for the tabulated closure (N1).  p(e) is piecewise linear on the knots e_k = e_min + k de, first and last
+// segment continued.  The energy density is the root of
+//     g(e) = (E - e)(E + p(e)) - M^2,
+// which has the sign of E - M^2/(E + p(e)) - e wherever E + p > 0 and, like it, falls through its single root.  On
+// segment k, with x = e - e_k, H_k = E + p_k, D_k = E - e_k and slope c (= c_s^2 of the segment),
+//     g = -c x^2 - B x + g_k,   B = H_k - c D_k = (1 - c) E + p_k + c e_k > 0,   g_k = D_k H_k - M^2 = g(e_k),
+// so the root of the segment's parabola is x = 2 g_k / (B + sqrt(B^2 + 4 c g_k)) in closed form: no iteration on e.
+// What is searched is the segment.  x < 0 says g_k < 0, the root lies below e_k; x >= de says g(e_{k+1}) >= 0, it
+// lies at or above e_{k+1}; either way the bracket [lo, hi] of candidate segments shrinks, and the next candidate is
+// the segment the extrapolated root e_k + x points to (on a smooth table that is the right one or its neighbour),
+// plain bisection of the bracket after 8 such jumps.  At most 8 + log2(n) candidates, typically one or two.
+// All in double whatever T is.  Same outputs and clamp policy (E >= 1e-300, |M| <= (1 - 1e-12) E, reading Q16) as
+// con2prim, plus cs2.  A root within rounding of a knot may take the slope of either neighbour segment.
 template <class T>
 HD void con2prim_tab(T E_, T M0, T M1, T M2, const EosArgs& eos, T& winv, T& p, T& v2, T& cs2, int& flag) {
     double E = (double)E_;
@@ -210,27 +206,41 @@ HD void con2prim_tab(T E_, T M0, T M1, T M2, const EosArgs& eos, T& winv, T& p, 
     const double lim = (1.0 - 1e-12) * E;
     if (!(m2 <= lim * lim)) {
         const double mabs = sqrt(m2);
-        if (!(mabs <= lim)) {
+        if (!(mabs <= lim)) {   // NaN momentum lands here too
             sc = lim / mabs;
             m2 = lim * lim;
             flag = 1;
         }
     }
-    double e = E, pe = 0.0, c2 = 0.0;
-    for (int it = 0; it < 60; ++it) {
-        eos_table_lookup(eos, e, pe, c2);
-        const double H = E + pe;
-        const double f = E - m2 / H - e;
-        const double fp = m2 * c2 / (H * H) - 1.0;
-        const double en = e - f / fp;
-        const bool done = fabs(en - e) <= 1e-15 * fabs(en);
-        e = en;
-        if (done) break;
+    const double de = eos.de, inv_de = 1.0 / de;
+    int lo = 0, hi = eos.n - 2;
+    double t = (E - eos.e_min) * inv_de;   // first candidate: the segment of e = E (the root is at or below E)
+    double pk = 0.0, c = 0.0, x = 0.0;
+    for (int it = 0; it < 96; ++it) {
+        const int k = t >= (double)hi ? hi : (t > (double)lo ? (int)t : lo);   // a NaN picks lo
+#ifdef __CUDA_ARCH__
+        pk = __ldg(eos.tab + k);
+        const double pn = __ldg(eos.tab + k + 1);
+#else
+        pk = eos.tab[k];
+        const double pn = eos.tab[k + 1];
+#endif
+        const double ek = fma((double)k, de, eos.e_min);
+        c = (pn - pk) * inv_de;
+        const double Hk = E + pk, Dk = E - ek;
+        const double gk = fma(Dk, Hk, -m2);
+        const double B = fma(-c, Dk, Hk);
+        const double disc = fma(B, B, 4.0 * c * gk);
+        x = 2.0 * gk / (B + sqrt(disc > 0.0 ? disc : 0.0));
+        if (x < 0.0 && k > lo) hi = k - 1;
+        else if (x >= de && k < hi) lo = k + 1;
+        else break;   // the root lies on this segment (or on the continued end segment)
+        t = it < 8 ? (ek + x - eos.e_min) * inv_de : (double)((lo + hi) >> 1);
     }
-    eos_table_lookup(eos, e, pe, c2);
+    const double pe = fma(c, x, pk);
     const double w = 1.0 / (E + pe);
     p = (T)pe;
-    cs2 = (T)c2;
+    cs2 = (T)c;
     v2 = (T)(m2 * w * w);
     winv = (T)(w * sc);
 }
@@ -282,7 +292,9 @@ HD void normalise_indicators(T (&B)[NB]) {}
 template <>
 __device__ __forceinline__ void normalise_indicators<float, 3>(float (&B)[3]) {
     const float m = fminf(B[0], fminf(B[1], B[2]));
-    const float s = __int_as_float(0x7f000000 - (__float_as_int(m) & 0x7f800000));   // 2^(127 - exponent(m)) / 2^0
+    // 2^(127 - exponent(m)); the exponent field is held at 253 so that s stays a normal positive number when the
+    // smallest indicator is 2^127 or beyond (or Inf): s = 0 would zero every B_k and N / D would be 0 / 0
+    const float s = __int_as_float(0x7f000000 - min(__float_as_int(m) & 0x7f800000, 0x7e800000));
     // WENO5 takes B only to the 4th power: the clamp can sit at 2^25 (products below 2^100)
     const float cap = 33554432.0f;   // 2^25
 #pragma unroll
@@ -291,7 +303,7 @@ __device__ __forceinline__ void normalise_indicators<float, 3>(float (&B)[3]) {
 template <>
 __device__ __forceinline__ void normalise_indicators<float, 4>(float (&B)[4]) {
     const float m = fminf(fminf(B[0], B[1]), fminf(B[2], B[3]));
-    const float s = __int_as_float(0x7f000000 - (__float_as_int(m) & 0x7f800000));
+    const float s = __int_as_float(0x7f000000 - min(__float_as_int(m) & 0x7f800000, 0x7e800000));
     const float cap = 131072.0f;     // 2^17
 #pragma unroll
     for (int k = 0; k < 4; ++k) B[k] = fminf(B[k] * s, cap);

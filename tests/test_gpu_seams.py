@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 
 from paper_1604_03360_b200 import workloads as W
-from test_gpu_parity import SCHEMES, TOL_STAGE, reldiff, small_workload, to_dev, _crop_periodic
+from test_gpu_parity import SCHEMES, TOL_100_F32, TOL_STAGE, reldiff, small_workload, to_dev, _crop_periodic
 
 pytestmark = pytest.mark.gpu
 
@@ -214,6 +214,28 @@ def test_tabulated_eos_matches_the_oracle(B, oracle, scheme, kernel):
     hg.close()
 
 
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_tabulated_eos_fp32_against_the_fp64_oracle(B, oracle, scheme):
+    """Reading Q17 for the tabulated closure: the fp32 kernels, whose table con2prim runs in double
+    on float inputs, against the fp64 oracle: L(u) and the state after ten steps."""
+    n = (45, 23, 38)
+    w0 = small_workload(scheme, n)
+    tab = W.crossover_eos_table(n=2048, e_max=float(np.max(w0.cons[0])) * 1.5)
+    w = W.Workload("xover32", n, w0.dx, (0, 0, 0), scheme, (W.BC_PERIODIC, W.BC_OUTFLOW, W.BC_PERIODIC), w0.cons, 0.0,
+                   cfl=0.2, nsteps=10, eos_table=tab)
+    o = oracle.from_workload(w)
+    h = B.from_workload(w, precision=1)
+    scale = np.max(np.abs(w.cons[0])) / w.dx
+    Lo = o.eval_L(w.cons)
+    Lg = h.eval_L(to_dev(B, w.cons, h.dtype)).double().cpu().numpy()
+    assert reldiff(Lg, Lo, scale=scale) <= 3e-5
+    for dt in oracle.run(o, w):
+        h.step(dt, 1)
+    assert reldiff(h.get_state().double().cpu().numpy(), o.get_state()) <= TOL_100_F32
+    assert h.status() == 0
+    h.close()
+
+
 def test_eos_table_arguments_are_checked(B):
     import torch
     h = B.Hydro(16, 16, 16, 0.1, W.WENO5)
@@ -251,6 +273,16 @@ def test_fp32_weno_weights_survive_any_data_scale(B, oracle, scheme, scale, eps)
     assert reldiff(Lg, Lo, scale=np.max(np.abs(cons[0])) / w.dx) <= 3e-5
     assert h.status() == 0
     h.close()
+
+
+@pytest.mark.parametrize("scheme,scale", [(W.WENO5, 1e16), (W.WENO7, 1e13)])
+def test_fp32_data_bound_stated_in_the_header(B, oracle, scheme, scale):
+    """include/hydro.h gives the fp32 path a data bound (the rescaled weights have no limit of their
+    own, but the indicators -- squares of flux differences, with coefficients of order 1e4 in WENO7 -- overflow
+    fp32): conserved values up to about 1e16 (WENO5) / 1e13 (WENO7).  The lumpy state times `scale` reaches about ten
+    times that and must still give a finite L(u) that matches the fp64 oracle.  (Measured on the B200: WENO5 fails
+    at scale 1e17, WENO7 at 1e14.)"""
+    test_fp32_weno_weights_survive_any_data_scale(B, oracle, scheme, scale, 1e-6)
 
 
 # ------------------------------------------------------------------ maximum sizes: index arithmetic beyond 2^31 elements
