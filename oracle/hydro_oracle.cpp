@@ -23,7 +23,9 @@
 // Eq. (1) by finite differences, configs 2 and 3 at reduced size, the outflow rule against a by-hand
 // extension, the FORCE flux for unequal velocities from its definition, charge advection at measured
 // order 5 / 7 / 2, an isentropic simple wave, mirror / permutation symmetry, the active-axes rule of
-// the CFL maximum and the Q16 clamp values.  No function here is "parity unpinned".
+// the CFL maximum and the Q16 clamp values.  The long-double and float instantiations of the solver
+// (oracle_eval_L_extended, "precision" = 1) are pinned to the fp64 one on rough data with every copied option away
+// from its default (tests/test_oracle_referee.py).  No function here is "parity unpinned".
 //
 // Build: g++ -O2 -std=c++17 -shared -fPIC -ffp-contract=off hydro_oracle.cpp -o liboracle_hydro.so
 // (-ffp-contract=off: no FMA contraction, the arithmetic is exactly what is written).
