@@ -469,13 +469,16 @@ def test_config4_lumpy_musta_full_size_conservation(B):
 
 
 # ------------------------------------------------------------------ several events at once: one context per stream
-def test_two_contexts_on_two_streams_do_not_interfere(B):
+def test_two_contexts_on_two_streams_do_not_interfere(B, oracle):
     """Event-by-event use: independent contexts on their own CUDA streams, launches interleaved from
-    the host, must give exactly what each gives alone."""
+    the host, must give exactly what each gives alone, and what the oracle gives for that event within 1e-10."""
     import torch
     ws = [small_workload(W.WENO5, (45, 23, 70), seed=W.SEED), small_workload(W.MUSTA_FORCE, (45, 23, 70), seed=W.SEED + 1)]
-    alone = []
+    alone, ref_o = [], []
     for w in ws:
+        o = oracle.from_workload(w)
+        oracle.run(o, w, nsteps=4)
+        ref_o.append(o.get_state())
         h = B.from_workload(w)
         h.step_cfl(0.2, 4)
         alone.append(h.get_state().cpu())
@@ -493,8 +496,9 @@ def test_two_contexts_on_two_streams_do_not_interfere(B):
         with torch.cuda.stream(st):
             outs.append(h.get_state())
     torch.cuda.synchronize()
-    for o, a, h in zip(outs, alone, hs):
+    for o, a, h, ro in zip(outs, alone, hs, ref_o):
         assert torch.equal(o.cpu(), a)
+        assert reldiff(o.cpu().numpy(), ro) <= 1e-10
         assert h.status() == 0
         h.close()
 
