@@ -13,7 +13,12 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "hydro_oracle.cpp")
-_LIB = os.path.join(_HERE, "liboracle_hydro.so")
+# ORACLE_SANITIZE=1: build and load a second library compiled with -fsanitize=address,undefined (SURVEY section 5,
+# sanitizers row).  The Python process must then preload the runtimes, e.g.
+#   LD_PRELOAD="$(gcc -print-file-name=libasan.so) $(gcc -print-file-name=libubsan.so)" ASAN_OPTIONS=detect_leaks=0 \
+#   UBSAN_OPTIONS=halt_on_error=1 ORACLE_SANITIZE=1 python -m pytest tests -m "not gpu" -q
+_SANITIZE = os.environ.get("ORACLE_SANITIZE", "") not in ("", "0")
+_LIB = os.path.join(_HERE, "liboracle_hydro_san.so" if _SANITIZE else "liboracle_hydro.so")
 
 OK, EINVAL, EUNPHYSICAL = 0, -1, -4
 
@@ -22,8 +27,10 @@ def build(force: bool = False) -> str:
     """Compile the oracle with g++ (no FMA contraction, -O2).  Returns the library path."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + ".tmp%d" % os.getpid()
-        subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-ffp-contract=off",
-                               _SRC, "-o", tmp])
+        san = ["-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer", "-g"] \
+            if _SANITIZE else []
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-ffp-contract=off"] + san +
+                              [_SRC, "-o", tmp])
         os.replace(tmp, _LIB)
     return _LIB
 
