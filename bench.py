@@ -105,8 +105,14 @@ class ClockSampler:
             for nm, v in zip(names, f[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(nm)
+        hist = {}
+        for v in sm:                                   # SM clock histogram in 50 MHz bins (lower edge -> samples)
+            b = str(int(v // 50 * 50))
+            hist[b] = hist.get(b, 0) + 1
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax,
-                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+                "power_w": float(np.median(power)) if power else None,
+                "power_w_max": max(power) if power else None, "sm_mhz_hist": hist,
+                "samples": len(sm), "reasons": sorted(reasons)}
 
 
 def make_workload(n, scheme, rank=0):
@@ -326,7 +332,8 @@ def roofline(scheme, precision, ncell, stage_ms, stage_n, alu_peak_tf, peaks, pr
 def batch_bench(B, torch, scheme, n=128, nb=8, steps=10, warmup=3):
     """SURVEY 8(f)-N2 / N4 ("event-by-event simulations"): nb independent n^3 events.  (a) one after the
     other on one stream, (b) hydro_step_cfl_batch with one stream per event, (c) the same with every event's step
-    replayed from a CUDA graph.  Whole-batch cell-updates/s, CUDA events around the batch."""
+    replayed from a CUDA graph -- all `steps` steps of an event from ONE graph launch.  Whole-batch cell-updates/s,
+    CUDA events around the batch; host_enqueue_ms_per_step = host time spent issuing the work, per step of the batch."""
     ws = [make_workload(n, scheme, rank=k) for k in range(nb)]
     out = {"grid": [n, n, n], "events": nb, "steps": steps, "unit": UNIT}
     for mode in ("sequential", "streams", "streams+graph"):
@@ -345,13 +352,16 @@ def batch_bench(B, torch, scheme, n=128, nb=8, steps=10, warmup=3):
             else:
                 B.step_cfl_batch(hs, CFL, k)
         advance(warmup)
+        advance(steps)            # untimed: the k-step graph of (c) is captured and instantiated on its first use
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(torch.cuda.default_stream())
         for st in streams:
             st.wait_event(e0)
+        tq = time.perf_counter()
         advance(steps)
+        enqueue_s = time.perf_counter() - tq
         for st in streams:
             torch.cuda.default_stream().wait_stream(st)
         e1.record(torch.cuda.default_stream())
@@ -359,7 +369,8 @@ def batch_bench(B, torch, scheme, n=128, nb=8, steps=10, warmup=3):
         host_s = time.perf_counter() - t0
         ms = e0.elapsed_time(e1)
         out[mode] = {"value": nb * n ** 3 * steps / (ms * 1e-3), "ms_per_step_per_event": ms / steps / nb,
-                     "host_seconds": host_s, "status": max(h.status() for h in hs)}
+                     "host_seconds": host_s, "host_enqueue_ms_per_step": enqueue_s / steps * 1e3,
+                     "status": max(h.status() for h in hs)}
         for h in hs:
             h.close()
         torch.cuda.empty_cache()
@@ -533,6 +544,7 @@ def run_ours(args):
     batch = None
     if not args.no_variants and rank == 0 and world == 1 and not slab_mode:
         batch = batch_bench(B, torch, args.scheme, n=128, nb=8, steps=args.steps)
+        batch["at_64"] = batch_bench(B, torch, args.scheme, n=64, nb=8, steps=args.steps)
 
     # ---- the oracle beside it: bounded sample on the host cores (rank 0, N = 1 only)
     cpu = None
@@ -571,6 +583,15 @@ def run_ours(args):
             "batch": batch,
             "context": "paper: GPU ~200x one CPU thread for MUSTA-FORCE on unnamed 2016 hardware (PAPER.md:38)",
         }
+        # last key, so that a record that keeps only the tail of this line still holds every variant's numbers:
+        # [ms per step, stage-kernel roofline fraction of the nominal peak, median SM MHz, median W]
+        summary = {"%s_%s" % (args.scheme, args.precision): [round(ms / max(args.steps, 1), 3),
+                                                             round(roof["frac"], 4) if roof else None,
+                                                             clocks.get("sm_mhz"), clocks.get("power_w")]}
+        for k, v in variants.items():
+            summary[k] = [round(v["ms_per_step"], 3), round(v["roofline_frac"], 4) if v["roofline_frac"] else None,
+                          v["clocks"].get("sm_mhz"), v["clocks"].get("power_w")]
+        line["variants_summary"] = summary
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()

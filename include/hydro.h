@@ -88,9 +88,11 @@ int hydro_create(hydro_ctx **out, int nx, int ny, int nz, double dx, int scheme)
  *                   march amortises the one redundant flux and the pipeline fill of a chunk)
  *   "profile"       0 (default) | 1: record a CUDA event pair on the stream around every stage-kernel
  *                   launch, read back with hydro_stage_kernel_time
- *   "graph"         0 (default) | 1: hydro_step_cfl replays one steady-state step from a CUDA graph (one
- *                   cudaGraphLaunch instead of 11 kernel launches per step; every step-dependent value, dt included,
- *                   lives in the device control block).  Needs a non-default stream (hydro_set_stream) and the
+ *   "graph"         0 (default) | 1: hydro_step_cfl(ctx, cfl, k) replays its k steady-state steps from ONE CUDA graph
+ *                   (one cudaGraphLaunch instead of 11 k kernel launches, in pieces of at most 64 steps; every
+ *                   step-dependent value, dt included, lives in the device control block; one graph per (cfl, k), the
+ *                   six most recent are kept).  hydro_step_cfl_batch gives each context all its steps in one launch
+ *                   once every context of the batch can replay.  Needs a non-default stream (hydro_set_stream) and the
  *                   marching kernels; on the legacy default stream, with "profile" on, or while the control block
  *                   does not yet hold the max signal speed of u^n (i.e. before the stage-3 epilogue of a first plain
  *                   step, or hydro_max_signal_speed, has left it there) the plain launches run instead.  The

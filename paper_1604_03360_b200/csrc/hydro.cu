@@ -56,11 +56,12 @@ struct hydro_ctx {
     // "profile" option: CUDA events around every stage-kernel launch (bench.py roofline)
     int profile = 0;
     std::vector<cudaEvent_t> ev;  // pairs (start, stop), recorded on the stream
-    // "graph" option: one steady-state step of hydro_step_cfl captured as a CUDA graph and replayed (N4); one graph
-    // per value of cfl.
+    // "graph" option: k consecutive steady-state steps of hydro_step_cfl captured as ONE CUDA graph and replayed with
+    // one cudaGraphLaunch (N4: "the whole multi-step loop in one graph"); one graph per (cfl, k), a few kept.
     struct StepGraph {
         cudaGraphExec_t exec;
         double cfl;
+        int nsteps;
         long long launches;
     };
     int use_graph = 0;
@@ -387,10 +388,26 @@ bool graph_ready(const hydro_ctx* c) {
     return c->use_graph && !c->profile && c->stream != nullptr && want_fused(c) && c->max_ready;
 }
 
+// Steps of one graph at most (a step is 11 kernel nodes), and graphs kept per context (the oldest is dropped).
+constexpr int GRAPH_MAX_STEPS = 64;
+constexpr size_t GRAPH_KEEP = 6;
+
 template <class T>
-int graph_step(hydro_ctx* c, double cfl) {
+int plain_steps(hydro_ctx* c, double cfl, int nsteps) {
+    for (int s = 0; s < nsteps; ++s) {
+        const int rc = do_step<T>(c, -1.0, cfl);
+        if (rc) return rc;
+    }
+    return HYDRO_OK;
+}
+
+// nsteps (<= GRAPH_MAX_STEPS) steady-state steps with ONE cudaGraphLaunch.  Every step reads u^n from and writes
+// u^{n+1} to the same buffer, and dt, t and the max signal speed live in the control block, so the k-step graph is
+// the one-step sequence of nodes k times over.
+template <class T>
+int graph_steps(hydro_ctx* c, double cfl, int nsteps) {
     for (const auto& g : c->graphs)
-        if (g.cfl == cfl) {
+        if (g.cfl == cfl && g.nsteps == nsteps) {
             CUDA_OK(c, cudaGraphLaunch(g.exec, c->stream));
             c->launches += g.launches;
             return HYDRO_OK;
@@ -400,30 +417,35 @@ int graph_step(hydro_ctx* c, double cfl) {
     if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
         cudaGetLastError();
         c->use_graph = 0;   // e.g. the legacy default stream: fall back to plain launches for good
-        return do_step<T>(c, -1.0, cfl);
+        return plain_steps<T>(c, cfl, nsteps);
     }
-    const int rc = do_step<T>(c, -1.0, cfl);
+    const int rc = plain_steps<T>(c, cfl, nsteps);
     cudaGraph_t graph = nullptr;
     const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
     hydro_ctx::StepGraph g;
     g.cfl = cfl;
+    g.nsteps = nsteps;
     g.launches = c->launches - l0;
     c->launches = l0;
     if (rc != HYDRO_OK || e != cudaSuccess || graph == nullptr) {
         if (graph) cudaGraphDestroy(graph);
         cudaGetLastError();
         c->use_graph = 0;
-        return rc != HYDRO_OK ? rc : do_step<T>(c, -1.0, cfl);
+        return rc != HYDRO_OK ? rc : plain_steps<T>(c, cfl, nsteps);
     }
     const cudaError_t ei = cudaGraphInstantiate(&g.exec, graph, 0);
     cudaGraphDestroy(graph);
     if (ei != cudaSuccess) {
         cudaGetLastError();
         c->use_graph = 0;
-        return do_step<T>(c, -1.0, cfl);
+        return plain_steps<T>(c, cfl, nsteps);
+    }
+    if (c->graphs.size() >= GRAPH_KEEP) {
+        cudaGraphExecDestroy(c->graphs.front().exec);
+        c->graphs.erase(c->graphs.begin());
     }
     c->graphs.push_back(g);
-    return graph_step<T>(c, cfl);
+    return graph_steps<T>(c, cfl, nsteps);
 }
 
 // z-halo planes of one state buffer <-> a packed device buffer [5][g][ny][nx] (slab decomposition, DESIGN 9).
@@ -698,10 +720,14 @@ int hydro_step_cfl(hydro_ctx* c, double cfl, int nsteps) {
     DeviceGuard dg(c);
     if (!(cfl > 0) || nsteps < 0) return fail(c, HYDRO_EINVAL, "hydro_step_cfl: cfl <= 0 or nsteps < 0");
     if (c->stage_open) return fail(c, HYDRO_EINVAL, "hydro_step_cfl inside a hydro_step_stage sequence");
-    for (int s = 0; s < nsteps; ++s) {
-        if (graph_ready(c)) rc = c->precision == HYDRO_F64 ? graph_step<double>(c, cfl) : graph_step<float>(c, cfl);
-        else rc = c->precision == HYDRO_F64 ? do_step<double>(c, -1.0, cfl) : do_step<float>(c, -1.0, cfl);
+    for (int s = 0; s < nsteps;) {
+        int k = 1;
+        if (graph_ready(c)) {   // all the steps that are left (in pieces of GRAPH_MAX_STEPS) from one graph launch each
+            k = nsteps - s < GRAPH_MAX_STEPS ? nsteps - s : GRAPH_MAX_STEPS;
+            rc = c->precision == HYDRO_F64 ? graph_steps<double>(c, cfl, k) : graph_steps<float>(c, cfl, k);
+        } else rc = c->precision == HYDRO_F64 ? do_step<double>(c, -1.0, cfl) : do_step<float>(c, -1.0, cfl);
         if (rc) return rc;
+        s += k;
     }
     return HYDRO_OK;
 }
@@ -731,12 +757,17 @@ int hydro_step_cfl_batch(hydro_ctx** ctxs, int nctx, double cfl, int nsteps) {
     if (!ctxs || nctx < 0) return HYDRO_EINVAL;
     for (int i = 0; i < nctx; ++i)
         if (!ctxs[i]) return HYDRO_EINVAL;
-    // step by step over the batch, so that the launches of the contexts interleave on their streams
-    for (int s = 0; s < nsteps; ++s)
+    // step by step over the batch, so that the launches of the contexts interleave on their streams; once every
+    // context can replay from a graph, each gets all its remaining steps at once (one graph launch per context)
+    for (int s = 0; s < nsteps; ++s) {
+        bool all_graph = nctx > 0;
+        for (int i = 0; i < nctx; ++i) all_graph = all_graph && graph_ready(ctxs[i]);
         for (int i = 0; i < nctx; ++i) {
-            const int rc = hydro_step_cfl(ctxs[i], cfl, 1);
+            const int rc = hydro_step_cfl(ctxs[i], cfl, all_graph ? nsteps - s : 1);
             if (rc) return rc;
         }
+        if (all_graph) break;
+    }
     return HYDRO_OK;
 }
 

@@ -95,3 +95,28 @@ def test_batched_events_equal_their_stand_alone_runs(B, oracle, scheme):
         assert reldiff(got.cpu().numpy(), ro) <= 1e-10
         h.close()
     assert not torch.equal(want[0], want[1])
+
+
+def test_many_steps_from_one_graph_launch_in_pieces(B, oracle):
+    """N4 as SURVEY 8(f) words it: the whole k-step loop of hydro_step_cfl from one graph launch (pieces of 64 steps).
+    70 steps = one 64-step graph + one 6-step graph: bit-identical to 71 plain steps, same launch count, and the
+    oracle's state within 1e-9."""
+    w = small_workload(W.WENO5, (24, 20, 16))
+    o = oracle.from_workload(w)
+    oracle.run(o, w, nsteps=71)
+    plain = B.from_workload(w)
+    plain.step_cfl(0.2, 71)
+    want, t_want, n_want = plain.get_state(), plain.time, plain.launch_count
+    plain.close()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        h = B.from_workload(w)
+        h.set_option("graph", 1)
+        h.step_cfl(0.2, 1)
+        h.step_cfl(0.2, 70)
+        got = h.get_state()
+        side.synchronize()
+        assert torch.equal(got, want) and h.time == t_want and h.launch_count == n_want
+        assert reldiff(got.cpu().numpy(), o.get_state()) <= 1e-9
+        assert h.status() == 0
+        h.close()
