@@ -42,11 +42,13 @@ SCHEMES = {"weno5": W.WENO5, "weno7": W.WENO7, "musta": W.MUSTA_FORCE}
 FLOPS_PER_CELL_STEP = {"weno5": 7041.0, "weno7": 14331.0, "musta": 3831.0}
 FLOPS_PER_CELL_L = {"weno5": 2327.0, "weno7": 4757.0, "musta": 1257.0}
 BYTES_PER_CELL_STEP = {"f64": 320.0, "f32": 160.0}
-# DRAM bytes of one stage (x/z kernel + y sweep), dram__bytes_read.sum + dram__bytes_write.sum of one
-# `ncu --set full` capture of each kernel at 512^3 (profiles/r02_*_ncu.txt); algorithmic bytes of one stage at that
-# size: 320/3 B x 512^3 = 1.43e10
-TRAFFIC_BYTES_PER_STAGE = {("musta", "f64", 512): 27.61e9, ("weno5", "f64", 512): 27.6e9, ("weno7", "f64", 512): 27.6e9}
-# (the captured launches are the first stage of a step, which does not read u^n: stages 2 and 3 add 5.4e9 each)
+# DRAM bytes of one stage (x/z kernel + y sweep) = dram__bytes_read.sum + dram__bytes_write.sum of both launches, per
+# scheme and per Runge-Kutta stage, from the ncu pass over a whole step of each scheme at 512^3
+# (profiles/r03_traffic.md, raw lists profiles/r03_traffic_<scheme>.csv).  Stage 1 does not read u^n; stages 2 and 3
+# do (+5.4e9).  Algorithmic bytes per stage at that size: 80 / 120 / 120 B x 512^3 = 1.07e10 / 1.61e10 / 1.61e10.
+TRAFFIC_BYTES_PER_STAGE = {("weno5", "f64", 512): (27.59e9, 33.10e9, 32.97e9),
+                           ("weno7", "f64", 512): (27.59e9, 33.09e9, 33.05e9),
+                           ("musta", "f64", 512): (27.61e9, 33.06e9, 32.92e9)}
 KERNEL_NAMES = {"weno5": "weno_xz_kernel<T,3> + weno_y_kernel<T,3,EPI>", "weno7": "weno_xz_kernel<T,4> + weno_y_kernel<T,4,EPI>",
                 "musta": "musta_xz_kernel<T,FAST> + musta_y_kernel<T,EPI,FAST>"}
 METRIC = "3D cell-updates/s per RK3 step"
@@ -315,9 +317,12 @@ def roofline(scheme, precision, ncell, stage_ms, stage_n, alu_peak_tf, peaks, pr
     byts = BYTES_PER_CELL_STEP[precision] / 3.0 * ncell
     r = {"bound": "alu", "achieved": achieved, "peak": alu_peak_tf, "unit": "TFLOP/s",
          "frac": achieved / alu_peak_tf, "frac_is": "of the NOMINAL fp peak (clocks.max.sm)",
-         "traffic": TRAFFIC_BYTES_PER_STAGE.get((scheme, precision, round(ncell ** (1.0 / 3.0)))),
-         "traffic_note": "DRAM bytes of one stage (both kernels) from the ncu --set full captures under profiles/; "
-                         "algorithmic bytes of one stage: %.3g" % byts,
+         "traffic": (lambda t: sum(t) / 3.0 if t else None)(
+             TRAFFIC_BYTES_PER_STAGE.get((scheme, precision, round(ncell ** (1.0 / 3.0))))),
+         "traffic_per_stage": TRAFFIC_BYTES_PER_STAGE.get((scheme, precision, round(ncell ** (1.0 / 3.0)))),
+         "traffic_note": "DRAM bytes (read + write, both kernels) of one stage launch: mean over the three stages of a "
+                         "step, and stage 1 / 2 / 3 beside it, from the ncu pass of this scheme under "
+                         "profiles/r03_traffic.md; algorithmic bytes of a mean stage: %.3g" % byts,
          "kernel": "one RK stage = %s, timed together with one CUDA-event pair on the stream" % KERNEL_NAMES[scheme],
          "launch_ms": per_launch_s * 1e3, "algorithmic_flops_per_launch": flops,
          "hbm_gbs_achieved": byts / per_launch_s / 1e9, "hbm_frac": byts / per_launch_s / 1e9 / peaks["hbm_gbs"]}
