@@ -122,10 +122,10 @@ def _planes(nz):
     return [math.sin(0.7 * k) + 0.05 * k for k in range(nz)]
 
 
-def _step_worker(rank, world, port, bc, nz, nsteps, overlap, out):
+def _step_worker(rank, world, port, bc, nz, nsteps, overlap, out, bounds=None):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group("gloo", rank=rank, world_size=world)
-    k0, k1 = S.split_planes(nz, world)[rank]
+    k0, k1 = (bounds or S.split_planes(nz, world))[rank]
     h = FakeHydro(_planes(nz)[k0:k1])
     S.SlabGroup([h], S.DistComm(dist, bc), 1.0).step_cfl(0.1, nsteps, overlap=overlap)
     out[rank] = (h.interior().tolist(), h.calls[:9])
@@ -152,6 +152,22 @@ def test_step_cfl_control_flow_over_gloo_two_ranks(bc, overlap):
     # per stage: both ghost sides of the stage's input buffer are written, then the stage runs
     assert res[0][1] == [("put", 0, 0), ("put", 0, 1), ("stage", 0), ("put", 1, 0), ("put", 1, 1), ("stage", 1),
                          ("put", 2, 0), ("put", 2, 1), ("stage", 2)]
+
+
+@pytest.mark.parametrize("bc", [S.BC_PERIODIC, S.BC_OUTFLOW])
+def test_very_unequal_slabs_over_gloo_two_ranks(bc):
+    """The same with slabs of 8 and 3 planes (nothing in the exchange may assume equal slabs: a slab only ever sends
+    and receives g planes per side) through the overlap call, zero-gradient ends or the ring of two."""
+    nz, nsteps, world = 11, 4, 2
+    one = FakeHydro(_planes(nz))
+    S.SlabGroup([one], S.LocalComm(1, bc), 1.0).step_cfl(0.1, nsteps, overlap=True)
+    port = 35600 + os.getpid() % 2000 + bc
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_step_worker, args=(world, port, bc, nz, nsteps, True, out, [(0, 8), (8, 11)]), nprocs=world, join=True)
+        res = dict(out)
+    assert len(res[0][0]) == 8 and len(res[1][0]) == 3
+    assert res[0][0] + res[1][0] == one.interior().tolist()
 
 
 # ------------------------------------------------------------------ GPU: bit-identity with the undecomposed run
